@@ -1,0 +1,166 @@
+/* include/mdwf.h -- C-ABI boundary of the B200-native MDWF hot path (libmdwf.so).
+ *
+ * What it is.  The paper (reference PAPER.md) names its method only: "Moebius Domain-Wall
+ * discretization", a "radius-one stencil" with "12x12 dense" spin-colour blocks,
+ * a "red-black preconditioned" operator solved by "CG on the normal equations" in "double-half"
+ * mixed precision with "reliable updates", Feynman-Hellmann propagators
+ * and nucleon contractions.  The operator definitions used here
+ * are the readings fixed in SURVEY.md section 8 ("Notation", A1-A23) and restated in DESIGN.md.
+ *
+ * Conventions for every call
+ *  - returns int: 0 = MDWF_OK, <0 = error, >0 = soft status.  Nothing throws or exits.
+ *    mdwf_last_error(ctx) gives a message owned by ctx (valid until the next call on ctx).
+ *  - every data pointer is a DEVICE pointer owned by the caller unless the name ends in _host.
+ *    The library never frees or retains caller memory past the call; mdwf_load_gauge and
+ *    mdwf_field_pack make their own packed copies.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Calls are
+ *    asynchronous on it, except mdwf_solve* (host-visible info => synchronises before returning)
+ *    and the *_host variants.
+ *  - canonical interchange layouts (fp64, x fastest): x4 = x + X*(y + Y*(z + Z*t));
+ *      5D spinor  psi[rhs][s][site][spin 4][colour 3][re,im]   site = x4 (full lattice) or
+ *                                                              xh = x4>>1 over the sites of one parity
+ *      gauge      U[mu][x4][row 3][col 3][re,im]               U_mu(x) = link from x to x+mu
+ *      4D field   eta[col][x4][spin][colour][re,im]            col = 3*spin_src + colour_src
+ *  - there is no CPU fallback: every entry point needs a CUDA device.
+ */
+#ifndef MDWF_H
+#define MDWF_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MDWF_OK 0
+#define MDWF_EINVAL (-1)
+#define MDWF_ENOMEM (-2)
+#define MDWF_ECUDA (-3)
+#define MDWF_ESTATE (-4)
+#define MDWF_NOT_CONVERGED 1
+#define MDWF_BREAKDOWN 2
+
+/* operators of mdwf_dslash (SURVEY 8 "Even-odd form"; a = b5(4-M5)+1, d = c5(4-M5)-1):
+ *   HOP        H_{p <- pbar}                 4D Wilson hopping stencil on every s slice
+ *   M4PRE      A  = b5 + c5 L                (s-direction, 4D-site local)
+ *   M5         M5 = a + d L                  ("Ls-direction M5/mass coupling", north_star)
+ *   M5INV      M5^-1
+ *   DHAT_ASYM  Dhat = M5 - 1/4 H A M5^-1 H A          (red-black Schur complement)
+ *   DHAT_SYM   Mhat = M5^-1 Dhat
+ *   NORMAL_ASYM / NORMAL_SYM   Dhat^dag Dhat / Mhat^dag Mhat   (the CG operator)
+ *   FULL       D = M5 - 1/2 H A on the full lattice (both parities)                        */
+enum { MDWF_OP_HOP = 0, MDWF_OP_M4PRE = 1, MDWF_OP_M5 = 2, MDWF_OP_M5INV = 3, MDWF_OP_DHAT_ASYM = 4,
+       MDWF_OP_DHAT_SYM = 5, MDWF_OP_NORMAL_ASYM = 6, MDWF_OP_NORMAL_SYM = 7, MDWF_OP_FULL = 8 };
+
+typedef struct mdwf_ctx mdwf_ctx;
+typedef struct mdwf_field mdwf_field;
+
+typedef struct {
+    int32_t dims[4]; /* X,Y,Z,T: all even, >= 2                                   */
+    int32_t Ls;      /* >= 1, <= 32                                               */
+    int32_t bc[4];   /* +1 periodic, -1 antiperiodic (runs use {1,1,1,-1})        */
+    int32_t device;  /* CUDA device ordinal                                       */
+} mdwf_geometry;
+
+/* Create a context for one lattice geometry and one set of Moebius parameters (north_star:
+ * mdwf_create(geometry, M5, b5, c5, mf)).  Precomputes the Ls x Ls chirality blocks of A, M5, M5^-1
+ * (closed form, SURVEY 8 Notation) and their products.  EINVAL: odd/too small extent, Ls out of range. */
+int mdwf_create(mdwf_ctx** out, const mdwf_geometry* g, double M5, double b5, double c5, double mf);
+int mdwf_destroy(mdwf_ctx* ctx);
+const char* mdwf_last_error(const mdwf_ctx* ctx);
+
+/* Pack the canonical fp64 gauge field (device pointer) into the even/odd-split device format
+ * {store_prec 64|32|16} x {recon 18|12|8 reals per link} (north_star "gauge-field ... layout/packing,
+ * with optional 12/8-parameter link reconstruction and fp16/fp32 storage"; formats: SURVEY A12).
+ * May be called repeatedly: each (store_prec, recon) pair stays resident until destroy.
+ * The boundary sign bc is never stored in a link; kernels apply it after reconstruction.
+ * recon 8 cannot represent links with |U01|^2+|U02|^2 -> 0 (e.g. unit links): EINVAL, nothing loaded. */
+int mdwf_load_gauge(mdwf_ctx* ctx, const void* U, int store_prec, int recon, void* stream);
+
+/* out = op(in) on `nrhs` canonical fp64 fields (device).  Half-lattice ops (everything but FULL)
+ * take/return half-lattice fields [rhs][s][xh][4][3][2]; `parity` is the parity of the OUTPUT sites
+ * (HOP reads the other parity, all other ops read the same parity).  FULL takes/returns
+ * full-lattice fields [rhs][s][x4][4][3][2] and ignores parity.  `prec` 64|32|16 selects the storage
+ * precision of every packed spinor and of the links (compute is fp64 for 64, fp32 otherwise);
+ * (prec, recon) must have been loaded.  This is pack -> packed kernels -> unpack; the parity tests
+ * call it.  For NORMAL_* `dagger` is ignored. */
+int mdwf_dslash(mdwf_ctx* ctx, int op, int parity, int dagger, int prec, int recon, void* out,
+                const void* in, int nrhs, void* stream);
+
+/* Packed fields for timing loops (canonical<->packed conversion stays outside the timed region). */
+int mdwf_field_create(mdwf_ctx* ctx, int prec, int nrhs, mdwf_field** out);
+int mdwf_field_destroy(mdwf_field* f);
+/* canonical half-lattice fp64 [rhs][s][xh][4][3][2] (device) <-> packed */
+int mdwf_field_pack(mdwf_field* f, const void* canonical, void* stream);
+int mdwf_field_unpack(const mdwf_field* f, void* canonical, void* stream);
+/* out = op(in) on packed half-lattice fields of equal prec/nrhs (op != FULL); out must not alias in. */
+int mdwf_dslash_packed(mdwf_ctx* ctx, int op, int parity, int dagger, int recon, mdwf_field* out,
+                       const mdwf_field* in, void* stream);
+/* algorithmic bytes / flops of one mdwf_dslash_packed(op) call under DESIGN.md's convention
+ * (SURVEY 8(d), A19): returns 0 and fills *bytes, *flops. */
+int mdwf_dslash_cost(const mdwf_ctx* ctx, int op, int prec, int recon, int nrhs, double* bytes, double* flops);
+
+typedef struct {
+    double tol;          /* target ||b - D psi|| / ||b|| (full system, fp64)                        */
+    int32_t max_iter;    /* cap on inner CG iterations per rhs                                       */
+    int32_t inner_prec;  /* 64 | 32 | 16: storage precision of the inner CG vectors and links        */
+    int32_t recon;       /* link format used by the inner operator (outer fp64 uses 18 if loaded,
+                            else the same recon)                                                     */
+    int32_t parity;      /* parity p that is solved (the other one is reconstructed)                 */
+    int32_t symmetric;   /* 0: Dhat, 1: Mhat = M5^-1 Dhat                                            */
+    double delta;        /* reliable-update threshold, <=0 -> 0.1                       */
+    int32_t src_kind;    /* 0: b is a 5D full-lattice field; 1: b is a 4D source, wall-injected (O3) */
+    int32_t out_kind;    /* 0: x is the 5D solution; 1: x is the 4D wall projection q (O3)           */
+    int32_t batch;       /* max rhs solved concurrently (0 = as many as fit in free device memory)   */
+    int32_t check_every; /* host convergence check period in iterations (<=0 -> 1)                   */
+} mdwf_solve_opts;
+
+#define MDWF_MAX_RHS 64
+typedef struct {
+    int32_t iters[MDWF_MAX_RHS];
+    int32_t reliable_updates[MDWF_MAX_RHS];
+    int32_t status[MDWF_MAX_RHS];      /* MDWF_OK | MDWF_NOT_CONVERGED | MDWF_BREAKDOWN per rhs */
+    double true_resid[MDWF_MAX_RHS];   /* ||bhat - Dhat psi_p|| / ||b|| in fp64 = full-system residual */
+    double seconds;                    /* device time of the whole call (CUDA events)                 */
+    double seconds_inner;              /* device time spent in inner (low precision) iterations       */
+    int64_t kernel_launches;           /* kernels launched by this call                               */
+} mdwf_solve_info;
+
+/* Solve D psi = b for nrhs (<= MDWF_MAX_RHS) right-hand sides by even-odd preconditioning +
+ * batched mixed-precision CG on the normal equations with reliable updates (
+ * SURVEY 8(a) a7-a9, A9, A10, A20).  b, x: canonical fp64 device fields; 5D full-lattice
+ * [rhs][s][x4][4][3][2] or 4D [rhs][x4][4][3][2] per src_kind/out_kind.  x may alias b only if both are
+ * 5D.  Returns MDWF_OK, or MDWF_NOT_CONVERGED / MDWF_BREAKDOWN if any rhs ended that way. */
+int mdwf_solve(mdwf_ctx* ctx, void* x, const void* b, int nrhs, const mdwf_solve_opts* opts,
+               mdwf_solve_info* info, void* stream);
+/* Same with HOST buffers (pageable or pinned): the call stages each batch host->device, solves,
+ * and copies the result back; all copies are inside the call. */
+int mdwf_solve_host(mdwf_ctx* ctx, void* x_host, const void* b_host, int nrhs, const mdwf_solve_opts* opts,
+                    mdwf_solve_info* info, void* stream);
+
+/* Feynman-Hellmann sequential source:
+ * out4d[col](x) = Gamma . prop4d[col](x) on timeslices t_min <= t <= t_max (all t = "sum over t"),
+ * zero elsewhere.  Gamma: 4x4 complex, row-major [re,im], HOST pointer.  ncol columns of
+ * canonical 4D fields [col][x4][4][3][2] fp64 (device).  out4d may alias prop4d. */
+int mdwf_seq_source(mdwf_ctx* ctx, void* out4d, const void* prop4d, int ncol, const double* Gamma_host,
+                    int t_min, int t_max, void* stream);
+
+/* Nucleon two-point function (SURVEY a11, O4 C-def, A15).  Three 12-column 4D
+ * propagators (device, canonical): S_u1 (diquark u), S_d, S_u2 (spectator u); proj: 4x4 complex
+ * HOST; corr: device double [T][2], index (t - t0) mod T, overwritten. */
+int mdwf_nucleon_2pt(mdwf_ctx* ctx, double* corr, const void* S_u1, const void* S_d, const void* S_u2,
+                     const double* proj_host, int t0, void* stream);
+
+/* 4D <-> 5D maps of SURVEY O3 as stand-alone calls (used by the tests; mdwf_solve applies them
+ * itself for src_kind/out_kind = 1):  b5 = -D_- (P+ eta @ s=0 (+) P- eta @ s=Ls-1),
+ * q = P- psi_0 + P+ psi_{Ls-1}.  Full-lattice canonical fp64 device fields. */
+int mdwf_wall_inject(mdwf_ctx* ctx, void* b5, const void* eta4, int ncol, int recon, void* stream);
+int mdwf_wall_project(mdwf_ctx* ctx, void* q4, const void* psi5, int ncol, void* stream);
+
+/* number of kernels this context has launched so far (bench.py's gpu_launches) */
+int64_t mdwf_launch_count(const mdwf_ctx* ctx);
+/* set the z-slab depth of the hop kernel's site traversal (L2 tiling); 0 = automatic */
+int mdwf_set_tiling(mdwf_ctx* ctx, int zc);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,376 @@
+// csrc/api.cu -- the C-ABI entry points declared in include/mdwf.h (context, gauge load, Dslash family,
+// packed fields) and the composite even-odd operators built from the fused kernels.
+#include "mdwf_host.h"
+#include <cmath>
+#include <cstring>
+#include <algorithm>
+
+using namespace mdwf;
+
+// ---------------------------------------------------------------------------------------------
+// Ls x Ls chirality blocks (SURVEY 8 Notation): L+ [s][s-1] = 1, L+ [0][Ls-1] = -mf ; L- [s][s+1] = 1,
+// L- [Ls-1][0] = -mf ; A = b5 + c5 L ; M5 = a + d L ; M5^-1 by its closed form
+//   (M5^-1)+[s][s'] = kappa^{(s-s') mod Ls} (s >= s' ? 1 : -mf) / (a (1 + mf kappa^Ls)),  kappa = -d/a
+//   (M5^-1)-[s][s'] = kappa^{(s'-s) mod Ls} (s' >= s ? 1 : -mf) / (a (1 + mf kappa^Ls)).
+// dagger = transpose inside each chirality block.
+// ---------------------------------------------------------------------------------------------
+static void build_matrices(int Ls, double M5, double b5, double c5, double mf, std::vector<double> mats[MAT_COUNT]) {
+    const double a = b5 * (4.0 - M5) + 1.0, d = c5 * (4.0 - M5) - 1.0, kappa = -d / a;
+    const int n = Ls * Ls;
+    std::vector<double> L[2], A[2], M[2], Mi[2], AMi[2];
+    for (int ch = 0; ch < 2; ++ch) {
+        L[ch].assign(n, 0.0);
+        for (int s = 0; s < Ls; ++s) {
+            if (ch == 0) { if (s >= 1) L[0][s * Ls + s - 1] += 1.0; else L[0][0 * Ls + Ls - 1] += -mf; }
+            else { if (s + 1 < Ls) L[1][s * Ls + s + 1] += 1.0; else L[1][(Ls - 1) * Ls + 0] += -mf; }
+        }
+        A[ch].assign(n, 0.0);
+        M[ch].assign(n, 0.0);
+        Mi[ch].assign(n, 0.0);
+        AMi[ch].assign(n, 0.0);
+        const double den = a * (1.0 + mf * std::pow(kappa, Ls));
+        for (int s = 0; s < Ls; ++s)
+            for (int t = 0; t < Ls; ++t) {
+                const double id = s == t ? 1.0 : 0.0;
+                A[ch][s * Ls + t] = b5 * id + c5 * L[ch][s * Ls + t];
+                M[ch][s * Ls + t] = a * id + d * L[ch][s * Ls + t];
+                const int k = ch == 0 ? ((s - t) % Ls + Ls) % Ls : ((t - s) % Ls + Ls) % Ls;
+                const bool nowrap = ch == 0 ? (s >= t) : (t >= s);
+                Mi[ch][s * Ls + t] = std::pow(kappa, k) * (nowrap ? 1.0 : -mf) / den;
+            }
+        for (int s = 0; s < Ls; ++s)
+            for (int t = 0; t < Ls; ++t) {
+                double acc = 0.0;
+                for (int k = 0; k < Ls; ++k) acc += A[ch][s * Ls + k] * Mi[ch][k * Ls + t];
+                AMi[ch][s * Ls + t] = acc;
+            }
+    }
+    // device layout Gt[chi][s'][s] = Mat_chi[s][s'] ; dagger: Mat_chi[s'][s]
+    std::vector<double>* src[4] = {A, M, Mi, AMi};
+    const int ids[4] = {MAT_A, MAT_M5, MAT_M5INV, MAT_AM5INV};
+    for (int m = 0; m < 4; ++m) {
+        mats[ids[m]].assign(2 * n, 0.0);
+        mats[ids[m] + 4].assign(2 * n, 0.0);
+        for (int ch = 0; ch < 2; ++ch)
+            for (int s = 0; s < Ls; ++s)
+                for (int t = 0; t < Ls; ++t) {
+                    mats[ids[m]][ch * n + t * Ls + s] = src[m][ch][s * Ls + t];
+                    mats[ids[m] + 4][ch * n + t * Ls + s] = src[m][ch][t * Ls + s];
+                }
+    }
+}
+
+static int pick_zc(const mdwf_ctx* c, int want) {
+    const Geom& g = c->g;
+    if (want > 0 && g.Z % want == 0) return want;
+    // automatic: deepest z-slab whose three-timeslice working set (input gathers + output) of ~4 fp32 rhs
+    // stays within ~1/2 of L2; small lattices use the canonical order (zc = Z)
+    const double per_site = (double)g.Ls * 96.0 * 2.0 * 4.0;
+    int best = 1;
+    for (int z = 1; z <= g.Z; ++z)
+        if (g.Z % z == 0 && 3.0 * g.XH * g.Y * z * per_site <= 48e6) best = z;
+    return best;
+}
+static void set_zc(mdwf_ctx* c, int zc) {
+    Geom& g = c->g;
+    g.zc = zc;
+    g.dZc = make_fastdiv(zc);
+    g.dSlab = make_fastdiv((uint32_t)(g.XH * g.Y * zc));
+    g.dTslab = make_fastdiv((uint32_t)(g.XH * g.Y * zc) * (uint32_t)g.T);
+}
+
+extern "C" {
+
+int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, double c5, double mf) {
+    if (!out || !geo) return MDWF_EINVAL;
+    *out = nullptr;
+    mdwf_ctx* c = new mdwf_ctx;
+    c->geo = *geo;
+    c->M5 = M5; c->b5 = b5; c->c5 = c5; c->mf = mf;
+    c->partial = nullptr; c->dscal = nullptr; c->hscal = nullptr; c->launches = 0;
+    for (int i = 0; i < MAT_COUNT; ++i) c->mat_d[i] = c->mat_f[i] = nullptr;
+    *out = c;   // returned even on failure so that mdwf_last_error can be read; caller destroys it
+    long long v4 = 1;
+    for (int m = 0; m < 4; ++m) {
+        if (geo->dims[m] < 2 || (geo->dims[m] & 1)) MDWF_FAIL(c, MDWF_EINVAL, "extent %d of direction %d must be even and >= 2", geo->dims[m], m);
+        if (geo->bc[m] != 1 && geo->bc[m] != -1) MDWF_FAIL(c, MDWF_EINVAL, "bc[%d] must be +1 or -1", m);
+        v4 *= geo->dims[m];
+    }
+    if (geo->Ls < 1 || geo->Ls > 32) MDWF_FAIL(c, MDWF_EINVAL, "Ls must be in 1..32 (got %d)", geo->Ls);
+    if (v4 / 2 * geo->Ls >= (1ll << 31) / 2) MDWF_FAIL(c, MDWF_EINVAL, "lattice too large for 32-bit 5D site indices");
+    const double a = b5 * (4.0 - M5) + 1.0;
+    if (a == 0.0) MDWF_FAIL(c, MDWF_EINVAL, "b5(4-M5)+1 must be non-zero");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        MDWF_FAIL(c, MDWF_ECUDA, "no CUDA device: libmdwf has no CPU fallback");
+    }
+    if (geo->device < 0 || geo->device >= ndev) MDWF_FAIL(c, MDWF_EINVAL, "device %d out of range (%d devices)", geo->device, ndev);
+    MDWF_CUDA(c, cudaSetDevice(geo->device));
+    cudaDeviceProp prop;
+    MDWF_CUDA(c, cudaGetDeviceProperties(&prop, geo->device));
+    c->sm_count = prop.multiProcessorCount;
+    Geom& g = c->g;
+    g.X = geo->dims[0]; g.Y = geo->dims[1]; g.Z = geo->dims[2]; g.T = geo->dims[3];
+    g.XH = g.X / 2; g.Ls = geo->Ls;
+    g.Vh = (int)(v4 / 2);
+    g.N5h = g.Vh * g.Ls;
+    for (int m = 0; m < 4; ++m) g.bc[m] = geo->bc[m];
+    g.dLs = make_fastdiv(g.Ls); g.dXH = make_fastdiv(g.XH); g.dY = make_fastdiv(g.Y); g.dZ = make_fastdiv(g.Z);
+    set_zc(c, pick_zc(c, 0));
+    c->block = (256 / g.Ls) * g.Ls;
+    c->nblk = (g.N5h + c->block - 1) / c->block;
+    MDWF_CUDA(c, cudaMalloc(&c->partial, sizeof(double) * 64 * (size_t)c->nblk));
+    MDWF_CUDA(c, cudaMalloc(&c->dscal, sizeof(double) * 8 * 64));
+    MDWF_CUDA(c, cudaMemset(c->dscal, 0, sizeof(double) * 8 * 64));
+    MDWF_CUDA(c, cudaHostAlloc(&c->hscal, sizeof(double) * 8 * 64, cudaHostAllocDefault));
+    std::vector<double> mats[MAT_COUNT];
+    build_matrices(g.Ls, M5, b5, c5, mf, mats);
+    for (int i = 0; i < MAT_COUNT; ++i) {
+        const size_t n = mats[i].size();
+        std::vector<float> mf32(n);
+        for (size_t k = 0; k < n; ++k) mf32[k] = (float)mats[i][k];
+        MDWF_CUDA(c, cudaMalloc(&c->mat_d[i], n * sizeof(double)));
+        MDWF_CUDA(c, cudaMalloc(&c->mat_f[i], n * sizeof(float)));
+        MDWF_CUDA(c, cudaMemcpy(c->mat_d[i], mats[i].data(), n * sizeof(double), cudaMemcpyHostToDevice));
+        MDWF_CUDA(c, cudaMemcpy(c->mat_f[i], mf32.data(), n * sizeof(float), cudaMemcpyHostToDevice));
+    }
+    return MDWF_OK;
+}
+
+int mdwf_destroy(mdwf_ctx* c) {
+    if (!c) return MDWF_OK;
+    for (size_t i = 0; i < c->gauges.size(); ++i) { cudaFree(c->gauges[i].v[0]); cudaFree(c->gauges[i].v[1]); }
+    for (auto& kv : c->temps) for (mdwf_field* f : kv.second) free_field(f);
+    for (int i = 0; i < MAT_COUNT; ++i) { if (c->mat_d[i]) cudaFree(c->mat_d[i]); if (c->mat_f[i]) cudaFree(c->mat_f[i]); }
+    if (c->partial) cudaFree(c->partial);
+    if (c->dscal) cudaFree(c->dscal);
+    if (c->hscal) cudaFreeHost(c->hscal);
+    delete c;
+    return MDWF_OK;
+}
+
+const char* mdwf_last_error(const mdwf_ctx* c) { return c ? c->err.c_str() : "null context"; }
+int64_t mdwf_launch_count(const mdwf_ctx* c) { return c ? c->launches : 0; }
+
+int mdwf_set_tiling(mdwf_ctx* c, int zc) {
+    if (!c) return MDWF_EINVAL;
+    if (zc < 0 || (zc > 0 && c->g.Z % zc != 0)) MDWF_FAIL(c, MDWF_EINVAL, "zc = %d must divide Z = %d", zc, c->g.Z);
+    set_zc(c, pick_zc(c, zc));
+    return MDWF_OK;
+}
+
+int mdwf_load_gauge(mdwf_ctx* c, const void* U, int store_prec, int recon, void* stream) {
+    if (!c) return MDWF_EINVAL;
+    if (!U) MDWF_FAIL(c, MDWF_EINVAL, "null gauge pointer");
+    GaugeSet gs;
+    int rc = pack_gauge(c, U, store_prec, recon, &gs, (cudaStream_t)stream);
+    if (rc) return rc;
+    for (size_t i = 0; i < c->gauges.size(); ++i)
+        if (c->gauges[i].prec == store_prec && c->gauges[i].recon == recon) {
+            cudaFree(c->gauges[i].v[0]);
+            cudaFree(c->gauges[i].v[1]);
+            c->gauges[i] = gs;
+            return MDWF_OK;
+        }
+    c->gauges.push_back(gs);
+    return MDWF_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+namespace mdwf {
+
+int op_ls(const OpCtx& o, const SpinorView& out, const SpinorView& in, int mat, const SpinorView* xin, double cx,
+          double ch, const RhsList& rl, double* partial, int write) {
+    LsArgs a;
+    a.out = out; a.in = in;
+    if (xin) a.xin = *xin; else { a.xin.v = nullptr; a.xin.n = nullptr; a.xin.rs = a.xin.rn = 0; }
+    a.G = mat >= 0 ? o.c->mat(mat, o.prec) : nullptr;
+    a.cx = cx; a.ch = ch; a.partial = partial; a.write = write; a.rl = rl;
+    return launch_ls(o.c, o.prec, a, o.st);
+}
+
+int op_hop(const OpCtx& o, const SpinorView& out, const SpinorView& in, int out_par, int dagger, int mat,
+           const SpinorView* xin, double cx, double ch, const RhsList& rl, double* partial) {
+    HopArgs a;
+    a.out = out; a.in = in;
+    if (xin) a.xin = *xin; else { a.xin.v = nullptr; a.xin.n = nullptr; a.xin.rs = a.xin.rn = 0; }
+    a.g.v[0] = o.gs->v[0]; a.g.v[1] = o.gs->v[1];
+    a.G = mat >= 0 ? o.c->mat(mat, o.prec) : nullptr;
+    a.cx = cx; a.ch = ch; a.partial = partial; a.par = out_par; a.nact = rl.nact;
+    for (int i = 0; i < 64; ++i) a.rhs_list[i] = rl.rhs[i];
+    const int fused = (mat >= 0 || xin || partial || ch != 1.0) ? 1 : 0;
+    return launch_hop(o.c, o.prec, o.recon, dagger, fused, a, o.st);
+}
+
+// Dhat = M5 - 1/4 H A M5^-1 H A,  Mhat = M5^-1 Dhat,  and their adjoints (SURVEY 8 "Even-odd form"):
+//   Mhat v     : t1 = A v ; t2 = (A M5^-1) H t1 ; out = v - 1/4 M5^-1 H t2
+//   Dhat v     : t1 = A v ; t2 = (A M5^-1) H t1 ; t1 = M5 v ; out = t1 - 1/4 H t2
+//   Mhat^dag v : t1 = M5^-dag v ; t2 = (A M5^-1)^dag H^dag t1 ; out = v - 1/4 A^dag H^dag t2
+//   Dhat^dag v : t2 = (A M5^-1)^dag H^dag v ; t1 = M5^dag v ; out = t1 - 1/4 A^dag H^dag t2
+int op_schur(const OpCtx& o, const SpinorView& out, const SpinorView& in, int par, int dagger, int symmetric,
+             const SpinorView& t1, const SpinorView& t2, const RhsList& rl, double* partial) {
+    int rc;
+    if (!dagger) {
+        if ((rc = op_ls(o, t1, in, MAT_A, nullptr, 0.0, 1.0, rl))) return rc;
+        if ((rc = op_hop(o, t2, t1, 1 - par, 0, MAT_AM5INV, nullptr, 0.0, 1.0, rl))) return rc;
+        if (symmetric) return op_hop(o, out, t2, par, 0, MAT_M5INV, &in, 1.0, -0.25, rl, partial);
+        if ((rc = op_ls(o, t1, in, MAT_M5, nullptr, 0.0, 1.0, rl))) return rc;
+        return op_hop(o, out, t2, par, 0, -1, &t1, 1.0, -0.25, rl, partial);
+    }
+    if (symmetric) {
+        if ((rc = op_ls(o, t1, in, MAT_M5INV_D, nullptr, 0.0, 1.0, rl))) return rc;
+        if ((rc = op_hop(o, t2, t1, 1 - par, 1, MAT_AM5INV_D, nullptr, 0.0, 1.0, rl))) return rc;
+        return op_hop(o, out, t2, par, 1, MAT_A_D, &in, 1.0, -0.25, rl, partial);
+    }
+    if ((rc = op_hop(o, t2, in, 1 - par, 1, MAT_AM5INV_D, nullptr, 0.0, 1.0, rl))) return rc;
+    if ((rc = op_ls(o, t1, in, MAT_M5_D, nullptr, 0.0, 1.0, rl))) return rc;
+    return op_hop(o, out, t2, par, 1, MAT_A_D, &t1, 1.0, -0.25, rl, partial);
+}
+
+static int make_opctx(mdwf_ctx* c, int prec, int recon, cudaStream_t st, OpCtx* o) {
+    o->c = c; o->prec = prec; o->recon = recon; o->st = st;
+    o->gs = c->find_gauge(prec, recon);
+    if (!o->gs) MDWF_FAIL(c, MDWF_ESTATE, "gauge format (prec %d, recon %d) not loaded: call mdwf_load_gauge first", prec, recon);
+    return MDWF_OK;
+}
+
+static int dslash_packed_impl(mdwf_ctx* c, int op, int parity, int dagger, int recon, mdwf_field* out,
+                              const mdwf_field* in, cudaStream_t st) {
+    if (!out || !in) MDWF_FAIL(c, MDWF_EINVAL, "null field");
+    if (out->prec != in->prec || out->nrhs != in->nrhs) MDWF_FAIL(c, MDWF_EINVAL, "in/out fields differ in precision or nrhs");
+    if (out->v == in->v) MDWF_FAIL(c, MDWF_EINVAL, "out must not alias in");
+    if (parity != 0 && parity != 1) MDWF_FAIL(c, MDWF_EINVAL, "parity must be 0 or 1");
+    const int prec = in->prec, nrhs = in->nrhs;
+    const RhsList rl = all_rhs(nrhs);
+    OpCtx o;
+    o.c = c; o.prec = prec; o.recon = recon; o.st = st; o.gs = nullptr;
+    const bool needs_gauge = !(op == MDWF_OP_M4PRE || op == MDWF_OP_M5 || op == MDWF_OP_M5INV);
+    int rc;
+    if (needs_gauge && (rc = make_opctx(c, prec, recon, st, &o))) return rc;
+    const SpinorView vi = in->view(), vo = out->view();
+    const int dg = dagger ? 4 : 0;
+    switch (op) {
+        case MDWF_OP_HOP: return op_hop(o, vo, vi, parity, dagger, -1, nullptr, 0.0, 1.0, rl);
+        case MDWF_OP_M4PRE: return op_ls(o, vo, vi, MAT_A + dg, nullptr, 0.0, 1.0, rl);
+        case MDWF_OP_M5: return op_ls(o, vo, vi, MAT_M5 + dg, nullptr, 0.0, 1.0, rl);
+        case MDWF_OP_M5INV: return op_ls(o, vo, vi, MAT_M5INV + dg, nullptr, 0.0, 1.0, rl);
+        case MDWF_OP_DHAT_ASYM:
+        case MDWF_OP_DHAT_SYM: {
+            mdwf_field *t1, *t2;
+            if ((rc = temp_field(c, prec, nrhs, 2, &t1)) || (rc = temp_field(c, prec, nrhs, 3, &t2))) return rc;
+            return op_schur(o, vo, vi, parity, dagger, op == MDWF_OP_DHAT_SYM, t1->view(), t2->view(), rl);
+        }
+        case MDWF_OP_NORMAL_ASYM:
+        case MDWF_OP_NORMAL_SYM: {
+            mdwf_field *t1, *t2, *t3;
+            if ((rc = temp_field(c, prec, nrhs, 2, &t1)) || (rc = temp_field(c, prec, nrhs, 3, &t2)) ||
+                (rc = temp_field(c, prec, nrhs, 4, &t3))) return rc;
+            const int sym = op == MDWF_OP_NORMAL_SYM;
+            if ((rc = op_schur(o, t3->view(), vi, parity, 0, sym, t1->view(), t2->view(), rl))) return rc;
+            return op_schur(o, vo, t3->view(), parity, 1, sym, t1->view(), t2->view(), rl);
+        }
+    }
+    MDWF_FAIL(c, MDWF_EINVAL, "unknown or non-packed op %d", op);
+}
+
+}  // namespace mdwf
+
+extern "C" {
+
+int mdwf_field_create(mdwf_ctx* c, int prec, int nrhs, mdwf_field** out) {
+    if (!c || !out) return MDWF_EINVAL;
+    return alloc_field(c, prec, nrhs, out);
+}
+int mdwf_field_destroy(mdwf_field* f) {
+    free_field(f);
+    return MDWF_OK;
+}
+int mdwf_field_pack(mdwf_field* f, const void* canonical, void* stream) {
+    if (!f || !canonical) return MDWF_EINVAL;
+    PackArgs a;
+    a.f = f->view(); a.canon = (double*)canonical; a.Vc = f->ctx->g.Vh; a.full = 0; a.par = 0; a.nrhs = f->nrhs; a.rhs0 = 0;
+    return launch_pack(f->ctx, f->prec, false, a, (cudaStream_t)stream);
+}
+int mdwf_field_unpack(const mdwf_field* f, void* canonical, void* stream) {
+    if (!f || !canonical) return MDWF_EINVAL;
+    PackArgs a;
+    a.f = f->view(); a.canon = (double*)canonical; a.Vc = f->ctx->g.Vh; a.full = 0; a.par = 0; a.nrhs = f->nrhs; a.rhs0 = 0;
+    return launch_pack(f->ctx, f->prec, true, a, (cudaStream_t)stream);
+}
+
+int mdwf_dslash_packed(mdwf_ctx* c, int op, int parity, int dagger, int recon, mdwf_field* out,
+                       const mdwf_field* in, void* stream) {
+    if (!c) return MDWF_EINVAL;
+    return dslash_packed_impl(c, op, parity, dagger, recon, out, in, (cudaStream_t)stream);
+}
+
+int mdwf_dslash(mdwf_ctx* c, int op, int parity, int dagger, int prec, int recon, void* out, const void* in,
+                int nrhs, void* stream) {
+    if (!c) return MDWF_EINVAL;
+    if (!out || !in) MDWF_FAIL(c, MDWF_EINVAL, "null field pointer");
+    if (nrhs < 1 || nrhs > MDWF_MAX_RHS) MDWF_FAIL(c, MDWF_EINVAL, "nrhs must be in 1..%d", MDWF_MAX_RHS);
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    if (op != MDWF_OP_FULL) {
+        mdwf_field *fi, *fo;
+        if ((rc = temp_field(c, prec, nrhs, 0, &fi)) || (rc = temp_field(c, prec, nrhs, 1, &fo))) return rc;
+        if ((rc = mdwf_field_pack(fi, in, stream))) return rc;
+        if ((rc = dslash_packed_impl(c, op, parity, dagger, recon, fo, fi, st))) return rc;
+        return mdwf_field_unpack(fo, out, stream);
+    }
+    // FULL: D = M5 - 1/2 H A ; D^dag = M5^dag - 1/2 A^dag H^dag  (SURVEY 8 "Even-odd form")
+    OpCtx o;
+    if ((rc = make_opctx(c, prec, recon, st, &o))) return rc;
+    mdwf_field *f[2], *fo, *t1, *t2;
+    if ((rc = temp_field(c, prec, nrhs, 0, &f[0])) || (rc = temp_field(c, prec, nrhs, 5, &f[1])) ||
+        (rc = temp_field(c, prec, nrhs, 1, &fo)) || (rc = temp_field(c, prec, nrhs, 2, &t1)) ||
+        (rc = temp_field(c, prec, nrhs, 3, &t2))) return rc;
+    const RhsList rl = all_rhs(nrhs);
+    for (int p = 0; p < 2; ++p) {
+        PackArgs a;
+        a.f = f[p]->view(); a.canon = (double*)in; a.Vc = 2ll * c->g.Vh; a.full = 1; a.par = p; a.nrhs = nrhs; a.rhs0 = 0;
+        if ((rc = launch_pack(c, prec, false, a, st))) return rc;
+    }
+    for (int p = 0; p < 2; ++p) {
+        const SpinorView same = f[p]->view(), other = f[1 - p]->view(), v1 = t1->view(), v2 = t2->view();
+        if (!dagger) {
+            if ((rc = op_ls(o, v1, other, MAT_A, nullptr, 0.0, 1.0, rl))) return rc;
+            if ((rc = op_ls(o, v2, same, MAT_M5, nullptr, 0.0, 1.0, rl))) return rc;
+            if ((rc = op_hop(o, fo->view(), v1, p, 0, -1, &v2, 1.0, -0.5, rl))) return rc;
+        } else {
+            if ((rc = op_ls(o, v2, same, MAT_M5_D, nullptr, 0.0, 1.0, rl))) return rc;
+            if ((rc = op_hop(o, fo->view(), other, p, 1, MAT_A_D, &v2, 1.0, -0.5, rl))) return rc;
+        }
+        PackArgs a;
+        a.f = fo->view(); a.canon = (double*)out; a.Vc = 2ll * c->g.Vh; a.full = 1; a.par = p; a.nrhs = nrhs; a.rhs0 = 0;
+        if ((rc = launch_pack(c, prec, true, a, st))) return rc;
+    }
+    return MDWF_OK;
+}
+
+// per 5D site and rhs, w = bytes per real,
+//   hop: 1320 flop, 2*24*w (+8 for fp16 norms) + 8*R*w/(Ls*nrhs) bytes;  A, M5: 72 flop;  M5^-1: 48*Ls flop;
+//   site-local ops: 2*24*w (+8) bytes;  Dhat/Mhat: 2832 + 96*Ls flop, fused floor 5 spinor passes + 2 link passes.
+int mdwf_dslash_cost(const mdwf_ctx* c, int op, int prec, int recon, int nrhs, double* bytes, double* flops) {
+    if (!c || !bytes || !flops) return MDWF_EINVAL;
+    const double w = prec / 8.0, n5 = (double)c->g.N5h * nrhs, Ls = c->g.Ls;
+    const double pass = 24.0 * w + (prec == 16 ? 4.0 : 0.0);
+    const double links = 8.0 * recon * w * c->g.Vh;
+    switch (op) {
+        case MDWF_OP_HOP: *bytes = 2 * pass * n5 + links; *flops = 1320.0 * n5; return MDWF_OK;
+        case MDWF_OP_M4PRE:
+        case MDWF_OP_M5: *bytes = 2 * pass * n5; *flops = 72.0 * n5; return MDWF_OK;
+        case MDWF_OP_M5INV: *bytes = 2 * pass * n5; *flops = 48.0 * Ls * n5; return MDWF_OK;
+        case MDWF_OP_DHAT_ASYM:
+        case MDWF_OP_DHAT_SYM: *bytes = 5 * pass * n5 + 2 * links; *flops = (2832.0 + 96.0 * Ls) * n5; return MDWF_OK;
+        case MDWF_OP_NORMAL_ASYM:
+        case MDWF_OP_NORMAL_SYM: *bytes = 2 * (5 * pass * n5 + 2 * links); *flops = 2 * (2832.0 + 96.0 * Ls) * n5; return MDWF_OK;
+        case MDWF_OP_FULL: *bytes = 2 * (3 * pass * n5 + links); *flops = 2 * (1320.0 + 72.0 * 2 + 48.0) * n5; return MDWF_OK;
+    }
+    return MDWF_EINVAL;
+}
+
+}  // extern "C"

@@ -1,0 +1,246 @@
+// csrc/mdwf_blas.cuh -- 4D-site-local kernels: the Ls-direction operators (A = "M4pre", M5, M5^-1 and
+// their products are one Ls x Ls real matrix per chirality, SURVEY 8 Notation), the fused BLAS-1 of the
+// CG iteration with fp64 fixed-order reductions ("all reductions are done in double precision",
+// PAPER.md:183), precision conversion and canonical<->packed packing.
+// One thread per 5D site (s fastest), one rhs per block, blockIdx.x = tile*nact + slot.
+#pragma once
+#include "mdwf_hop.cuh"
+
+namespace mdwf {
+
+struct RhsList {
+    int nact;
+    int rhs[64];
+};
+
+// out = cx*xin + ch * G in   (G == nullptr: identity), optional sum |out|^2, optional no store
+struct LsArgs {
+    SpinorView out, in, xin;
+    const void* G;
+    double cx, ch;
+    double* partial;
+    int write;
+    RhsList rl;
+};
+template <typename S>
+__global__ void __launch_bounds__(256) ls_kernel(const Geom g, const LsArgs a) {
+    typedef typename Store<S>::real T;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int slot = blockIdx.x % a.rl.nact, tile = blockIdx.x / a.rl.nact, rhs = a.rl.rhs[slot];
+    const int idx = tile * blockDim.x + threadIdx.x;
+    const bool live = idx < g.N5h;
+    T acc[24];
+    if (live) load_spinor<S>(a.in, rhs, idx, g.N5h, acc);
+    else {
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[i] = 0;
+    }
+    if (a.G != nullptr) apply_G<T>(acc, a.G, g.Ls, smem_raw);
+    const T ch = (T)a.ch, cx = (T)a.cx;
+    if (a.xin.v != nullptr && live) {
+        T xv[24];
+        load_spinor<S>(a.xin, rhs, idx, g.N5h, xv);
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[i] = cx * xv[i] + ch * acc[i];
+    } else {
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[i] *= ch;
+    }
+    if (live && a.write) store_spinor<S>(a.out, rhs, idx, g.N5h, acc);
+    if (a.partial != nullptr) {
+        double s2 = 0.0;
+        if (live) {
+#pragma unroll
+            for (int i = 0; i < 24; ++i) s2 += (double)acc[i] * (double)acc[i];
+        }
+        block_sum_store(s2, smem_raw, a.partial + (long long)slot * (gridDim.x / a.rl.nact) + tile);
+    }
+}
+
+// out = ca*a + cb*b with independent storage types (conversion, x_hi += x_lo, r = bhat - y, ...);
+// a or b may be absent (v == nullptr); optional sum |out|^2.
+struct AxpbyArgs {
+    SpinorView out, a, b;
+    double ca, cb;
+    double* partial;
+    RhsList rl;
+};
+template <typename SO, typename SA, typename SB>
+__global__ void __launch_bounds__(256) axpby_kernel(const Geom g, const AxpbyArgs p) {
+    typedef typename Store<SO>::real TO;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int slot = blockIdx.x % p.rl.nact, tile = blockIdx.x / p.rl.nact, rhs = p.rl.rhs[slot];
+    const int idx = tile * blockDim.x + threadIdx.x;
+    const bool live = idx < g.N5h;
+    double s2 = 0.0;
+    if (live) {
+        double o[24];
+#pragma unroll
+        for (int i = 0; i < 24; ++i) o[i] = 0.0;
+        if (p.a.v != nullptr) {
+            typename Store<SA>::real v[24];
+            load_spinor<SA>(p.a, rhs, idx, g.N5h, v);
+#pragma unroll
+            for (int i = 0; i < 24; ++i) o[i] = p.ca * (double)v[i];
+        }
+        if (p.b.v != nullptr) {
+            typename Store<SB>::real v[24];
+            load_spinor<SB>(p.b, rhs, idx, g.N5h, v);
+#pragma unroll
+            for (int i = 0; i < 24; ++i) o[i] += p.cb * (double)v[i];
+        }
+        TO w[24];
+#pragma unroll
+        for (int i = 0; i < 24; ++i) {
+            w[i] = (TO)o[i];
+            s2 += o[i] * o[i];
+        }
+        store_spinor<SO>(p.out, rhs, idx, g.N5h, w);
+    }
+    if (p.partial != nullptr)
+        block_sum_store(s2, smem_raw, p.partial + (long long)slot * (gridDim.x / p.rl.nact) + tile);
+}
+
+// CG step, part 1:  alpha = rr/pAp ;  x += alpha p ;  r -= alpha Ap ;  partial |r|^2
+struct CgXrArgs {
+    SpinorView x, r, p, Ap;
+    const double* rr;     // [64] by rhs id
+    const double* pAp;    // [64]
+    double* partial;
+    RhsList rl;
+};
+template <typename SX, typename S>
+__global__ void __launch_bounds__(256) cg_update_xr_kernel(const Geom g, const CgXrArgs a) {
+    typedef typename Store<S>::real T;
+    typedef typename Store<SX>::real TX;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int slot = blockIdx.x % a.rl.nact, tile = blockIdx.x / a.rl.nact, rhs = a.rl.rhs[slot];
+    const int idx = tile * blockDim.x + threadIdx.x;
+    const bool live = idx < g.N5h;
+    double s2 = 0.0;
+    if (live) {
+        const double alpha_d = a.rr[rhs] / a.pAp[rhs];
+        T pv[24], rv[24], av[24];
+        TX xv[24];
+        load_spinor<S>(a.p, rhs, idx, g.N5h, pv);
+        load_spinor<S>(a.Ap, rhs, idx, g.N5h, av);
+        load_spinor<S>(a.r, rhs, idx, g.N5h, rv);
+        load_spinor<SX>(a.x, rhs, idx, g.N5h, xv);
+        const T al = (T)alpha_d;
+        const TX alx = (TX)alpha_d;
+#pragma unroll
+        for (int i = 0; i < 24; ++i) {
+            xv[i] += alx * (TX)pv[i];
+            rv[i] -= al * av[i];
+            s2 += (double)rv[i] * (double)rv[i];
+        }
+        store_spinor<SX>(a.x, rhs, idx, g.N5h, xv);
+        store_spinor<S>(a.r, rhs, idx, g.N5h, rv);
+    }
+    block_sum_store(s2, smem_raw, a.partial + (long long)slot * (gridDim.x / a.rl.nact) + tile);
+}
+
+// CG step, part 2:  beta = rr_new/rr_old ;  p = r + beta p ;  optionally also q = G p (G = A or M5^-dag:
+// the leading s-direction factor of the next operator application, fused to save one pass)
+struct CgPArgs {
+    SpinorView p, r, q;
+    const void* G;
+    const double* rr_new;
+    const double* rr_old;
+    RhsList rl;
+};
+template <typename S>
+__global__ void __launch_bounds__(256) cg_update_p_kernel(const Geom g, const CgPArgs a) {
+    typedef typename Store<S>::real T;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int slot = blockIdx.x % a.rl.nact, tile = blockIdx.x / a.rl.nact, rhs = a.rl.rhs[slot];
+    const int idx = tile * blockDim.x + threadIdx.x;
+    const bool live = idx < g.N5h;
+    T pv[24];
+#pragma unroll
+    for (int i = 0; i < 24; ++i) pv[i] = 0;
+    if (live) {
+        const T beta = (T)(a.rr_new[rhs] / a.rr_old[rhs]);
+        T rv[24];
+        load_spinor<S>(a.p, rhs, idx, g.N5h, pv);
+        load_spinor<S>(a.r, rhs, idx, g.N5h, rv);
+#pragma unroll
+        for (int i = 0; i < 24; ++i) pv[i] = rv[i] + beta * pv[i];
+        store_spinor<S>(a.p, rhs, idx, g.N5h, pv);
+    }
+    if (a.G != nullptr) {
+        apply_G<T>(pv, a.G, g.Ls, smem_raw);
+        if (live) store_spinor<S>(a.q, rhs, idx, g.N5h, pv);
+    }
+}
+
+// out[rhs] = sum_b partial[slot][b] in a fixed order; optionally mirrored to (mapped) host memory
+struct FinishArgs {
+    const double* partial;
+    int nblk;
+    double* out;        // [64] by rhs id
+    double* out2;       // optional second destination (e.g. host-mapped), may be nullptr
+    RhsList rl;
+};
+static __global__ void __launch_bounds__(256) finish_sum_kernel(const FinishArgs a) {
+    __shared__ double red[256];
+    const int slot = blockIdx.x, rhs = a.rl.rhs[slot];
+    const double* p = a.partial + (long long)slot * a.nblk;
+    double s = 0.0;
+    for (int i = threadIdx.x; i < a.nblk; i += 256) s += p[i];
+    red[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        a.out[rhs] = red[0];
+        if (a.out2) a.out2[rhs] = red[0];
+    }
+}
+
+// canonical fp64 <-> packed.  Canonical site index: half-lattice (full == 0): xh; full lattice: x4 = 2*xh + o.
+struct PackArgs {
+    SpinorView f;
+    double* canon;          // [rhs][s][Vc][24]
+    long long Vc;           // Vh or V4
+    int full, par, nrhs;
+    int rhs0;               // packed rhs index = rhs0 + r for canonical rhs r
+};
+__device__ __forceinline__ long long canon_site(const Geom& g, int full, int par, int xh) {
+    if (!full) return xh;
+    uint32_t row, xx, r2, y, t, z;
+    g.dXH.divmod((uint32_t)xh, row, xx);
+    g.dY.divmod(row, r2, y);
+    g.dZ.divmod(r2, t, z);
+    const int o = (par + y + z + t) & 1;
+    return 2ll * xh + o;
+}
+template <typename S, bool UNPACK>
+__global__ void __launch_bounds__(256) pack_kernel(const Geom g, const PackArgs a) {
+    typedef typename Store<S>::real T;
+    const int rhs = blockIdx.y;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= g.N5h) return;
+    uint32_t xh, s;
+    g.dLs.divmod((uint32_t)idx, xh, s);
+    const long long xs = canon_site(g, a.full, a.par, (int)xh);
+    double* c = a.canon + (((long long)rhs * g.Ls + s) * a.Vc + xs) * 24;
+    T v[24];
+    if (UNPACK) {
+        load_spinor<S>(a.f, a.rhs0 + rhs, idx, g.N5h, v);
+#pragma unroll
+        for (int i = 0; i < 12; ++i) reinterpret_cast<double2*>(c)[i] = make_double2((double)v[2 * i], (double)v[2 * i + 1]);
+    } else {
+#pragma unroll
+        for (int i = 0; i < 12; ++i) {
+            const double2 t = reinterpret_cast<const double2*>(c)[i];
+            v[2 * i] = (T)t.x;
+            v[2 * i + 1] = (T)t.y;
+        }
+        store_spinor<S>(a.f, a.rhs0 + rhs, idx, g.N5h, v);
+    }
+}
+
+}  // namespace mdwf

@@ -1,0 +1,329 @@
+// csrc/mdwf_device.cuh -- device-side layout, storage traits and spinor/link accessors of the CUDA
+// product path (sm_100a).  Private to csrc/.  Shares nothing with oracle/.
+//
+// Packed layouts:
+//   spinor, one parity, one rhs:  vec[c][xh][s]  c = 0..NV-1, 16-byte vectors
+//        fp64: NV = 12 x double2     fp32: NV = 6 x float4     fp16: NV = 3 x (8 x half) + float norm[xh][s]
+//        reals inside a site are in canonical order r = ((spin*3 + colour)*2 + reim), vector c holds
+//        r = c*RPV .. c*RPV+RPV-1.  A thread owns one 5D site idx = xh*Ls + s (s fastest), so a warp
+//        reads 512 contiguous bytes per vector index.  rhs are separate fields (stride in vectors).
+//   gauge, per (site parity, mu): vec[c][xh]   fp64: double2 x ceil(R/2), fp32: float4 x ceil(R/4),
+//        fp16: 4 x half (8 bytes) x ceil(R/4);  R = 18 | 12 | 8 reals.
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+
+namespace mdwf {
+
+// ---------------------------------------------------------------------------------------------
+// division by a run-time constant: q = (umulhi(M, n) + n) >> l, exact for 0 <= n < 2^31, 1 <= d < 2^31
+// (Granlund-Montgomery round-up method).  Checked exhaustively on the host in tests (fastdiv_selftest).
+struct FastDiv {
+    uint32_t d, M, l;
+    __host__ __device__ __forceinline__ uint32_t div(uint32_t n) const {
+#ifdef __CUDA_ARCH__
+        return (__umulhi(M, n) + n) >> l;
+#else
+        return (uint32_t)((((uint64_t)M * n) >> 32) + n) >> l;
+#endif
+    }
+    __host__ __device__ __forceinline__ void divmod(uint32_t n, uint32_t& q, uint32_t& r) const {
+        q = div(n);
+        r = n - q * d;
+    }
+};
+inline FastDiv make_fastdiv(uint32_t d) {
+    FastDiv f;
+    f.d = d;
+    uint32_t l = 0;
+    while ((1ull << l) < d) ++l;
+    f.l = l;
+    f.M = (uint32_t)((((1ull << l) - d) << 32) / d + 1);
+    return f;
+}
+
+// ---------------------------------------------------------------------------------------------
+struct Geom {
+    int X, Y, Z, T, XH;       // XH = X/2
+    int Ls;
+    int Vh;                   // sites per parity
+    int N5h;                  // Vh*Ls = 5D sites per parity (thread count per rhs)
+    int bc[4];
+    int zc;                   // z-slab depth of the hop traversal (divides Z)
+    FastDiv dLs, dXH, dY, dZ;       // canonical decode of xh
+    FastDiv dZc, dSlab, dTslab;     // slab traversal decode: slab = XH*Y*zc sites, Tslab = T*slab
+};
+
+// one packed spinor field set (nrhs fields of one parity)
+struct SpinorView {
+    void* v;          // vectors
+    float* n;         // fp16 only: per 5D-site scale
+    long long rs;     // rhs stride in vectors (= NV*N5h)
+    long long rn;     // rhs stride in norms (= N5h)
+};
+
+struct GaugeView {
+    const void* v[2];   // per parity of the link's base site; [mu][c][xh] vectors
+};
+
+// ---------------------------------------------------------------------------------------------
+template <typename S> struct Store;
+template <> struct Store<double> {
+    typedef double real;
+    typedef double2 vec;
+    static constexpr int NV = 12, RPV = 2, BYTES = 8;
+    static constexpr bool HALF = false;
+};
+template <> struct Store<float> {
+    typedef float real;
+    typedef float4 vec;
+    static constexpr int NV = 6, RPV = 4, BYTES = 4;
+    static constexpr bool HALF = false;
+};
+template <> struct Store<__half> {
+    typedef float real;
+    typedef uint4 vec;
+    static constexpr int NV = 3, RPV = 8, BYTES = 2;
+    static constexpr bool HALF = true;
+};
+
+__device__ __forceinline__ double2 ldg(const double2* p) { return __ldg(p); }
+__device__ __forceinline__ float4 ldg(const float4* p) { return __ldg(p); }
+__device__ __forceinline__ uint4 ldg(const uint4* p) { return __ldg(p); }
+__device__ __forceinline__ uint2 ldg(const uint2* p) { return __ldg(p); }
+
+__device__ __forceinline__ float2 h2f(uint32_t w) {
+    __half2 h = *reinterpret_cast<__half2*>(&w);
+    return __half22float2(h);
+}
+__device__ __forceinline__ uint32_t f2h(float a, float b) {
+    __half2 h = __floats2half2_rn(a, b);
+    return *reinterpret_cast<uint32_t*>(&h);
+}
+
+// load the 24 reals of 5D site `idx` of rhs `r`.  fp16: returns the UNSCALED values and the scale
+// (callers fold the scale into a later multiply); other types: scale = 1.
+template <typename S>
+__device__ __forceinline__ void load_raw(const SpinorView& f, int r, int idx, int N5h,
+                                         typename Store<S>::real v[24], typename Store<S>::real& scale);
+
+template <>
+__device__ __forceinline__ void load_raw<double>(const SpinorView& f, int r, int idx, int N5h, double v[24],
+                                                 double& scale) {
+    const double2* p = reinterpret_cast<const double2*>(f.v) + (long long)r * f.rs + idx;
+#pragma unroll
+    for (int c = 0; c < 12; ++c) {
+        double2 t = ldg(p + (long long)c * N5h);
+        v[2 * c] = t.x;
+        v[2 * c + 1] = t.y;
+    }
+    scale = 1.0;
+}
+template <>
+__device__ __forceinline__ void load_raw<float>(const SpinorView& f, int r, int idx, int N5h, float v[24],
+                                                float& scale) {
+    const float4* p = reinterpret_cast<const float4*>(f.v) + (long long)r * f.rs + idx;
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+        float4 t = ldg(p + (long long)c * N5h);
+        v[4 * c] = t.x;
+        v[4 * c + 1] = t.y;
+        v[4 * c + 2] = t.z;
+        v[4 * c + 3] = t.w;
+    }
+    scale = 1.0f;
+}
+template <>
+__device__ __forceinline__ void load_raw<__half>(const SpinorView& f, int r, int idx, int N5h, float v[24],
+                                                 float& scale) {
+    const uint4* p = reinterpret_cast<const uint4*>(f.v) + (long long)r * f.rs + idx;
+    scale = __ldg(f.n + (long long)r * f.rn + idx);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        uint4 t = ldg(p + (long long)c * N5h);
+        float2 a = h2f(t.x), b = h2f(t.y), cc = h2f(t.z), d = h2f(t.w);
+        v[8 * c] = a.x; v[8 * c + 1] = a.y; v[8 * c + 2] = b.x; v[8 * c + 3] = b.y;
+        v[8 * c + 4] = cc.x; v[8 * c + 5] = cc.y; v[8 * c + 6] = d.x; v[8 * c + 7] = d.y;
+    }
+}
+
+// load with the scale applied
+template <typename S>
+__device__ __forceinline__ void load_spinor(const SpinorView& f, int r, int idx, int N5h,
+                                            typename Store<S>::real v[24]) {
+    typename Store<S>::real sc;
+    load_raw<S>(f, r, idx, N5h, v, sc);
+    if (Store<S>::HALF) {
+#pragma unroll
+        for (int i = 0; i < 24; ++i) v[i] *= sc;
+    }
+}
+
+template <typename S>
+__device__ __forceinline__ void store_spinor(const SpinorView& f, int r, int idx, int N5h,
+                                             const typename Store<S>::real v[24]);
+template <>
+__device__ __forceinline__ void store_spinor<double>(const SpinorView& f, int r, int idx, int N5h,
+                                                     const double v[24]) {
+    double2* p = reinterpret_cast<double2*>(f.v) + (long long)r * f.rs + idx;
+#pragma unroll
+    for (int c = 0; c < 12; ++c) p[(long long)c * N5h] = make_double2(v[2 * c], v[2 * c + 1]);
+}
+template <>
+__device__ __forceinline__ void store_spinor<float>(const SpinorView& f, int r, int idx, int N5h,
+                                                    const float v[24]) {
+    float4* p = reinterpret_cast<float4*>(f.v) + (long long)r * f.rs + idx;
+#pragma unroll
+    for (int c = 0; c < 6; ++c) p[(long long)c * N5h] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
+}
+// fp16: per-site max-norm scale (fp32) + IEEE half mantissas in [-1,1] ("16-bit storage, single-precision
+// computation"; format choice: SURVEY A11 / DESIGN.md reading R11)
+template <>
+__device__ __forceinline__ void store_spinor<__half>(const SpinorView& f, int r, int idx, int N5h,
+                                                     const float v[24]) {
+    float m = 0.f;
+#pragma unroll
+    for (int i = 0; i < 24; ++i) m = fmaxf(m, fabsf(v[i]));
+    const float inv = m > 0.f ? __fdividef(1.0f, m) : 0.f;
+    f.n[(long long)r * f.rn + idx] = m;
+    uint4* p = reinterpret_cast<uint4*>(f.v) + (long long)r * f.rs + idx;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        uint4 t;
+        t.x = f2h(v[8 * c] * inv, v[8 * c + 1] * inv);
+        t.y = f2h(v[8 * c + 2] * inv, v[8 * c + 3] * inv);
+        t.z = f2h(v[8 * c + 4] * inv, v[8 * c + 5] * inv);
+        t.w = f2h(v[8 * c + 6] * inv, v[8 * c + 7] * inv);
+        p[(long long)c * N5h] = t;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Links.  NGV = vectors per link; U[18] = [row][col][re,im] after reconstruction.
+template <typename S, int R> struct GaugeFmt;
+template <int R> struct GaugeFmt<double, R> { static constexpr int NGV = (R + 1) / 2; typedef double2 vec; };
+template <int R> struct GaugeFmt<float, R> { static constexpr int NGV = (R + 3) / 4; typedef float4 vec; };
+template <int R> struct GaugeFmt<__half, R> { static constexpr int NGV = (R + 3) / 4; typedef uint2 vec; };
+
+template <typename S, int R>
+__device__ __forceinline__ void load_link_raw(const void* base, int mu, int xh, int Vh, typename Store<S>::real g[20]);
+
+#define MDWF_LINK_LOADERS(R)                                                                              \
+    template <>                                                                                           \
+    __device__ __forceinline__ void load_link_raw<double, R>(const void* base, int mu, int xh, int Vh,    \
+                                                             double g[20]) {                              \
+        constexpr int NG = GaugeFmt<double, R>::NGV;                                                      \
+        const double2* p = reinterpret_cast<const double2*>(base) + (long long)mu * NG * Vh + xh;         \
+        _Pragma("unroll") for (int c = 0; c < NG; ++c) {                                                  \
+            double2 t = ldg(p + (long long)c * Vh);                                                       \
+            g[2 * c] = t.x;                                                                               \
+            g[2 * c + 1] = t.y;                                                                           \
+        }                                                                                                 \
+    }                                                                                                     \
+    template <>                                                                                           \
+    __device__ __forceinline__ void load_link_raw<float, R>(const void* base, int mu, int xh, int Vh,     \
+                                                            float g[20]) {                                \
+        constexpr int NG = GaugeFmt<float, R>::NGV;                                                       \
+        const float4* p = reinterpret_cast<const float4*>(base) + (long long)mu * NG * Vh + xh;           \
+        _Pragma("unroll") for (int c = 0; c < NG; ++c) {                                                  \
+            float4 t = ldg(p + (long long)c * Vh);                                                        \
+            g[4 * c] = t.x; g[4 * c + 1] = t.y; g[4 * c + 2] = t.z; g[4 * c + 3] = t.w;                   \
+        }                                                                                                 \
+    }                                                                                                     \
+    template <>                                                                                           \
+    __device__ __forceinline__ void load_link_raw<__half, R>(const void* base, int mu, int xh, int Vh,    \
+                                                             float g[20]) {                               \
+        constexpr int NG = GaugeFmt<__half, R>::NGV;                                                      \
+        const uint2* p = reinterpret_cast<const uint2*>(base) + (long long)mu * NG * Vh + xh;             \
+        _Pragma("unroll") for (int c = 0; c < NG; ++c) {                                                  \
+            uint2 t = ldg(p + (long long)c * Vh);                                                         \
+            float2 a = h2f(t.x), b = h2f(t.y);                                                            \
+            g[4 * c] = a.x; g[4 * c + 1] = a.y; g[4 * c + 2] = b.x; g[4 * c + 3] = b.y;                   \
+        }                                                                                                 \
+    }
+MDWF_LINK_LOADERS(18)
+MDWF_LINK_LOADERS(12)
+MDWF_LINK_LOADERS(8)
+#undef MDWF_LINK_LOADERS
+
+template <typename T> __device__ __forceinline__ void sincos_(T a, T& s, T& c);
+template <> __device__ __forceinline__ void sincos_<double>(double a, double& s, double& c) { sincos(a, &s, &c); }
+template <> __device__ __forceinline__ void sincos_<float>(float a, float& s, float& c) { sincosf(a, &s, &c); }
+template <typename T> __device__ __forceinline__ T sqrt_(T a);
+template <> __device__ __forceinline__ double sqrt_<double>(double a) { return sqrt(a); }
+template <> __device__ __forceinline__ float sqrt_<float>(float a) { return sqrtf(a); }
+
+// rows 0,1 known -> row 2 = conj(row0 x row1)   (SURVEY A12, 12-real format)
+template <typename T> __device__ __forceinline__ void row2_from_rows01(T U[18]) {
+#define RE(r, c) U[((r) * 3 + (c)) * 2]
+#define IM(r, c) U[((r) * 3 + (c)) * 2 + 1]
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+        // (row0 x row1)_c = r0[c1]*r1[c2] - r0[c2]*r1[c1]; conj -> negate imaginary part
+        const T re = RE(0, c1) * RE(1, c2) - IM(0, c1) * IM(1, c2) - RE(0, c2) * RE(1, c1) + IM(0, c2) * IM(1, c1);
+        const T im = RE(0, c1) * IM(1, c2) + IM(0, c1) * RE(1, c2) - RE(0, c2) * IM(1, c1) - IM(0, c2) * RE(1, c1);
+        RE(2, c) = re;
+        IM(2, c) = -im;
+    }
+#undef RE
+#undef IM
+}
+
+// 8-real format: g = {a2.re,a2.im,a3.re,a3.im,b1.re,b1.im, arg a1, arg c1}; fp16 stores the
+// two phases divided by pi.  rows: (a1,a2,a3), (b1,b2,b3), (c1,c2,c3).
+template <typename T, bool PHASE_OVER_PI>
+__device__ __forceinline__ void reconstruct8(const T g[8], T U[18]) {
+    const T a2r = g[0], a2i = g[1], a3r = g[2], a3i = g[3], b1r = g[4], b1i = g[5];
+    T tha = g[6], thc = g[7];
+    if (PHASE_OVER_PI) { tha *= (T)3.14159265358979323846; thc *= (T)3.14159265358979323846; }
+    const T N = a2r * a2r + a2i * a2i + a3r * a3r + a3i * a3i;
+    const T ma = sqrt_<T>(fmax((T)0, (T)1 - N));
+    const T mc = sqrt_<T>(fmax((T)0, N - b1r * b1r - b1i * b1i));
+    T sa, ca, sc, cc;
+    sincos_<T>(tha, sa, ca);
+    sincos_<T>(thc, sc, cc);
+    const T a1r = ma * ca, a1i = ma * sa, c1r = mc * cc, c1i = mc * sc;
+    const T iN = (T)1 / N;
+    // p = conj(a1)*b1, q = conj(a1)*c1
+    const T pr = a1r * b1r + a1i * b1i, pi = a1r * b1i - a1i * b1r;
+    const T qr = a1r * c1r + a1i * c1i, qi = a1r * c1i - a1i * c1r;
+    // b2 = -(p a2 + conj(c1) conj(a3))/N ; b3 = (-p a3 + conj(c1) conj(a2))/N
+    // c2 = (-q a2 + conj(b1) conj(a3))/N ; c3 = -(q a3 + conj(b1) conj(a2))/N
+    // conj(u) conj(v) = conj(u v)
+    const T c1a3r = c1r * a3r - c1i * a3i, c1a3i = c1r * a3i + c1i * a3r;
+    const T c1a2r = c1r * a2r - c1i * a2i, c1a2i = c1r * a2i + c1i * a2r;
+    const T b1a3r = b1r * a3r - b1i * a3i, b1a3i = b1r * a3i + b1i * a3r;
+    const T b1a2r = b1r * a2r - b1i * a2i, b1a2i = b1r * a2i + b1i * a2r;
+    U[0] = a1r; U[1] = a1i; U[2] = a2r; U[3] = a2i; U[4] = a3r; U[5] = a3i;
+    U[6] = b1r; U[7] = b1i;
+    U[8] = -((pr * a2r - pi * a2i) + c1a3r) * iN;
+    U[9] = -((pr * a2i + pi * a2r) - c1a3i) * iN;
+    U[10] = (-(pr * a3r - pi * a3i) + c1a2r) * iN;
+    U[11] = (-(pr * a3i + pi * a3r) - c1a2i) * iN;
+    U[12] = c1r; U[13] = c1i;
+    U[14] = (-(qr * a2r - qi * a2i) + b1a3r) * iN;
+    U[15] = (-(qr * a2i + qi * a2r) - b1a3i) * iN;
+    U[16] = -((qr * a3r - qi * a3i) + b1a2r) * iN;
+    U[17] = -((qr * a3i + qi * a3r) - b1a2i) * iN;
+}
+
+template <typename S, int R>
+__device__ __forceinline__ void load_link(const void* base, int mu, int xh, int Vh, typename Store<S>::real U[18]) {
+    typedef typename Store<S>::real T;
+    T g[20];
+    load_link_raw<S, R>(base, mu, xh, Vh, g);
+    if (R == 18) {
+#pragma unroll
+        for (int i = 0; i < 18; ++i) U[i] = g[i];
+    } else if (R == 12) {
+#pragma unroll
+        for (int i = 0; i < 12; ++i) U[i] = g[i];
+        row2_from_rows01<T>(U);
+    } else {
+        reconstruct8<T, Store<S>::HALF>(g, U);
+    }
+}
+
+}  // namespace mdwf

@@ -1,0 +1,54 @@
+// csrc/mdwf_hop_launch.cuh -- launcher template for hop_kernel; instantiated per storage precision in
+// hop_f64.cu / hop_f32.cu / hop_f16.cu so the three compile in parallel.
+#pragma once
+#include "mdwf_host.h"
+#include <set>
+
+namespace mdwf {
+
+template <typename K>
+static inline int launch_with_smem(mdwf_ctx* c, K kern, int grid, int block, size_t smem, cudaStream_t st,
+                                   const Geom& g, const HopArgs& a) {
+    static std::set<const void*> raised;
+    if (smem > 48 * 1024 && !raised.count((const void*)kern)) {
+        MDWF_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        raised.insert((const void*)kern);
+    }
+    kern<<<grid, block, smem, st>>>(g, a);
+    MDWF_CUDA(c, cudaGetLastError());
+    c->launches++;
+    return MDWF_OK;
+}
+
+template <typename S, int R>
+static int launch_hop_SR(mdwf_ctx* c, int dagger, int fused, HopArgs& a, cudaStream_t st) {
+    typedef typename Store<S>::real T;
+    const int grid = c->nblk * a.nact;
+    size_t smem = 0;
+    if (fused) {
+        smem = (size_t)c->block * sizeof(double);
+        if (a.G) smem = std::max(smem, (size_t)smem_reals_G<T>(c->g.Ls, c->block) * sizeof(T));
+    }
+    if (fused) {
+        if (dagger) return launch_with_smem(c, hop_kernel<S, R, true, true>, grid, c->block, smem, st, c->g, a);
+        return launch_with_smem(c, hop_kernel<S, R, false, true>, grid, c->block, smem, st, c->g, a);
+    }
+    if (dagger) return launch_with_smem(c, hop_kernel<S, R, true, false>, grid, c->block, smem, st, c->g, a);
+    return launch_with_smem(c, hop_kernel<S, R, false, false>, grid, c->block, smem, st, c->g, a);
+}
+
+template <typename S>
+static int launch_hop_S(mdwf_ctx* c, int recon, int dagger, int fused, HopArgs& a, cudaStream_t st) {
+    switch (recon) {
+        case 18: return launch_hop_SR<S, 18>(c, dagger, fused, a, st);
+        case 12: return launch_hop_SR<S, 12>(c, dagger, fused, a, st);
+        case 8: return launch_hop_SR<S, 8>(c, dagger, fused, a, st);
+    }
+    MDWF_FAIL(c, MDWF_EINVAL, "recon must be 18, 12 or 8 (got %d)", recon);
+}
+
+int launch_hop_f64(mdwf_ctx* c, int recon, int dagger, int fused, HopArgs& a, cudaStream_t st);
+int launch_hop_f32(mdwf_ctx* c, int recon, int dagger, int fused, HopArgs& a, cudaStream_t st);
+int launch_hop_f16(mdwf_ctx* c, int recon, int dagger, int fused, HopArgs& a, cudaStream_t st);
+
+}  // namespace mdwf

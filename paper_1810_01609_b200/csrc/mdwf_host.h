@@ -1,0 +1,111 @@
+// csrc/mdwf_host.h -- host-side context and launcher prototypes of libmdwf.so (private to csrc/).
+#pragma once
+#include <string>
+#include <vector>
+#include <map>
+#include <cstdio>
+#include "../../include/mdwf.h"
+#include "mdwf_blas.cuh"
+
+// Ls x Ls chirality-block matrices kept on the device (fp64 and fp32 copies), layout Gt[chi][s'][s]
+enum MatId { MAT_A = 0, MAT_M5, MAT_M5INV, MAT_AM5INV, MAT_A_D, MAT_M5_D, MAT_M5INV_D, MAT_AM5INV_D, MAT_COUNT };
+
+struct GaugeSet {
+    int prec, recon;
+    void* v[2];
+    size_t bytes_per_parity;
+};
+
+struct mdwf_field {
+    mdwf_ctx* ctx;
+    int prec, nrhs;
+    void* v;
+    float* n;
+    size_t bytes;
+    mdwf::SpinorView view() const;
+};
+
+struct mdwf_ctx {
+    mdwf_geometry geo;
+    double M5, b5, c5, mf;
+    mdwf::Geom g;
+    int block;                 // threads per block: a multiple of Ls, <= 256
+    int nblk;                  // blocks per rhs = ceil(N5h / block)
+    std::vector<GaugeSet> gauges;
+    void* mat_d[MAT_COUNT];
+    void* mat_f[MAT_COUNT];
+    double* partial;           // [64][nblk] per-block partial sums
+    double* dscal;             // device scalars [8][64]
+    double* hscal;             // pinned host mirror [8][64]
+    std::map<long long, std::vector<mdwf_field*> > temps;   // cached work fields keyed by prec*1000+nrhs
+    std::string err;
+    long long launches;
+    int sm_count;
+    const GaugeSet* find_gauge(int prec, int recon) const {
+        for (size_t i = 0; i < gauges.size(); ++i)
+            if (gauges[i].prec == prec && gauges[i].recon == recon) return &gauges[i];
+        return nullptr;
+    }
+    const void* mat(int id, int prec) const { return prec == 64 ? mat_d[id] : mat_f[id]; }
+};
+
+#define MDWF_FAIL(ctx, code, ...)                          \
+    do {                                                   \
+        char _b[512];                                      \
+        snprintf(_b, sizeof(_b), __VA_ARGS__);             \
+        (ctx)->err = _b;                                   \
+        return (code);                                     \
+    } while (0)
+#define MDWF_CUDA(ctx, expr)                                                                             \
+    do {                                                                                                 \
+        cudaError_t _e = (expr);                                                                         \
+        if (_e != cudaSuccess) MDWF_FAIL(ctx, MDWF_ECUDA, "%s: %s (%s:%d)", #expr, cudaGetErrorString(_e), \
+                                         __FILE__, __LINE__);                                            \
+    } while (0)
+
+namespace mdwf {
+
+inline RhsList all_rhs(int n) {
+    RhsList r;
+    r.nact = n;
+    for (int i = 0; i < 64; ++i) r.rhs[i] = i < n ? i : 0;
+    return r;
+}
+
+size_t field_bytes(const Geom& g, int prec, int nrhs, size_t* norm_off);
+int alloc_field(mdwf_ctx* c, int prec, int nrhs, mdwf_field** out);
+void free_field(mdwf_field* f);
+// cached temporaries: slot-th work field of (prec, nrhs)
+int temp_field(mdwf_ctx* c, int prec, int nrhs, int slot, mdwf_field** out);
+
+// ---- launchers (each returns MDWF_OK or an error code with ctx->err set) --------------------------
+// out = H in (fused == 0) or cx*xin + ch*G*(H in) (fused != 0; G/xin optional; partial optional)
+int launch_hop(mdwf_ctx* c, int prec, int recon, int dagger, int fused, HopArgs& a, cudaStream_t st);
+int launch_ls(mdwf_ctx* c, int prec, LsArgs& a, cudaStream_t st);
+int launch_axpby(mdwf_ctx* c, int prec_out, int prec_a, int prec_b, AxpbyArgs& a, cudaStream_t st);
+int launch_cg_xr(mdwf_ctx* c, int prec_x, int prec, CgXrArgs& a, cudaStream_t st);
+int launch_cg_p(mdwf_ctx* c, int prec, CgPArgs& a, cudaStream_t st);
+int launch_finish(mdwf_ctx* c, const RhsList& rl, double* out, double* out2, cudaStream_t st);
+int launch_pack(mdwf_ctx* c, int prec, bool unpack, PackArgs& a, cudaStream_t st);
+int pack_gauge(mdwf_ctx* c, const void* U, int prec, int recon, GaugeSet* gs, cudaStream_t st);
+
+// ---- composite operators on packed fields (solver + API) ------------------------------------------
+struct OpCtx {
+    mdwf_ctx* c;
+    int prec, recon;
+    const GaugeSet* gs;
+    cudaStream_t st;
+};
+// simple helpers: out = cx*xin + ch*G*in ; out = cx*xin + ch*G*H(in)
+int op_ls(const OpCtx& o, const SpinorView& out, const SpinorView& in, int mat, const SpinorView* xin, double cx,
+          double ch, const RhsList& rl, double* partial = nullptr, int write = 1);
+int op_hop(const OpCtx& o, const SpinorView& out, const SpinorView& in, int out_par, int dagger, int mat,
+           const SpinorView* xin, double cx, double ch, const RhsList& rl, double* partial = nullptr);
+// Schur operator: out = Dhat/Mhat (dagger) in, parity p; t1, t2 are work fields; if partial != nullptr the
+// per-block |out|^2 sums are written there (to be finished with launch_finish)
+int op_schur(const OpCtx& o, const SpinorView& out, const SpinorView& in, int par, int dagger, int symmetric,
+             const SpinorView& t1, const SpinorView& t2, const RhsList& rl, double* partial = nullptr);
+
+int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_opts* opts, mdwf_solve_info* info,
+               cudaStream_t st, bool host_buffers);
+}  // namespace mdwf
