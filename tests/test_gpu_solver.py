@@ -1,0 +1,105 @@
+"""GPU parity: mdwf_solve (mixed-precision CG with reliable updates) and the FH chain against the oracle.
+Acceptance (north_star / SURVEY O2): full-system true residual <= tol with the ORACLE's D in fp64;
+solution rel-L2 vs the oracle solution <= 1e-6; manufactured solution b = D psi*."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+
+pytestmark = pytest.mark.gpu
+
+
+def rel(a, b):
+    a = np.asarray(a).reshape(-1)
+    b = np.asarray(b).reshape(-1)
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+def make(cfg_index, dims=None, Ls=None, mf=None):
+    import paper_1810_01609_b200 as mdwf
+    cfg = synth.CONFIGS[cfg_index]
+    dims = dims or cfg.dims
+    Ls = Ls or cfg.Ls
+    mf = mf if mf is not None else cfg.mf
+    p = oracle.Params(dims=tuple(dims), Ls=Ls, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=mf, bc=cfg.bc)
+    U = synth.gauge_field(dims, cfg.eps, synth.seed_for(cfg_index, 1))
+    ctx = mdwf.Context(dims, Ls, cfg.M5, cfg.b5, cfg.c5, mf, bc=cfg.bc)
+    Ud = U.cuda()
+    ctx.mdwf_load_gauge(Ud, 64, 18)
+    return mdwf, cfg, p, U, ctx, Ud
+
+
+@pytest.mark.parametrize("inner,recon", [(64, 18), (32, 12), (16, 12), (16, 8)])
+@pytest.mark.parametrize("symmetric", [True, False])
+def test_config1_solve(inner, recon, symmetric):
+    """BASELINE configs[0]: 4^4, Ls=4, CG to 1e-10; oracle variant A (unpreconditioned) is the reference."""
+    mdwf, cfg, p, U, ctx, Ud = make(1)
+    if inner != 64:
+        ctx.mdwf_load_gauge(Ud, inner, recon)
+    elif recon != 18:
+        ctx.mdwf_load_gauge(Ud, 64, recon)
+    b = synth.gaussian_spinor(cfg.dims, cfg.Ls, 1, synth.seed_for(1, 2))
+    x, res = ctx.mdwf_solve(b.cuda(), tol=1e-10, inner_prec=inner, recon=recon, symmetric=symmetric)
+    assert res.status == mdwf.OK, res
+    xn = x.cpu().numpy()
+    tr = oracle.true_residual(p, U.numpy(), xn, b.numpy())
+    assert tr.max() <= 1e-10, (tr, res)
+    assert abs(res.true_resid[0] - tr[0]) <= 0.05 * tr[0] + 1e-13      # library's own residual is the true one
+    xo, _, _ = oracle.solve_full(p, U.numpy(), b.numpy(), tol=1e-13)
+    assert rel(xn, xo) <= 1e-6
+
+
+@pytest.mark.parametrize("parity", [0, 1])
+def test_multi_rhs_batched_manufactured(parity):
+    """8^3x16, Ls=8, 5 rhs in batches of 2 (ragged last batch): psi* Gaussian, b = D psi* by the oracle."""
+    mdwf, cfg, p, U, ctx, Ud = make(3, dims=(8, 8, 8, 16))
+    ctx.mdwf_load_gauge(Ud, 16, 12)
+    star = synth.gaussian_spinor(p.dims, p.Ls, 5, synth.seed_for(3, 50)).numpy()
+    b = oracle.D(p, U.numpy(), star)
+    x, res = ctx.mdwf_solve(torch.from_numpy(b).cuda(), tol=1e-9, inner_prec=16, recon=12, parity=parity, batch=2)
+    assert res.status == mdwf.OK, res
+    xn = x.cpu().numpy()
+    for r in range(5):
+        assert rel(xn[r], star[r]) <= 1e-6, (r, rel(xn[r], star[r]))
+    assert oracle.true_residual(p, U.numpy(), xn, b).max() <= 1e-9
+    assert all(n >= 1 for n in res.reliable_updates)
+
+
+def test_point_source_propagator_4d():
+    """configs[2] shape scaled to 8^3x16: 12 point sources on the walls (O3), 4D in / 4D out; checked against
+    the oracle's wall_inject -> solve_eo -> wall_project, and through the true residual of the 5D system."""
+    mdwf, cfg, p, U, ctx, Ud = make(3, dims=(8, 8, 8, 16))
+    ctx.mdwf_load_gauge(Ud, 16, 12)
+    eta = synth.point_sources_4d(p.dims)
+    q, res = ctx.mdwf_solve(eta.cuda(), tol=1e-9, inner_prec=16, recon=12, src_kind=1, out_kind=1)
+    assert res.status == mdwf.OK, res
+    Un = U.numpy()
+    cols = [0, 7]
+    b5 = oracle.wall_inject(p, Un, eta.numpy()[cols])
+    assert rel(ctx.mdwf_wall_inject(eta.cuda()).cpu().numpy()[cols], b5) <= 1e-12
+    xo, _, _ = oracle.solve_eo(p, Un, b5, tol=1e-12)
+    qo = oracle.wall_project(p, xo)
+    assert rel(q.cpu().numpy()[cols], qo) <= 1e-6
+    # 5D output of the same solve satisfies the full system
+    x5, res5 = ctx.mdwf_solve(eta.cuda()[cols], tol=1e-9, inner_prec=16, recon=12, src_kind=1, out_kind=0)
+    assert oracle.true_residual(p, Un, x5.cpu().numpy(), b5).max() <= 1e-9
+    assert rel(ctx.mdwf_wall_project(x5).cpu().numpy(), qo) <= 1e-6
+
+
+def test_host_buffer_solve_matches_device_solve():
+    mdwf, cfg, p, U, ctx, Ud = make(1)
+    ctx.mdwf_load_gauge(Ud, 32, 12)
+    b = synth.gaussian_spinor(cfg.dims, cfg.Ls, 3, synth.seed_for(1, 3))
+    xh = torch.empty_like(b).pin_memory()
+    _, res = ctx.mdwf_solve_host(b.pin_memory(), xh, tol=1e-10, inner_prec=32, recon=12, batch=2)
+    assert res.status == mdwf.OK
+    assert oracle.true_residual(p, U.numpy(), xh.numpy(), b.numpy()).max() <= 1e-10
+
+
+def test_not_converged_is_reported():
+    mdwf, cfg, p, U, ctx, Ud = make(1)
+    b = synth.gaussian_spinor(cfg.dims, cfg.Ls, 1, synth.seed_for(1, 2))
+    x, res = ctx.mdwf_solve(b.cuda(), tol=1e-10, inner_prec=64, recon=18, max_iter=3)
+    assert res.status == mdwf.NOT_CONVERGED and res.rhs_status[0] == mdwf.NOT_CONVERGED
