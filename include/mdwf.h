@@ -157,6 +157,14 @@ int mdwf_wall_project(mdwf_ctx* ctx, void* q4, const void* psi5, int ncol, void*
 
 /* number of kernels this context has launched so far (bench.py's gpu_launches) */
 int64_t mdwf_launch_count(const mdwf_ctx* ctx);
+/* Per-launch timing of the hop (Dslash stencil) kernel with CUDA events on the launching stream.
+ * mdwf_profile(ctx, 1) clears the counters and starts recording, mdwf_profile(ctx, 0) stops.
+ * mdwf_profile_read synchronises the recorded events and returns, for class cls (0: fp16 storage, 1: fp32,
+ * 2: fp64), the summed device time [ms], algorithmic bytes and flops (DESIGN.md cost convention: per 5D
+ * site 24*w (+4) bytes per spinor pass, 2 passes (+1 with an xpay input), links once per launch; 1320 flop)
+ * and the launch count. */
+int mdwf_profile(mdwf_ctx* ctx, int enable);
+int mdwf_profile_read(mdwf_ctx* ctx, int cls, double* ms, double* bytes, double* flops, int64_t* launches);
 /* set the z-slab depth of the hop kernel's site traversal (L2 tiling); 0 = automatic */
 int mdwf_set_tiling(mdwf_ctx* ctx, int zc);
 

@@ -24,7 +24,7 @@ EXPORTS = [
     "mdwf_create", "mdwf_destroy", "mdwf_last_error", "mdwf_load_gauge", "mdwf_dslash", "mdwf_field_create",
     "mdwf_field_destroy", "mdwf_field_pack", "mdwf_field_unpack", "mdwf_dslash_packed", "mdwf_dslash_cost",
     "mdwf_solve", "mdwf_solve_host", "mdwf_seq_source", "mdwf_nucleon_2pt", "mdwf_wall_inject",
-    "mdwf_wall_project", "mdwf_launch_count", "mdwf_set_tiling",
+    "mdwf_wall_project", "mdwf_launch_count", "mdwf_set_tiling", "mdwf_profile", "mdwf_profile_read",
 ]
 
 
@@ -86,6 +86,9 @@ def lib():
         L.mdwf_launch_count.argtypes = [vp]
         L.mdwf_launch_count.restype = ctypes.c_int64
         L.mdwf_set_tiling.argtypes = [vp, ci]
+        L.mdwf_profile.argtypes = [vp, ci]
+        L.mdwf_profile_read.argtypes = [vp, ci, ctypes.POINTER(cd), ctypes.POINTER(cd), ctypes.POINTER(cd),
+                                        ctypes.POINTER(ctypes.c_int64)]
         _lib = L
     return _lib
 
@@ -283,3 +286,13 @@ class Context:
 
     def mdwf_set_tiling(self, zc):
         self._chk(lib().mdwf_set_tiling(self._h, zc))
+
+    def mdwf_profile(self, enable):
+        self._chk(lib().mdwf_profile(self._h, int(bool(enable))))
+
+    def mdwf_profile_read(self, cls):
+        """(ms, bytes, flops, launches) of the hop kernel for storage class cls (0 fp16, 1 fp32, 2 fp64)."""
+        ms, by, fl, n = ctypes.c_double(), ctypes.c_double(), ctypes.c_double(), ctypes.c_int64()
+        self._chk(lib().mdwf_profile_read(self._h, cls, ctypes.byref(ms), ctypes.byref(by), ctypes.byref(fl),
+                                          ctypes.byref(n)))
+        return ms.value, by.value, fl.value, n.value

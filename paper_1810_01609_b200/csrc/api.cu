@@ -79,6 +79,19 @@ static void set_zc(mdwf_ctx* c, int zc) {
     g.dTslab = make_fastdiv((uint32_t)(g.XH * g.Y * zc) * (uint32_t)g.T);
 }
 
+static void prof_drain(mdwf_ctx* c) {
+    for (size_t i = 0; i < c->prof_pending.size(); ++i) {
+        mdwf_ctx::ProfRec& r = c->prof_pending[i];
+        float ms = 0.f;
+        if (cudaEventSynchronize(r.e1) == cudaSuccess && cudaEventElapsedTime(&ms, r.e0, r.e1) == cudaSuccess) {
+            c->prof_ms[r.cls] += ms; c->prof_bytes[r.cls] += r.bytes; c->prof_flops[r.cls] += r.flops; c->prof_n[r.cls]++;
+        }
+        c->prof_pool.push_back(r.e0);
+        c->prof_pool.push_back(r.e1);
+    }
+    c->prof_pending.clear();
+}
+
 extern "C" {
 
 int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, double c5, double mf) {
@@ -87,7 +100,8 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     mdwf_ctx* c = new mdwf_ctx;
     c->geo = *geo;
     c->M5 = M5; c->b5 = b5; c->c5 = c5; c->mf = mf;
-    c->partial = nullptr; c->dscal = nullptr; c->hscal = nullptr; c->launches = 0;
+    c->partial = nullptr; c->dscal = nullptr; c->hscal = nullptr; c->launches = 0; c->prof_on = 0;
+    for (int i = 0; i < 3; ++i) { c->prof_ms[i] = c->prof_bytes[i] = c->prof_flops[i] = 0.0; c->prof_n[i] = 0; }
     for (int i = 0; i < MAT_COUNT; ++i) c->mat_d[i] = c->mat_f[i] = nullptr;
     *out = c;   // returned even on failure so that mdwf_last_error can be read; caller destroys it
     long long v4 = 1;
@@ -143,6 +157,8 @@ int mdwf_destroy(mdwf_ctx* c) {
     for (size_t i = 0; i < c->gauges.size(); ++i) { cudaFree(c->gauges[i].v[0]); cudaFree(c->gauges[i].v[1]); }
     for (auto& kv : c->temps) for (mdwf_field* f : kv.second) free_field(f);
     for (int i = 0; i < MAT_COUNT; ++i) { if (c->mat_d[i]) cudaFree(c->mat_d[i]); if (c->mat_f[i]) cudaFree(c->mat_f[i]); }
+    prof_drain(c);
+    for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
     if (c->partial) cudaFree(c->partial);
     if (c->dscal) cudaFree(c->dscal);
     if (c->hscal) cudaFreeHost(c->hscal);
@@ -152,6 +168,20 @@ int mdwf_destroy(mdwf_ctx* c) {
 
 const char* mdwf_last_error(const mdwf_ctx* c) { return c ? c->err.c_str() : "null context"; }
 int64_t mdwf_launch_count(const mdwf_ctx* c) { return c ? c->launches : 0; }
+
+int mdwf_profile(mdwf_ctx* c, int enable) {
+    if (!c) return MDWF_EINVAL;
+    prof_drain(c);
+    if (enable) for (int i = 0; i < 3; ++i) { c->prof_ms[i] = c->prof_bytes[i] = c->prof_flops[i] = 0.0; c->prof_n[i] = 0; }
+    c->prof_on = enable ? 1 : 0;
+    return MDWF_OK;
+}
+int mdwf_profile_read(mdwf_ctx* c, int cls, double* ms, double* bytes, double* flops, int64_t* launches) {
+    if (!c || cls < 0 || cls > 2 || !ms || !bytes || !flops || !launches) return MDWF_EINVAL;
+    prof_drain(c);
+    *ms = c->prof_ms[cls]; *bytes = c->prof_bytes[cls]; *flops = c->prof_flops[cls]; *launches = c->prof_n[cls];
+    return MDWF_OK;
+}
 
 int mdwf_set_tiling(mdwf_ctx* c, int zc) {
     if (!c) return MDWF_EINVAL;

@@ -85,13 +85,33 @@ int launch_ls(mdwf_ctx* c, int prec, LsArgs& a, cudaStream_t st) {
     MDWF_FAIL(c, MDWF_EINVAL, "bad precision %d", prec);
 }
 
-int launch_hop(mdwf_ctx* c, int prec, int recon, int dagger, int fused, HopArgs& a, cudaStream_t st) {
+static int launch_hop_raw(mdwf_ctx* c, int prec, int recon, int dagger, int fused, HopArgs& a, cudaStream_t st) {
     switch (prec) {
         case 64: return launch_hop_f64(c, recon, dagger, fused, a, st);
         case 32: return launch_hop_f32(c, recon, dagger, fused, a, st);
         case 16: return launch_hop_f16(c, recon, dagger, fused, a, st);
     }
     MDWF_FAIL(c, MDWF_EINVAL, "bad precision %d", prec);
+}
+int launch_hop(mdwf_ctx* c, int prec, int recon, int dagger, int fused, HopArgs& a, cudaStream_t st) {
+    if (!c->prof_on) return launch_hop_raw(c, prec, recon, dagger, fused, a, st);
+    mdwf_ctx::ProfRec r;
+    for (int k = 0; k < 2; ++k) {
+        cudaEvent_t e;
+        if (!c->prof_pool.empty()) { e = c->prof_pool.back(); c->prof_pool.pop_back(); }
+        else MDWF_CUDA(c, cudaEventCreate(&e));
+        (k ? r.e1 : r.e0) = e;
+    }
+    const double w = prec / 8.0, n5 = (double)c->g.N5h * a.nact;
+    const double pass = 24.0 * w + (prec == 16 ? 4.0 : 0.0);
+    r.cls = prec == 16 ? 0 : prec == 32 ? 1 : 2;
+    r.bytes = (2.0 + (a.xin.v ? 1.0 : 0.0)) * pass * n5 + 8.0 * recon * w * c->g.Vh;
+    r.flops = 1320.0 * n5;
+    cudaEventRecord(r.e0, st);
+    int rc = launch_hop_raw(c, prec, recon, dagger, fused, a, st);
+    cudaEventRecord(r.e1, st);
+    c->prof_pending.push_back(r);
+    return rc;
 }
 
 template <typename SO, typename SA>

@@ -40,6 +40,14 @@ struct mdwf_ctx {
     std::map<long long, std::vector<mdwf_field*> > temps;   // cached work fields keyed by prec*1000+nrhs
     std::string err;
     long long launches;
+    // optional per-launch timing of the hop kernel (CUDA events on the launching stream), by class:
+    // 0 = fp16 storage, 1 = fp32, 2 = fp64
+    int prof_on;
+    struct ProfRec { cudaEvent_t e0, e1; int cls; double bytes, flops; };
+    std::vector<ProfRec> prof_pending;
+    std::vector<cudaEvent_t> prof_pool;
+    double prof_ms[3], prof_bytes[3], prof_flops[3];
+    long long prof_n[3];
     int sm_count;
     const GaugeSet* find_gauge(int prec, int recon) const {
         for (size_t i = 0; i < gauges.size(); ++i)

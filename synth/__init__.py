@@ -178,3 +178,18 @@ def gaussian_smeared_sources_4d(dims, width: float = 3.0, t0: int = 0) -> torch.
         for c in range(3):
             eta[3 * sp + c, :, sp, c] = p
     return eta
+
+
+def gaussian_spinor_device(dims, Ls: int, nrhs: int, seed: int, device="cuda", out=None) -> torch.Tensor:
+    """Full-size workloads only (bench.py, full-size parity tests): the same N(0,1)+iN(0,1) field as
+    gaussian_spinor but drawn by the DEVICE generator (seeded; one rhs at a time to bound memory), because
+    drawing 54 GB on the host would dominate the run.  The stream differs from the CPU-drawn one, so a
+    check that needs the oracle copies the slices it wants back to the host."""
+    V4 = int(np.prod(dims))
+    if out is None:
+        out = torch.empty((nrhs, Ls, V4, 4, 3), dtype=torch.complex128, device=device)
+    g = torch.Generator(device=device)
+    for r in range(nrhs):
+        g.manual_seed(int(seed) * 1000 + r)
+        torch.view_as_real(out[r]).normal_(0.0, 1.0, generator=g)
+    return out
