@@ -13,7 +13,7 @@ from dataclasses import dataclass
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libmdwf.so")
+LIB_PATH = os.environ.get("MDWF_LIB", os.path.join(_HERE, "libmdwf.so"))   # MDWF_LIB: alternative build of the same library
 
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 NOT_CONVERGED, BREAKDOWN = 1, 2

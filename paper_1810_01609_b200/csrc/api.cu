@@ -132,7 +132,8 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     for (int m = 0; m < 4; ++m) g.bc[m] = geo->bc[m];
     g.dLs = make_fastdiv(g.Ls); g.dXH = make_fastdiv(g.XH); g.dY = make_fastdiv(g.Y); g.dZ = make_fastdiv(g.Z);
     set_zc(c, pick_zc(c, 0));
-    c->block = (256 / g.Ls) * g.Ls;
+    // threads per block: whole (site, all s) groups, at most 32 sites (bounds the staged-link shared memory)
+    c->block = std::min(256 / g.Ls, 32) * g.Ls;
     c->nblk = (g.N5h + c->block - 1) / c->block;
     MDWF_CUDA(c, cudaMalloc(&c->partial, sizeof(double) * 64 * (size_t)c->nblk));
     MDWF_CUDA(c, cudaMalloc(&c->dscal, sizeof(double) * 8 * 64));

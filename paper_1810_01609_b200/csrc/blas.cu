@@ -3,13 +3,13 @@
 
 namespace mdwf {
 
+static size_t rhs_bytes(const Geom& g, int prec) {
+    const size_t nb = ((size_t)g.N5h + 31) / 32;
+    return nb * (size_t)((24 * (prec / 8) / 16) * 512 + (prec == 16 ? 128 : 0));
+}
 size_t field_bytes(const Geom& g, int prec, int nrhs, size_t* norm_off) {
-    const size_t per = (size_t)g.N5h * 24 * (size_t)(prec / 8);
-    size_t tot = per * nrhs;
-    tot = (tot + 255) & ~(size_t)255;
-    if (norm_off) *norm_off = tot;
-    if (prec == 16) tot += (size_t)g.N5h * 4 * nrhs;
-    return tot;
+    if (norm_off) *norm_off = 0;
+    return rhs_bytes(g, prec) * nrhs;
 }
 
 int alloc_field(mdwf_ctx* c, int prec, int nrhs, mdwf_field** out) {
@@ -28,7 +28,7 @@ int alloc_field(mdwf_ctx* c, int prec, int nrhs, mdwf_field** out) {
         cudaGetLastError();
         MDWF_FAIL(c, MDWF_ENOMEM, "cudaMalloc of %zu bytes for a packed field failed: %s", f->bytes, cudaGetErrorString(e));
     }
-    f->n = prec == 16 ? reinterpret_cast<float*>(reinterpret_cast<char*>(f->v) + noff) : nullptr;
+    f->n = nullptr;
     *out = f;
     return MDWF_OK;
 }
@@ -194,8 +194,8 @@ int launch_pack(mdwf_ctx* c, int prec, bool unpack, PackArgs& a, cudaStream_t st
 mdwf::SpinorView mdwf_field::view() const {
     mdwf::SpinorView s;
     s.v = v;
-    s.n = n;
-    s.rs = (long long)(24 * (prec / 8) / 16) * ctx->g.N5h;   // vectors per rhs: NV * N5h
-    s.rn = ctx->g.N5h;
+    s.n = nullptr;
+    s.rs = (long long)(bytes / nrhs);
+    s.rn = 0;
     return s;
 }

@@ -2,7 +2,8 @@
 // product path (sm_100a).  Private to csrc/.  Shares nothing with oracle/.
 //
 // Packed layouts:
-//   spinor, one parity, one rhs:  vec[c][xh][s]  c = 0..NV-1, 16-byte vectors
+//   spinor, one parity, one rhs:  blocks of 32 consecutive 5D sites, each block = vec[c][lane] c = 0..NV-1,
+//        16-byte vectors (+ 32 fp32 scales for fp16); 5D site idx = xh*Ls + s (s fastest)
 //        fp64: NV = 12 x double2     fp32: NV = 6 x float4     fp16: NV = 3 x (8 x half) + float norm[xh][s]
 //        reals inside a site are in canonical order r = ((spin*3 + colour)*2 + reim), vector c holds
 //        r = c*RPV .. c*RPV+RPV-1.  A thread owns one 5D site idx = xh*Ls + s (s fastest), so a warp
@@ -59,7 +60,7 @@ struct Geom {
 struct SpinorView {
     void* v;          // vectors
     float* n;         // fp16 only: per 5D-site scale
-    long long rs;     // rhs stride in vectors (= NV*N5h)
+    long long rs;     // rhs stride in BYTES (= ceil(N5h/32) * block bytes)
     long long rn;     // rhs stride in norms (= N5h)
 };
 
@@ -102,6 +103,14 @@ __device__ __forceinline__ uint32_t f2h(float a, float b) {
     return *reinterpret_cast<uint32_t*>(&h);
 }
 
+// Blocked layout: 32 consecutive 5D sites form one block of NV rows of 32 x 16 bytes (+ 32 fp32 scales for
+// fp16), so all vectors of a site sit within BLK bytes (one DRAM page, constant offsets between rows).
+template <typename S> struct Blk { static constexpr int BYTES = Store<S>::NV * 512 + (Store<S>::HALF ? 128 : 0); };
+template <typename S>
+__device__ __forceinline__ const char* site_ptr(const SpinorView& f, int r, int idx) {
+    return reinterpret_cast<const char*>(f.v) + (long long)r * f.rs + (long long)(idx >> 5) * Blk<S>::BYTES + (idx & 31) * 16;
+}
+
 // load the 24 reals of 5D site `idx` of rhs `r`.  fp16: returns the UNSCALED values and the scale
 // (callers fold the scale into a later multiply); other types: scale = 1.
 template <typename S>
@@ -111,10 +120,10 @@ __device__ __forceinline__ void load_raw(const SpinorView& f, int r, int idx, in
 template <>
 __device__ __forceinline__ void load_raw<double>(const SpinorView& f, int r, int idx, int N5h, double v[24],
                                                  double& scale) {
-    const double2* p = reinterpret_cast<const double2*>(f.v) + (long long)r * f.rs + idx;
+    const char* p = site_ptr<double>(f, r, idx);
 #pragma unroll
     for (int c = 0; c < 12; ++c) {
-        double2 t = ldg(p + (long long)c * N5h);
+        double2 t = ldg(reinterpret_cast<const double2*>(p + c * 512));
         v[2 * c] = t.x;
         v[2 * c + 1] = t.y;
     }
@@ -123,10 +132,10 @@ __device__ __forceinline__ void load_raw<double>(const SpinorView& f, int r, int
 template <>
 __device__ __forceinline__ void load_raw<float>(const SpinorView& f, int r, int idx, int N5h, float v[24],
                                                 float& scale) {
-    const float4* p = reinterpret_cast<const float4*>(f.v) + (long long)r * f.rs + idx;
+    const char* p = site_ptr<float>(f, r, idx);
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
-        float4 t = ldg(p + (long long)c * N5h);
+        float4 t = ldg(reinterpret_cast<const float4*>(p + c * 512));
         v[4 * c] = t.x;
         v[4 * c + 1] = t.y;
         v[4 * c + 2] = t.z;
@@ -137,11 +146,11 @@ __device__ __forceinline__ void load_raw<float>(const SpinorView& f, int r, int 
 template <>
 __device__ __forceinline__ void load_raw<__half>(const SpinorView& f, int r, int idx, int N5h, float v[24],
                                                  float& scale) {
-    const uint4* p = reinterpret_cast<const uint4*>(f.v) + (long long)r * f.rs + idx;
-    scale = __ldg(f.n + (long long)r * f.rn + idx);
+    const char* p = site_ptr<__half>(f, r, idx);
+    scale = __ldg(reinterpret_cast<const float*>(p - (idx & 31) * 12 + 3 * 512));
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        uint4 t = ldg(p + (long long)c * N5h);
+        uint4 t = ldg(reinterpret_cast<const uint4*>(p + c * 512));
         float2 a = h2f(t.x), b = h2f(t.y), cc = h2f(t.z), d = h2f(t.w);
         v[8 * c] = a.x; v[8 * c + 1] = a.y; v[8 * c + 2] = b.x; v[8 * c + 3] = b.y;
         v[8 * c + 4] = cc.x; v[8 * c + 5] = cc.y; v[8 * c + 6] = d.x; v[8 * c + 7] = d.y;
@@ -166,16 +175,17 @@ __device__ __forceinline__ void store_spinor(const SpinorView& f, int r, int idx
 template <>
 __device__ __forceinline__ void store_spinor<double>(const SpinorView& f, int r, int idx, int N5h,
                                                      const double v[24]) {
-    double2* p = reinterpret_cast<double2*>(f.v) + (long long)r * f.rs + idx;
+    char* p = const_cast<char*>(site_ptr<double>(f, r, idx));
 #pragma unroll
-    for (int c = 0; c < 12; ++c) p[(long long)c * N5h] = make_double2(v[2 * c], v[2 * c + 1]);
+    for (int c = 0; c < 12; ++c) *reinterpret_cast<double2*>(p + c * 512) = make_double2(v[2 * c], v[2 * c + 1]);
 }
 template <>
 __device__ __forceinline__ void store_spinor<float>(const SpinorView& f, int r, int idx, int N5h,
                                                     const float v[24]) {
-    float4* p = reinterpret_cast<float4*>(f.v) + (long long)r * f.rs + idx;
+    char* p = const_cast<char*>(site_ptr<float>(f, r, idx));
 #pragma unroll
-    for (int c = 0; c < 6; ++c) p[(long long)c * N5h] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
+    for (int c = 0; c < 6; ++c)
+        *reinterpret_cast<float4*>(p + c * 512) = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
 }
 // fp16: per-site max-norm scale (fp32) + IEEE half mantissas in [-1,1] ("16-bit storage, single-precision
 // computation"; format choice: SURVEY A11 / DESIGN.md reading R11)
@@ -186,8 +196,8 @@ __device__ __forceinline__ void store_spinor<__half>(const SpinorView& f, int r,
 #pragma unroll
     for (int i = 0; i < 24; ++i) m = fmaxf(m, fabsf(v[i]));
     const float inv = m > 0.f ? __fdividef(1.0f, m) : 0.f;
-    f.n[(long long)r * f.rn + idx] = m;
-    uint4* p = reinterpret_cast<uint4*>(f.v) + (long long)r * f.rs + idx;
+    char* p = const_cast<char*>(site_ptr<__half>(f, r, idx));
+    *reinterpret_cast<float*>(p - (idx & 31) * 12 + 3 * 512) = m;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         uint4 t;
@@ -195,7 +205,7 @@ __device__ __forceinline__ void store_spinor<__half>(const SpinorView& f, int r,
         t.y = f2h(v[8 * c + 2] * inv, v[8 * c + 3] * inv);
         t.z = f2h(v[8 * c + 4] * inv, v[8 * c + 5] * inv);
         t.w = f2h(v[8 * c + 6] * inv, v[8 * c + 7] * inv);
-        p[(long long)c * N5h] = t;
+        *reinterpret_cast<uint4*>(p + c * 512) = t;
     }
 }
 
@@ -246,6 +256,10 @@ MDWF_LINK_LOADERS(18)
 MDWF_LINK_LOADERS(12)
 MDWF_LINK_LOADERS(8)
 #undef MDWF_LINK_LOADERS
+
+template <typename T> __device__ __forceinline__ T fma_(T a, T b, T c);
+template <> __device__ __forceinline__ float fma_<float>(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+template <> __device__ __forceinline__ double fma_<double>(double a, double b, double c) { return __fma_rn(a, b, c); }
 
 template <typename T> __device__ __forceinline__ void sincos_(T a, T& s, T& c);
 template <> __device__ __forceinline__ void sincos_<double>(double a, double& s, double& c) { sincos(a, &s, &c); }

@@ -80,36 +80,20 @@ __device__ __forceinline__ void su3_mul(const T U[18], const T h[12], T w[12]) {
     for (int k = 0; k < 2; ++k)
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
-            T re = 0, im = 0;
+            T re, im;
 #pragma unroll
             for (int j = 0; j < 3; ++j) {
                 const T ur = ADJ ? U[(j * 3 + i) * 2] : U[(i * 3 + j) * 2];
                 const T ui = ADJ ? -U[(j * 3 + i) * 2 + 1] : U[(i * 3 + j) * 2 + 1];
                 const T hr = h[k * 6 + j * 2], hi = h[k * 6 + j * 2 + 1];
-                re += ur * hr - ui * hi;
-                im += ur * hi + ui * hr;
+                if (j == 0) { re = ur * hr; im = ur * hi; }
+                else { re = fma_<T>(ur, hr, re); im = fma_<T>(ur, hi, im); }
+                re = fma_<T>(-ui, hi, re);
+                im = fma_<T>(ui, hr, im);
             }
             w[k * 6 + i * 2] = re;
             w[k * 6 + i * 2 + 1] = im;
         }
-}
-
-// one of the eight stencil legs.  FWD: neighbour x+mu, link U_mu(x) (parity p array at xh);
-// !FWD: neighbour x-mu, link U_mu(x-mu)^dag (parity pbar array at the neighbour's xh).
-template <typename S, int R, int MU, bool FWD, bool DAG>
-__device__ __forceinline__ void leg(const SpinorView& in, const GaugeView& gv, int rhs, int N5h, int Ls, int Vh,
-                                    int par, int xh, int nxh, int s, typename Store<S>::real bcs,
-                                    typename Store<S>::real acc[24]) {
-    typedef typename Store<S>::real T;
-    constexpr int SGN = (FWD ? -1 : 1) * (DAG ? -1 : 1);
-    T v[24], sc;
-    load_raw<S>(in, rhs, nxh * Ls + s, N5h, v, sc);
-    T h[12], w[12], U[18];
-    project<MU, SGN, T>(v, h);
-    if (FWD) load_link<S, R>(gv.v[par], MU, xh, Vh, U);
-    else load_link<S, R>(gv.v[1 - par], MU, nxh, Vh, U);
-    su3_mul<!FWD, T>(U, h, w);
-    recon<MU, SGN, T>(w, sc * bcs, acc);
 }
 
 template <typename T> struct alignas(16) Pack16 {
@@ -173,6 +157,65 @@ __device__ __forceinline__ void block_sum_store(double v, unsigned char* smem_ra
     if (threadIdx.x == 0) *dst = red[0];
 }
 
+// ---- links staged in shared memory ------------------------------------------------------------------
+// Per block: for each of its 4D sites the 8 stencil links, reconstructed to 18 reals of the compute type,
+// already daggered for the backward legs and multiplied by the boundary sign, plus the 8 neighbour
+// half-indices and the site's own half-index.  Every thread of a site (all Ls slices) then reads the same
+// link rows (broadcast) -- "staging of links reused across the Ls slices" (north_star).
+//   smem link row: 20 reals (16-byte aligned); site stride 8*20+4 reals (keeps 16-byte reads of the sites
+//   of one warp in different banks); index table: 12 ints per site (8 neighbours, own xh, pad).
+#ifndef MDWF_HOP_MINB
+#define MDWF_HOP_MINB 3
+#endif
+#define MDWF_LROW 20
+#define MDWF_LSITE (8 * MDWF_LROW + 4)
+template <typename T> __host__ __device__ inline size_t smem_bytes_links(int nsite) {
+    return (size_t)nsite * (MDWF_LSITE * sizeof(T) + 12 * sizeof(int));
+}
+
+// one stencil leg from staged data: U (smem, already U or U^dag, sign folded), neighbour 5D index nidx
+template <typename S, int MU, bool FWD, bool DAG>
+__device__ __forceinline__ void leg2(const SpinorView& in, int rhs, int N5h, int nidx,
+                                     const typename Store<S>::real* __restrict__ Us,
+                                     typename Store<S>::real acc[24]) {
+    typedef typename Store<S>::real T;
+    constexpr int SGN = (FWD ? -1 : 1) * (DAG ? -1 : 1);
+    T v[24], sc;
+    load_raw<S>(in, rhs, nidx, N5h, v, sc);
+    T h[12], w[12], U[MDWF_LROW];
+    project<MU, SGN, T>(v, h);
+    typedef Pack16<T> P;
+#pragma unroll
+    for (int q = 0; q < MDWF_LROW / P::N; ++q) {
+        if (q * P::N >= 18) break;
+        const P t = reinterpret_cast<const P*>(Us)[q];
+#pragma unroll
+        for (int e = 0; e < P::N; ++e) U[q * P::N + e] = t.d[e];
+    }
+    su3_mul<false, T>(U, h, w);
+    // acc += sc * (rebuilt spinor), explicit FMAs (24 per leg)
+    const T cs = sc * (T)SGN;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const T w0r = w[c * 2], w0i = w[c * 2 + 1], w1r = w[6 + c * 2], w1i = w[6 + c * 2 + 1];
+        acc[c * 2] = fma_<T>(sc, w0r, acc[c * 2]); acc[c * 2 + 1] = fma_<T>(sc, w0i, acc[c * 2 + 1]);
+        acc[6 + c * 2] = fma_<T>(sc, w1r, acc[6 + c * 2]); acc[6 + c * 2 + 1] = fma_<T>(sc, w1i, acc[6 + c * 2 + 1]);
+        if (MU == 0) {
+            acc[12 + c * 2] = fma_<T>(cs, w1i, acc[12 + c * 2]); acc[12 + c * 2 + 1] = fma_<T>(-cs, w1r, acc[12 + c * 2 + 1]);
+            acc[18 + c * 2] = fma_<T>(cs, w0i, acc[18 + c * 2]); acc[18 + c * 2 + 1] = fma_<T>(-cs, w0r, acc[18 + c * 2 + 1]);
+        } else if (MU == 1) {
+            acc[12 + c * 2] = fma_<T>(cs, w1r, acc[12 + c * 2]); acc[12 + c * 2 + 1] = fma_<T>(cs, w1i, acc[12 + c * 2 + 1]);
+            acc[18 + c * 2] = fma_<T>(-cs, w0r, acc[18 + c * 2]); acc[18 + c * 2 + 1] = fma_<T>(-cs, w0i, acc[18 + c * 2 + 1]);
+        } else if (MU == 2) {
+            acc[12 + c * 2] = fma_<T>(cs, w0i, acc[12 + c * 2]); acc[12 + c * 2 + 1] = fma_<T>(-cs, w0r, acc[12 + c * 2 + 1]);
+            acc[18 + c * 2] = fma_<T>(-cs, w1i, acc[18 + c * 2]); acc[18 + c * 2 + 1] = fma_<T>(cs, w1r, acc[18 + c * 2 + 1]);
+        } else {
+            acc[12 + c * 2] = fma_<T>(cs, w0r, acc[12 + c * 2]); acc[12 + c * 2 + 1] = fma_<T>(cs, w0i, acc[12 + c * 2 + 1]);
+            acc[18 + c * 2] = fma_<T>(cs, w1r, acc[18 + c * 2]); acc[18 + c * 2 + 1] = fma_<T>(cs, w1i, acc[18 + c * 2 + 1]);
+        }
+    }
+}
+
 struct HopArgs {
     SpinorView out, in, xin;   // xin.v == nullptr -> no xpay term
     GaugeView g;
@@ -184,81 +227,106 @@ struct HopArgs {
     int rhs_list[64];
 };
 
-// thread linear index within a rhs -> (xh, s, coordinates) through the slab traversal
-struct SiteCoord { int xh, s, xx, y, z, t, o; };
-__device__ __forceinline__ SiteCoord decode_site(const Geom& g, int par, uint32_t j) {
+// 4D site index in the slab traversal -> coordinates
+struct SiteCoord { int xh, xx, y, z, t, o; };
+__device__ __forceinline__ SiteCoord decode_site(const Geom& g, int par, uint32_t site) {
     SiteCoord c;
-    uint32_t site, s;
-    g.dLs.divmod(j, site, s);
     uint32_t zcI, rem, t, rem2, row, xx, zl, y;
     g.dTslab.divmod(site, zcI, rem);
     g.dSlab.divmod(rem, t, rem2);
     g.dXH.divmod(rem2, row, xx);
     g.dY.divmod(row, zl, y);
-    c.s = s; c.xx = xx; c.y = y; c.z = zcI * g.zc + zl; c.t = t;
+    c.xx = xx; c.y = y; c.z = zcI * g.zc + zl; c.t = t;
     c.o = (par + c.y + c.z + c.t) & 1;                 // x = 2*xx + o
     c.xh = xx + g.XH * (c.y + g.Y * (c.z + g.Z * c.t));
     return c;
 }
 
 template <typename S, int R, bool DAG, bool FUSED>
-__global__ void __launch_bounds__(256) hop_kernel(const Geom g, const HopArgs a) {
+__global__ void __launch_bounds__(256, (sizeof(typename Store<S>::real) == 8 ? 1 : MDWF_HOP_MINB)) hop_kernel(const Geom g, const HopArgs a) {
     typedef typename Store<S>::real T;
+    typedef Pack16<T> P;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int Ls = g.Ls;
+    const int nsite = blockDim.x / Ls;
+    T* links = reinterpret_cast<T*>(smem_raw);
+    int* tab = reinterpret_cast<int*>(smem_raw + (size_t)nsite * MDWF_LSITE * sizeof(T));
+    unsigned char* smem_epi = smem_raw + smem_bytes_links<T>(nsite);
     const int slot = blockIdx.x % a.nact;
     const int tile = blockIdx.x / a.nact;
     const int rhs = a.rhs_list[slot];
-    const uint32_t j = (uint32_t)tile * blockDim.x + threadIdx.x;
-    const bool live = j < (uint32_t)g.N5h;
+    const int site0 = tile * nsite;
+    // ---- stage the block's links and neighbour table --------------------------------------------------
+    for (int task = threadIdx.x; task < nsite * 8; task += blockDim.x) {
+        const int i = task >> 3, l = task & 7, mu = l >> 1;
+        const bool fwd = (l & 1) == 0;
+        const int jsite = site0 + i;
+        if (jsite >= g.Vh) continue;
+        const SiteCoord c = decode_site(g, a.par, (uint32_t)jsite);
+        const int xh = c.xh;
+        int n;
+        bool wrap;
+        if (mu == 0) {
+            if (fwd) { wrap = (c.o == 1 && c.xx == g.XH - 1); n = wrap ? xh - (g.XH - 1) : xh + c.o; }
+            else { wrap = (c.o == 0 && c.xx == 0); n = wrap ? xh + (g.XH - 1) : xh - (1 - c.o); }
+        } else {
+            const int cm = mu == 1 ? c.y : mu == 2 ? c.z : c.t;
+            const int Lm = mu == 1 ? g.Y : mu == 2 ? g.Z : g.T;
+            const int sm = mu == 1 ? g.XH : mu == 2 ? g.XH * g.Y : g.XH * g.Y * g.Z;
+            if (fwd) { wrap = cm == Lm - 1; n = wrap ? xh - (Lm - 1) * sm : xh + sm; }
+            else { wrap = cm == 0; n = wrap ? xh + (Lm - 1) * sm : xh - sm; }
+        }
+        const T sgn = wrap ? (T)g.bc[mu] : (T)1;
+        T U[18], V[MDWF_LROW];
+        load_link<S, R>(fwd ? a.g.v[a.par] : a.g.v[1 - a.par], mu, fwd ? xh : n, g.Vh, U);
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) {
+                V[(r * 3 + cc) * 2] = sgn * (fwd ? U[(r * 3 + cc) * 2] : U[(cc * 3 + r) * 2]);
+                V[(r * 3 + cc) * 2 + 1] = sgn * (fwd ? U[(r * 3 + cc) * 2 + 1] : -U[(cc * 3 + r) * 2 + 1]);
+            }
+        V[18] = V[19] = 0;
+        P* dst = reinterpret_cast<P*>(links + i * MDWF_LSITE + l * MDWF_LROW);
+#pragma unroll
+        for (int q = 0; q < MDWF_LROW / P::N; ++q) {
+            P t;
+#pragma unroll
+            for (int e = 0; e < P::N; ++e) t.d[e] = V[q * P::N + e];
+            dst[q] = t;
+        }
+        tab[i * 12 + l] = n;
+        if (l == 0) tab[i * 12 + 8] = xh;
+    }
+    __syncthreads();
+    // ---- the stencil: one thread per (site, s) -----------------------------------------------------------
+    const int grp = (int)g.dLs.div(threadIdx.x), s = threadIdx.x - grp * Ls;
+    const bool live = grp < nsite && site0 + grp < g.Vh;
     T acc[24];
 #pragma unroll
     for (int i = 0; i < 24; ++i) acc[i] = 0;
     int idx = 0;
     if (live) {
-        const SiteCoord c = decode_site(g, a.par, j);
-        const int xh = c.xh, s = c.s, Ls = g.Ls, Vh = g.Vh, N5h = g.N5h;
-        idx = xh * Ls + s;
-        const int sy = g.XH, sz = g.XH * g.Y, st = g.XH * g.Y * g.Z;
-        // x: neighbours live in the other parity's half-index space
-        {
-            int nf = xh + c.o, nb = xh - (1 - c.o);
-            T bf = 1, bb = 1;
-            if (c.o == 1 && c.xx == g.XH - 1) { nf = xh - (g.XH - 1); bf = (T)g.bc[0]; }
-            if (c.o == 0 && c.xx == 0) { nb = xh + (g.XH - 1); bb = (T)g.bc[0]; }
-            leg<S, R, 0, true, DAG>(a.in, a.g, rhs, N5h, Ls, Vh, a.par, xh, nf, s, bf, acc);
-            leg<S, R, 0, false, DAG>(a.in, a.g, rhs, N5h, Ls, Vh, a.par, xh, nb, s, bb, acc);
-        }
-        {
-            int nf = xh + sy, nb = xh - sy;
-            T bf = 1, bb = 1;
-            if (c.y == g.Y - 1) { nf = xh - (g.Y - 1) * sy; bf = (T)g.bc[1]; }
-            if (c.y == 0) { nb = xh + (g.Y - 1) * sy; bb = (T)g.bc[1]; }
-            leg<S, R, 1, true, DAG>(a.in, a.g, rhs, N5h, Ls, Vh, a.par, xh, nf, s, bf, acc);
-            leg<S, R, 1, false, DAG>(a.in, a.g, rhs, N5h, Ls, Vh, a.par, xh, nb, s, bb, acc);
-        }
-        {
-            int nf = xh + sz, nb = xh - sz;
-            T bf = 1, bb = 1;
-            if (c.z == g.Z - 1) { nf = xh - (g.Z - 1) * sz; bf = (T)g.bc[2]; }
-            if (c.z == 0) { nb = xh + (g.Z - 1) * sz; bb = (T)g.bc[2]; }
-            leg<S, R, 2, true, DAG>(a.in, a.g, rhs, N5h, Ls, Vh, a.par, xh, nf, s, bf, acc);
-            leg<S, R, 2, false, DAG>(a.in, a.g, rhs, N5h, Ls, Vh, a.par, xh, nb, s, bb, acc);
-        }
-        {
-            int nf = xh + st, nb = xh - st;
-            T bf = 1, bb = 1;
-            if (c.t == g.T - 1) { nf = xh - (g.T - 1) * st; bf = (T)g.bc[3]; }
-            if (c.t == 0) { nb = xh + (g.T - 1) * st; bb = (T)g.bc[3]; }
-            leg<S, R, 3, true, DAG>(a.in, a.g, rhs, N5h, Ls, Vh, a.par, xh, nf, s, bf, acc);
-            leg<S, R, 3, false, DAG>(a.in, a.g, rhs, N5h, Ls, Vh, a.par, xh, nb, s, bb, acc);
-        }
+        const int4 n0 = reinterpret_cast<const int4*>(tab + grp * 12)[0];
+        const int4 n1 = reinterpret_cast<const int4*>(tab + grp * 12)[1];
+        idx = tab[grp * 12 + 8] * Ls + s;
+        const T* Ub = links + grp * MDWF_LSITE;
+        const int N5h = g.N5h;
+        leg2<S, 0, true, DAG>(a.in, rhs, N5h, n0.x * Ls + s, Ub + 0 * MDWF_LROW, acc);
+        leg2<S, 0, false, DAG>(a.in, rhs, N5h, n0.y * Ls + s, Ub + 1 * MDWF_LROW, acc);
+        leg2<S, 1, true, DAG>(a.in, rhs, N5h, n0.z * Ls + s, Ub + 2 * MDWF_LROW, acc);
+        leg2<S, 1, false, DAG>(a.in, rhs, N5h, n0.w * Ls + s, Ub + 3 * MDWF_LROW, acc);
+        leg2<S, 2, true, DAG>(a.in, rhs, N5h, n1.x * Ls + s, Ub + 4 * MDWF_LROW, acc);
+        leg2<S, 2, false, DAG>(a.in, rhs, N5h, n1.y * Ls + s, Ub + 5 * MDWF_LROW, acc);
+        leg2<S, 3, true, DAG>(a.in, rhs, N5h, n1.z * Ls + s, Ub + 6 * MDWF_LROW, acc);
+        leg2<S, 3, false, DAG>(a.in, rhs, N5h, n1.w * Ls + s, Ub + 7 * MDWF_LROW, acc);
     }
     if (!FUSED) {
         if (live) store_spinor<S>(a.out, rhs, idx, g.N5h, acc);
         return;
     }
     // ---- fused epilogue: s-direction matrix, xpay, optional |out|^2 ---------------------------
-    if (a.G != nullptr) apply_G<T>(acc, a.G, g.Ls, smem_raw);
+    if (a.G != nullptr) apply_G<T>(acc, a.G, g.Ls, smem_epi);
     const T ch = (T)a.ch;
     if (a.xin.v != nullptr) {
         if (live) {
@@ -279,7 +347,7 @@ __global__ void __launch_bounds__(256) hop_kernel(const Geom g, const HopArgs a)
 #pragma unroll
             for (int i = 0; i < 24; ++i) s2 += (double)acc[i] * (double)acc[i];
         }
-        block_sum_store(s2, smem_raw, a.partial + (long long)slot * (gridDim.x / a.nact) + tile);
+        block_sum_store(s2, smem_epi, a.partial + (long long)slot * (gridDim.x / a.nact) + tile);
     }
 }
 

@@ -29,6 +29,7 @@ static int launch_hop_SR(mdwf_ctx* c, int dagger, int fused, HopArgs& a, cudaStr
         smem = (size_t)c->block * sizeof(double);
         if (a.G) smem = std::max(smem, (size_t)smem_reals_G<T>(c->g.Ls, c->block) * sizeof(T));
     }
+    smem += smem_bytes_links<T>(c->block / c->g.Ls);
     if (fused) {
         if (dagger) return launch_with_smem(c, hop_kernel<S, R, true, true>, grid, c->block, smem, st, c->g, a);
         return launch_with_smem(c, hop_kernel<S, R, false, true>, grid, c->block, smem, st, c->g, a);

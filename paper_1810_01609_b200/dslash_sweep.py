@@ -1,0 +1,81 @@
+"""Dslash throughput sweep (BASELINE.json configs[1]: "Dslash-only throughput sweep in fp64/fp32/fp16
+storage with 18-, 12- and 8-real link formats"), through the packed C-ABI calls.
+
+    python -m paper_1810_01609_b200.dslash_sweep --config 2 [--nrhs 1] [--formats 32x12,16x12] [--ops hop,mhat]
+                                                  [--iters 20] [--rotate 4] [--zc 0]
+
+Prints one JSON line per (format, op): device time per call (CUDA events around `iters` back-to-back
+calls), algorithmic GB/s and GFLOP/s under DESIGN.md's cost convention, fraction of the measured HBM peak.
+--rotate R cycles over R independent in/out buffer sets so that small lattices are not L2-resident.
+"""
+import argparse
+import json
+import os
+import sys
+
+import torch
+
+sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+import synth  # noqa: E402
+import paper_1810_01609_b200 as mdwf  # noqa: E402
+
+OPS = {"hop": mdwf.OP_HOP, "mhat": mdwf.OP_DHAT_SYM, "dhat": mdwf.OP_DHAT_ASYM, "m5inv": mdwf.OP_M5INV,
+       "normal": mdwf.OP_NORMAL_SYM}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--nrhs", type=int, default=1)
+    ap.add_argument("--formats", default="64x18,64x12,64x8,32x18,32x12,32x8,16x18,16x12,16x8")
+    ap.add_argument("--ops", default="hop,mhat")
+    ap.add_argument("--iters", type=int, default=20)
+    ap.add_argument("--rotate", type=int, default=4)
+    ap.add_argument("--zc", type=int, default=0)
+    ap.add_argument("--dagger", type=int, default=0)
+    a = ap.parse_args()
+    cfg = synth.CONFIGS[a.config]
+    peak = 6650.0
+    pk = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "MEASURED_PEAKS.json")
+    if os.path.exists(pk):
+        peak = float(json.load(open(pk))["hbm_gbs"])
+    ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
+    ctx.mdwf_set_tiling(a.zc)
+    U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(cfg.index, 1), device="cuda")
+    fmts = [tuple(int(v) for v in f.split("x")) for f in a.formats.split(",")]
+    for prec, recon in fmts:
+        ctx.mdwf_load_gauge(U, prec, recon)
+    del U
+    torch.cuda.empty_cache()
+    Vh = cfg.V4 // 2
+    g = torch.Generator(device="cuda").manual_seed(synth.seed_for(cfg.index, 2))
+    for prec, recon in fmts:
+        fin = [ctx.mdwf_field_create(prec, a.nrhs) for _ in range(a.rotate)]
+        fout = [ctx.mdwf_field_create(prec, a.nrhs) for _ in range(a.rotate)]
+        for f in fin:
+            src = torch.empty((a.nrhs, cfg.Ls, Vh, 4, 3), dtype=torch.complex128, device="cuda")
+            torch.view_as_real(src).normal_(0.0, 1.0, generator=g)
+            f.mdwf_field_pack(src)
+            del src
+        for name in a.ops.split(","):
+            op = OPS[name]
+            for k in range(3):
+                ctx.mdwf_dslash_packed(op, fout[k % a.rotate], fin[k % a.rotate], 0, bool(a.dagger), recon)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for k in range(a.iters):
+                ctx.mdwf_dslash_packed(op, fout[k % a.rotate], fin[k % a.rotate], 0, bool(a.dagger), recon)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / a.iters
+            by, fl = ctx.mdwf_dslash_cost(op, prec, recon, a.nrhs)
+            print(json.dumps({"workload": cfg.name, "nrhs": a.nrhs, "prec": prec, "recon": recon, "op": name,
+                              "ms": round(ms, 5), "GBps": round(by / ms / 1e6, 1), "GFLOPs": round(fl / ms / 1e6, 1),
+                              "frac_of_measured_hbm": round(by / ms / 1e6 / peak, 4), "rotate": a.rotate}), flush=True)
+        for f in fin + fout:
+            f.mdwf_field_destroy()
+
+
+if __name__ == "__main__":
+    main()
