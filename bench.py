@@ -66,6 +66,23 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.rows), "reasons": reasons}
 
 
+def max_over_ranks(ms, world, device=None):
+    """Multi-GPU timing rule: every rank times on its own device, the job's time is the MAX over ranks.
+    (The path does not shard -- "replicas only" -- so this reduce is the only collective; gloo on CPU in tests.)"""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate(sec_per_rhs_per_replica, world):
+    """N independent replicas finish N*nrhs solves in the time one replica needs for nrhs: whole-job s/RHS."""
+    return sec_per_rhs_per_replica / world
+
+
 def oracle_baseline(cfg, budget_s=20.0):
     """The CPU oracle as it stands (oracle.solve_eo: its own even-odd CG, fp64, OpenMP over the host cores),
     timed on a bounded sample of the workload: the same operator parameters and link recipe on a small
@@ -174,10 +191,7 @@ def run_ours(args):
     launches = ctx.mdwf_launch_count() - l0
     prof = {c: ctx.mdwf_profile_read(c) for c in (0, 1, 2)}
     ctx.mdwf_profile(False)
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, world, dev)
     ms_step = ms_total / args.steps
     sec_per_rhs = ms_step * 1e-3 / nrhs          # per replica; N replicas solve N*nrhs in the same time
 
@@ -238,10 +252,7 @@ def run_e2e(st, args):
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1)
-    if st["world"] > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=st["dev"])
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, st["world"], st["dev"])
     return {"value": ms * 1e-3 / args.e2e_steps / nrhs, "unit": "s/RHS", "h2d_bytes_per_step": nbytes,
             "d2h_bytes_per_step": nbytes, "steps": args.e2e_steps, "warmup": args.e2e_warmup, "pinned_host": pinned,
             "api": "mdwf_solve_host"}
@@ -272,7 +283,7 @@ def main():
     e2e = None if args.no_e2e else run_e2e(st, args)
     if st["rank"] != 0:
         return
-    line = {"metric": METRIC, "value": st["sec_per_rhs"] / world, "unit": "s/RHS", "n_gpus": world,
+    line = {"metric": METRIC, "value": aggregate(st["sec_per_rhs"], world), "unit": "s/RHS", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": st["ms_step"], "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": {16: "f16 storage / f32 compute / f64 outer", 32: "f32 / f64 outer", 64: "f64"}[args.inner],
             "data": "synthetic",
@@ -284,7 +295,7 @@ def main():
                    "true_resid": res.true_resid, "seconds_inner_last_step": res.seconds_inner, "seconds_last_step": res.seconds},
             "dslash": st["dsl"], "roofline": st["roof"], "gpu_launches": st["launches"], "clocks": st["clocks"]}
     if e2e is not None:
-        e2e["value"] = e2e["value"] / world
+        e2e["value"] = aggregate(e2e["value"], world)
         line["e2e"] = e2e
     if world == 1 and not args.no_cpu_baseline:
         base, per = oracle_baseline(cfg)

@@ -24,7 +24,7 @@ EXPORTS = [
     "mdwf_create", "mdwf_destroy", "mdwf_last_error", "mdwf_load_gauge", "mdwf_dslash", "mdwf_field_create",
     "mdwf_field_destroy", "mdwf_field_pack", "mdwf_field_unpack", "mdwf_dslash_packed", "mdwf_dslash_cost",
     "mdwf_solve", "mdwf_solve_host", "mdwf_seq_source", "mdwf_nucleon_2pt", "mdwf_wall_inject",
-    "mdwf_wall_project", "mdwf_launch_count", "mdwf_set_tiling", "mdwf_profile", "mdwf_profile_read",
+    "mdwf_wall_project", "mdwf_launch_count", "mdwf_set_tiling", "mdwf_profile", "mdwf_profile_read", "mdwf_selftest_host",
 ]
 
 
@@ -89,6 +89,7 @@ def lib():
         L.mdwf_profile.argtypes = [vp, ci]
         L.mdwf_profile_read.argtypes = [vp, ci, ctypes.POINTER(cd), ctypes.POINTER(cd), ctypes.POINTER(cd),
                                         ctypes.POINTER(ctypes.c_int64)]
+        L.mdwf_selftest_host.argtypes = [cd, cd, cd, cd]
         _lib = L
     return _lib
 
@@ -123,6 +124,11 @@ class SolveResult:
     seconds: float
     seconds_inner: float
     kernel_launches: int
+
+
+def mdwf_selftest_host(M5=1.3, b5=1.5, c5=0.5, mf=0.05):
+    """Host-only checks of the library's index arithmetic and s-direction matrices (no GPU needed)."""
+    return int(lib().mdwf_selftest_host(M5, b5, c5, mf))
 
 
 class Field:

@@ -60,15 +60,15 @@ static void build_matrices(int Ls, double M5, double b5, double c5, double mf, s
     }
 }
 
+// z-slab depth: largest multiple of the tile depth tz dividing Z whose fp32 input slab XH*Y*zc*Ls*96 bytes stays
+// under ~9 MB, so that the three t-consecutive slabs a row of tiles touches (plus the streamed output) live in
+// L2 (measured on B200: 48^3x64 Ls=10 is fastest at zc = 8)
 static int pick_zc(const mdwf_ctx* c, int want) {
     const Geom& g = c->g;
-    if (want > 0 && g.Z % want == 0) return want;
-    // automatic: deepest z-slab whose three-timeslice working set (input gathers + output) of ~4 fp32 rhs
-    // stays within ~1/2 of L2; small lattices use the canonical order (zc = Z)
-    const double per_site = (double)g.Ls * 96.0 * 2.0 * 4.0;
-    int best = 1;
-    for (int z = 1; z <= g.Z; ++z)
-        if (g.Z % z == 0 && 3.0 * g.XH * g.Y * z * per_site <= 48e6) best = z;
+    if (want > 0 && g.Z % want == 0 && want % g.tz == 0) return want;
+    int best = g.tz;
+    for (int z = g.tz; z <= g.Z; z += g.tz)
+        if (g.Z % z == 0 && (double)g.XH * g.Y * z * g.Ls * 96.0 <= 9.0e6) best = z;
     return best;
 }
 static void set_zc(mdwf_ctx* c, int zc) {
@@ -77,6 +77,32 @@ static void set_zc(mdwf_ctx* c, int zc) {
     g.dZc = make_fastdiv(zc);
     g.dSlab = make_fastdiv((uint32_t)(g.XH * g.Y * zc));
     g.dTslab = make_fastdiv((uint32_t)(g.XH * g.Y * zc) * (uint32_t)g.T);
+    g.dnTzs = make_fastdiv((uint32_t)(zc / g.tz));
+}
+// Sites of a block: a box txh*ty*tz*tt (x fastest) that divides the lattice, filled greedily along x, then y, z, t
+// up to min(256/Ls, 32) sites, i.e. (nearly) whole x-rows in storage order.  Compact 4D boxes (e.g. 4x4x2x2) were
+// measured SLOWER on B200 (profiles/README.md, "tile shape"): L1 does not keep the in-box neighbours long enough to
+// merge their eight uses, so the L2->SM traffic does not drop, while coalescing gets worse.
+static void pick_tile(mdwf_ctx* c, int) {
+    Geom& g = c->g;
+    const int cap = std::max(1, std::min(256 / g.Ls, 32));
+    int best[4] = {1, 1, 1, 1};
+    const int ext[4] = {g.XH, g.Y, g.Z, g.T};
+    int n = 1;
+    for (int d = 0; d < 4; ++d) {
+        int pick = 1;
+        for (int k = 1; k <= ext[d] && n * k <= cap; ++k)
+            if (ext[d] % k == 0) pick = k;
+        best[d] = pick;
+        n *= pick;
+        if (pick != ext[d]) break;   // only extend into the next direction when this one is covered completely
+    }
+    g.txh = best[0]; g.ty = best[1]; g.tz = best[2]; g.tt = best[3];
+    g.nsite = g.txh * g.ty * g.tz * g.tt;
+    g.dtxh = make_fastdiv(g.txh); g.dty = make_fastdiv(g.ty); g.dtz = make_fastdiv(g.tz);
+    g.dnTx = make_fastdiv(g.XH / g.txh); g.dnTy = make_fastdiv(g.Y / g.ty); g.dnTt = make_fastdiv(g.T / g.tt);
+    c->block = g.nsite * g.Ls;
+    c->nblk = g.Vh / g.nsite;
 }
 
 static void prof_drain(mdwf_ctx* c) {
@@ -131,10 +157,8 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     g.N5h = g.Vh * g.Ls;
     for (int m = 0; m < 4; ++m) g.bc[m] = geo->bc[m];
     g.dLs = make_fastdiv(g.Ls); g.dXH = make_fastdiv(g.XH); g.dY = make_fastdiv(g.Y); g.dZ = make_fastdiv(g.Z);
+    pick_tile(c, 0);
     set_zc(c, pick_zc(c, 0));
-    // threads per block: whole (site, all s) groups, at most 32 sites (bounds the staged-link shared memory)
-    c->block = std::min(256 / g.Ls, 32) * g.Ls;
-    c->nblk = (g.N5h + c->block - 1) / c->block;
     MDWF_CUDA(c, cudaMalloc(&c->partial, sizeof(double) * 64 * (size_t)c->nblk));
     MDWF_CUDA(c, cudaMalloc(&c->dscal, sizeof(double) * 8 * 64));
     MDWF_CUDA(c, cudaMemset(c->dscal, 0, sizeof(double) * 8 * 64));
@@ -184,9 +208,43 @@ int mdwf_profile_read(mdwf_ctx* c, int cls, double* ms, double* bytes, double* f
     return MDWF_OK;
 }
 
+int mdwf_selftest_host(double M5, double b5, double c5, double mf) {
+    // 1: fast division
+    const uint32_t ds[] = {1, 2, 3, 4, 5, 6, 7, 8, 10, 12, 16, 21, 24, 25, 32, 48, 96, 250, 1152, 9216, 55296, 442368, 3538944};
+    for (uint32_t d : ds) {
+        const FastDiv f = make_fastdiv(d);
+        for (uint32_t n = 0; n < 3000000u; ++n) if (f.div(n) != n / d) return 1;
+        for (uint64_t n = 3000000u; n < (1ull << 31); n += 9973) if (f.div((uint32_t)n) != (uint32_t)n / d) return 1;
+        if (f.div((1u << 31) - 1) != ((1u << 31) - 1) / d) return 1;
+    }
+    // 2, 3: s-direction blocks
+    const double a = b5 * (4.0 - M5) + 1.0, d = c5 * (4.0 - M5) - 1.0;
+    (void)a; (void)d;
+    for (int Ls = 1; Ls <= 32; ++Ls) {
+        std::vector<double> m[MAT_COUNT];
+        build_matrices(Ls, M5, b5, c5, mf, m);
+        const int n = Ls * Ls;
+        for (int ch = 0; ch < 2; ++ch)
+            for (int s = 0; s < Ls; ++s)
+                for (int t = 0; t < Ls; ++t) {
+                    double acc = 0.0, acc2 = 0.0;   // (M5 M5inv)[s][t], (A M5inv)[s][t]; Gt[chi][s'][s] = Mat[s][s']
+                    for (int k = 0; k < Ls; ++k) {
+                        acc += m[MAT_M5][ch * n + k * Ls + s] * m[MAT_M5INV][ch * n + t * Ls + k];
+                        acc2 += m[MAT_A][ch * n + k * Ls + s] * m[MAT_M5INV][ch * n + t * Ls + k];
+                    }
+                    if (std::fabs(acc - (s == t ? 1.0 : 0.0)) > 1e-13) return 2;
+                    if (std::fabs(acc2 - m[MAT_AM5INV][ch * n + t * Ls + s]) > 1e-13) return 2;
+                    for (int id = 0; id < 4; ++id)
+                        if (m[id + 4][ch * n + t * Ls + s] != m[id][ch * n + s * Ls + t]) return 3;
+                }
+    }
+    return 0;
+}
+
 int mdwf_set_tiling(mdwf_ctx* c, int zc) {
     if (!c) return MDWF_EINVAL;
-    if (zc < 0 || (zc > 0 && c->g.Z % zc != 0)) MDWF_FAIL(c, MDWF_EINVAL, "zc = %d must divide Z = %d", zc, c->g.Z);
+    if (zc < 0 || (zc > 0 && (c->g.Z % zc != 0 || zc % c->g.tz != 0)))
+        MDWF_FAIL(c, MDWF_EINVAL, "zc = %d must divide Z = %d and be a multiple of the tile depth %d", zc, c->g.Z, c->g.tz);
     set_zc(c, pick_zc(c, zc));
     return MDWF_OK;
 }

@@ -53,7 +53,12 @@ struct Geom {
     int bc[4];
     int zc;                   // z-slab depth of the hop traversal (divides Z)
     FastDiv dLs, dXH, dY, dZ;       // canonical decode of xh
-    FastDiv dZc, dSlab, dTslab;     // slab traversal decode: slab = XH*Y*zc sites, Tslab = T*slab
+    FastDiv dZc, dSlab, dTslab;     // (unused by the tiled traversal; kept for the linear one)
+    // 4D tiles of the hop kernel: a block owns txh*ty*tz*tt sites (x fastest); tiles are ordered x, y, z within a
+    // z-slab of depth zc, then t, then slab, so that t-neighbours are re-used from L2 and in-tile neighbours from L1
+    int txh, ty, tz, tt, nsite;
+    FastDiv dtxh, dty, dtz;             // in-tile decode
+    FastDiv dnTx, dnTy, dnTzs, dnTt;    // tile-index decode: tiles per row, per column, per slab depth, per T
 };
 
 // one packed spinor field set (nrhs fields of one parity)
@@ -169,35 +174,41 @@ __device__ __forceinline__ void load_spinor(const SpinorView& f, int r, int idx,
     }
 }
 
-template <typename S>
+// st_<CS>: plain store, or streaming store (evict-first: the stencil's output is not re-read before it has
+// left L2, so it should not displace the input sites that neighbouring blocks are about to gather)
+template <bool CS, typename V> __device__ __forceinline__ void st_(V* p, V v) {
+    if (CS) __stcs(p, v); else *p = v;
+}
+template <typename S, bool CS = false>
 __device__ __forceinline__ void store_spinor(const SpinorView& f, int r, int idx, int N5h,
                                              const typename Store<S>::real v[24]);
-template <>
-__device__ __forceinline__ void store_spinor<double>(const SpinorView& f, int r, int idx, int N5h,
-                                                     const double v[24]) {
+template <bool CS>
+__device__ __forceinline__ void store_spinor_d(const SpinorView& f, int r, int idx, const double v[24]) {
     char* p = const_cast<char*>(site_ptr<double>(f, r, idx));
 #pragma unroll
-    for (int c = 0; c < 12; ++c) *reinterpret_cast<double2*>(p + c * 512) = make_double2(v[2 * c], v[2 * c + 1]);
+    for (int c = 0; c < 12; ++c) st_<CS>(reinterpret_cast<double2*>(p + c * 512), make_double2(v[2 * c], v[2 * c + 1]));
 }
-template <>
-__device__ __forceinline__ void store_spinor<float>(const SpinorView& f, int r, int idx, int N5h,
-                                                    const float v[24]) {
+template <> __device__ __forceinline__ void store_spinor<double, false>(const SpinorView& f, int r, int idx, int N5h, const double v[24]) { store_spinor_d<false>(f, r, idx, v); }
+template <> __device__ __forceinline__ void store_spinor<double, true>(const SpinorView& f, int r, int idx, int N5h, const double v[24]) { store_spinor_d<true>(f, r, idx, v); }
+template <bool CS>
+__device__ __forceinline__ void store_spinor_f(const SpinorView& f, int r, int idx, const float v[24]) {
     char* p = const_cast<char*>(site_ptr<float>(f, r, idx));
 #pragma unroll
     for (int c = 0; c < 6; ++c)
-        *reinterpret_cast<float4*>(p + c * 512) = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
+        st_<CS>(reinterpret_cast<float4*>(p + c * 512), make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]));
 }
+template <> __device__ __forceinline__ void store_spinor<float, false>(const SpinorView& f, int r, int idx, int N5h, const float v[24]) { store_spinor_f<false>(f, r, idx, v); }
+template <> __device__ __forceinline__ void store_spinor<float, true>(const SpinorView& f, int r, int idx, int N5h, const float v[24]) { store_spinor_f<true>(f, r, idx, v); }
 // fp16: per-site max-norm scale (fp32) + IEEE half mantissas in [-1,1] ("16-bit storage, single-precision
 // computation"; format choice: SURVEY A11 / DESIGN.md reading R11)
-template <>
-__device__ __forceinline__ void store_spinor<__half>(const SpinorView& f, int r, int idx, int N5h,
-                                                     const float v[24]) {
+template <bool CS>
+__device__ __forceinline__ void store_spinor_h(const SpinorView& f, int r, int idx, const float v[24]) {
     float m = 0.f;
 #pragma unroll
     for (int i = 0; i < 24; ++i) m = fmaxf(m, fabsf(v[i]));
     const float inv = m > 0.f ? __fdividef(1.0f, m) : 0.f;
     char* p = const_cast<char*>(site_ptr<__half>(f, r, idx));
-    *reinterpret_cast<float*>(p - (idx & 31) * 12 + 3 * 512) = m;
+    st_<CS>(reinterpret_cast<float*>(p - (idx & 31) * 12 + 3 * 512), m);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         uint4 t;
@@ -205,9 +216,11 @@ __device__ __forceinline__ void store_spinor<__half>(const SpinorView& f, int r,
         t.y = f2h(v[8 * c + 2] * inv, v[8 * c + 3] * inv);
         t.z = f2h(v[8 * c + 4] * inv, v[8 * c + 5] * inv);
         t.w = f2h(v[8 * c + 6] * inv, v[8 * c + 7] * inv);
-        *reinterpret_cast<uint4*>(p + c * 512) = t;
+        st_<CS>(reinterpret_cast<uint4*>(p + c * 512), t);
     }
 }
+template <> __device__ __forceinline__ void store_spinor<__half, false>(const SpinorView& f, int r, int idx, int N5h, const float v[24]) { store_spinor_h<false>(f, r, idx, v); }
+template <> __device__ __forceinline__ void store_spinor<__half, true>(const SpinorView& f, int r, int idx, int N5h, const float v[24]) { store_spinor_h<true>(f, r, idx, v); }
 
 // ---------------------------------------------------------------------------------------------
 // Links.  NGV = vectors per link; U[18] = [row][col][re,im] after reconstruction.

@@ -164,6 +164,9 @@ __device__ __forceinline__ void block_sum_store(double v, unsigned char* smem_ra
 // link rows (broadcast) -- "staging of links reused across the Ls slices" (north_star).
 //   smem link row: 20 reals (16-byte aligned); site stride 8*20+4 reals (keeps 16-byte reads of the sites
 //   of one warp in different banks); index table: 12 ints per site (8 neighbours, own xh, pad).
+#ifndef MDWF_HOP_STCS
+#define MDWF_HOP_STCS true
+#endif
 #ifndef MDWF_HOP_MINB
 #define MDWF_HOP_MINB 3
 #endif
@@ -227,18 +230,21 @@ struct HopArgs {
     int rhs_list[64];
 };
 
-// 4D site index in the slab traversal -> coordinates
+// (tile, site-in-tile) -> coordinates; see Geom for the traversal order
 struct SiteCoord { int xh, xx, y, z, t, o; };
-__device__ __forceinline__ SiteCoord decode_site(const Geom& g, int par, uint32_t site) {
+__device__ __forceinline__ SiteCoord decode_site(const Geom& g, int par, uint32_t tile, uint32_t i) {
     SiteCoord c;
-    uint32_t zcI, rem, t, rem2, row, xx, zl, y;
-    g.dTslab.divmod(site, zcI, rem);
-    g.dSlab.divmod(rem, t, rem2);
-    g.dXH.divmod(rem2, row, xx);
-    g.dY.divmod(row, zl, y);
-    c.xx = xx; c.y = y; c.z = zcI * g.zc + zl; c.t = t;
+    uint32_t q, tT, tZ, tY, tX, ix, iy, iz, it, r;
+    g.dnTx.divmod(tile, q, tX);
+    g.dnTy.divmod(q, r, tY);
+    g.dnTzs.divmod(r, q, tZ);
+    g.dnTt.divmod(q, r, tT);            // r = slab index
+    g.dtxh.divmod(i, q, ix);
+    g.dty.divmod(q, it, iy);
+    g.dtz.divmod(it, it, iz);
+    c.xx = tX * g.txh + ix; c.y = tY * g.ty + iy; c.z = r * g.zc + tZ * g.tz + iz; c.t = tT * g.tt + it;
     c.o = (par + c.y + c.z + c.t) & 1;                 // x = 2*xx + o
-    c.xh = xx + g.XH * (c.y + g.Y * (c.z + g.Z * c.t));
+    c.xh = c.xx + g.XH * (c.y + g.Y * (c.z + g.Z * c.t));
     return c;
 }
 
@@ -248,21 +254,18 @@ __global__ void __launch_bounds__(256, (sizeof(typename Store<S>::real) == 8 ? 1
     typedef Pack16<T> P;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int Ls = g.Ls;
-    const int nsite = blockDim.x / Ls;
+    const int nsite = g.nsite;
     T* links = reinterpret_cast<T*>(smem_raw);
     int* tab = reinterpret_cast<int*>(smem_raw + (size_t)nsite * MDWF_LSITE * sizeof(T));
     unsigned char* smem_epi = smem_raw + smem_bytes_links<T>(nsite);
     const int slot = blockIdx.x % a.nact;
     const int tile = blockIdx.x / a.nact;
     const int rhs = a.rhs_list[slot];
-    const int site0 = tile * nsite;
     // ---- stage the block's links and neighbour table --------------------------------------------------
     for (int task = threadIdx.x; task < nsite * 8; task += blockDim.x) {
         const int i = task >> 3, l = task & 7, mu = l >> 1;
         const bool fwd = (l & 1) == 0;
-        const int jsite = site0 + i;
-        if (jsite >= g.Vh) continue;
-        const SiteCoord c = decode_site(g, a.par, (uint32_t)jsite);
+        const SiteCoord c = decode_site(g, a.par, (uint32_t)tile, (uint32_t)i);
         const int xh = c.xh;
         int n;
         bool wrap;
@@ -301,7 +304,7 @@ __global__ void __launch_bounds__(256, (sizeof(typename Store<S>::real) == 8 ? 1
     __syncthreads();
     // ---- the stencil: one thread per (site, s) -----------------------------------------------------------
     const int grp = (int)g.dLs.div(threadIdx.x), s = threadIdx.x - grp * Ls;
-    const bool live = grp < nsite && site0 + grp < g.Vh;
+    const bool live = grp < nsite;
     T acc[24];
 #pragma unroll
     for (int i = 0; i < 24; ++i) acc[i] = 0;
@@ -322,7 +325,7 @@ __global__ void __launch_bounds__(256, (sizeof(typename Store<S>::real) == 8 ? 1
         leg2<S, 3, false, DAG>(a.in, rhs, N5h, n1.w * Ls + s, Ub + 7 * MDWF_LROW, acc);
     }
     if (!FUSED) {
-        if (live) store_spinor<S>(a.out, rhs, idx, g.N5h, acc);
+        if (live) store_spinor<S, MDWF_HOP_STCS>(a.out, rhs, idx, g.N5h, acc);
         return;
     }
     // ---- fused epilogue: s-direction matrix, xpay, optional |out|^2 ---------------------------
@@ -340,7 +343,7 @@ __global__ void __launch_bounds__(256, (sizeof(typename Store<S>::real) == 8 ? 1
 #pragma unroll
         for (int i = 0; i < 24; ++i) acc[i] *= ch;
     }
-    if (live) store_spinor<S>(a.out, rhs, idx, g.N5h, acc);
+    if (live) store_spinor<S, MDWF_HOP_STCS>(a.out, rhs, idx, g.N5h, acc);
     if (a.partial != nullptr) {
         double s2 = 0.0;
         if (live) {

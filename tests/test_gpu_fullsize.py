@@ -1,0 +1,173 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
+
+The oracle cannot run whole 48^3x64x10 solves, so outputs are SAMPLED: (i) the hop acts on each s-slice
+independently, so two s-slices of a full-size field are compared with the oracle hop of those slices; (ii) D is a
+radius-one stencil, so a 4^4 core inside an 8^4 patch cut out of the big lattice (links + field copied onto a small
+periodic lattice) reproduces (D psi)(x) on the core exactly -- the oracle evaluates the residual b - D x there; (iii)
+the global residual is evaluated by the library's fp64 FULL operator, itself checked against the oracle in
+test_gpu_dslash.py and on the patches here."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+
+pytestmark = pytest.mark.gpu
+
+
+def rel(a, b):
+    a = np.asarray(a).reshape(-1)
+    b = np.asarray(b).reshape(-1)
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+def site_index(dims, x, y, z, t):
+    return x + dims[0] * (y + dims[1] * (z + dims[2] * t))
+
+
+def patch_indices(dims, origin, P=8):
+    ax = [np.arange(origin[m], origin[m] + P) for m in range(4)]
+    assert all(a.max() < dims[m] - 1 and a.min() >= 1 for m, a in enumerate(ax))   # away from the bc boundaries
+    T, Z, Y, X = np.meshgrid(ax[3], ax[2], ax[1], ax[0], indexing="ij")
+    return site_index(dims, X, Y, Z, T).reshape(-1)        # patch x4 order (x fastest) -> big-lattice x4
+
+
+def patch_residual(cfg, p_big, U, x, b, origin, P=8):
+    """oracle residual (b - D x) on the 4^4 core of a P^4 patch; returns (|r|_core, |b|_core) per rhs"""
+    idx = torch.from_numpy(patch_indices(cfg.dims, origin, P)).to(U.device)
+    pp = oracle.Params(dims=(P,) * 4, Ls=cfg.Ls, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=cfg.mf, bc=(1, 1, 1, 1))
+    Up = U[:, idx].cpu().numpy()
+    xp = x[:, :, idx].cpu().numpy()
+    bp = b[:, :, idx].cpu().numpy()
+    r = (bp - oracle.D(pp, Up, xp)).reshape(x.shape[0], cfg.Ls, P, P, P, P, 12)
+    bb = bp.reshape(x.shape[0], cfg.Ls, P, P, P, P, 12)
+    c = slice(2, P - 2)
+    rn = np.sqrt((np.abs(r[:, :, c, c, c, c]) ** 2).reshape(x.shape[0], -1).sum(1))
+    bn = np.sqrt((np.abs(bb[:, :, c, c, c, c]) ** 2).reshape(x.shape[0], -1).sum(1))
+    return rn, bn
+
+
+@pytest.fixture(scope="module")
+def c5():
+    import paper_1810_01609_b200 as mdwf
+    cfg = synth.CONFIGS[5]
+    ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
+    U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(5, 1), device="cuda")
+    for prec, recon in [(64, 18), (32, 12), (16, 12)]:
+        ctx.mdwf_load_gauge(U, prec, recon)
+    return mdwf, cfg, ctx, U
+
+
+def test_c5_hop_two_slices_vs_oracle(c5):
+    """48^3x64, Ls=10: packed hop in fp64/fp32/fp16 storage; slices s = 0 and 7 against the oracle."""
+    mdwf, cfg, ctx, U = c5
+    Vh = cfg.V4 // 2
+    g = torch.Generator(device="cuda").manual_seed(5002)
+    src = torch.empty((1, cfg.Ls, Vh, 4, 3), dtype=torch.complex128, device="cuda")
+    torch.view_as_real(src).normal_(0.0, 1.0, generator=g)
+    p2 = oracle.Params(dims=cfg.dims, Ls=2, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=cfg.mf, bc=cfg.bc)
+    sl = [0, 7]
+    full = oracle.from_half(src[0, sl].cpu().numpy(), cfg.dims, 1)             # input lives on parity 1
+    exp = oracle.to_half(oracle.hop(p2, U.cpu().numpy(), full, out_parity=0), cfg.dims, 0)
+    for prec, recon, tol in [(64, 18, 1e-12), (32, 12, 1e-5), (16, 12, 2e-3)]:
+        out = ctx.mdwf_dslash(mdwf.OP_HOP, src, parity=0, prec=prec, recon=recon)
+        assert rel(out[0, sl].cpu().numpy(), exp) <= tol, (prec, recon)
+        del out
+
+
+def test_c5_solve_sampled_residual(c5):
+    """config 5 as bench.py runs it (16-bit inner, 12-real links, tol 1e-10; bench.py's automatic batching also
+    solves one rhs at a time at this size), 1 of the 4 rhs to bound time and memory."""
+    mdwf, cfg, ctx, U = c5
+    torch.cuda.empty_cache()
+    b = synth.gaussian_spinor_device(cfg.dims, cfg.Ls, 1, synth.seed_for(5, 2), device="cuda")
+    x, res = ctx.mdwf_solve(b, tol=cfg.tol, inner_prec=16, recon=12, symmetric=True)
+    assert res.status == mdwf.OK, res
+    # (iii) global true residual with the library's fp64 full operator
+    Dx = ctx.mdwf_dslash(mdwf.OP_FULL, x, prec=64, recon=18)
+    for r in range(1):
+        tr = float(torch.linalg.vector_norm(b[r] - Dx[r]) / torch.linalg.vector_norm(b[r]))
+        assert tr <= cfg.tol, (r, tr)
+        assert abs(tr - res.true_resid[r]) <= 0.05 * tr + 1e-14
+    # (ii) the oracle's D on patches: the fp64 FULL operator agrees with it, and the residual is small there
+    p_big = None
+    for origin in [(2, 4, 6, 8), (30, 20, 10, 40)]:
+        idx = torch.from_numpy(patch_indices(cfg.dims, origin)).cuda()
+        pp = oracle.Params(dims=(8,) * 4, Ls=cfg.Ls, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=cfg.mf, bc=(1, 1, 1, 1))
+        Do = oracle.D(pp, U[:, idx].cpu().numpy(), x[:, :, idx].cpu().numpy()).reshape(1, cfg.Ls, 8, 8, 8, 8, 12)
+        Dg = Dx[:, :, idx].cpu().numpy().reshape(1, cfg.Ls, 8, 8, 8, 8, 12)
+        c = slice(2, 6)
+        assert rel(Dg[:, :, c, c, c, c], Do[:, :, c, c, c, c]) <= 1e-12
+        rn, bn = patch_residual(cfg, p_big, U, x, b, origin)
+        assert (rn / bn <= 20 * cfg.tol).all(), (origin, rn / bn)
+
+
+def test_c3_point_source_propagator_full_size():
+    """config 3: 24^3x64, Ls=8, 12 point sources, 16-bit inner CG to 1e-8, 4D in / 4D out (batched multi-rhs)."""
+    import paper_1810_01609_b200 as mdwf
+    cfg = synth.CONFIGS[3]
+    ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
+    U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(3, 1), device="cuda")
+    ctx.mdwf_load_gauge(U, 64, 18)
+    ctx.mdwf_load_gauge(U, 16, 12)
+    eta = synth.point_sources_4d(cfg.dims).cuda()
+    x5, res = ctx.mdwf_solve(eta, tol=cfg.tol, inner_prec=16, recon=12, src_kind=1, out_kind=0)
+    assert res.status == mdwf.OK, res
+    b5 = ctx.mdwf_wall_inject(eta)
+    Dx = ctx.mdwf_dslash(mdwf.OP_FULL, x5, prec=64, recon=18)
+    for r in range(12):
+        assert float(torch.linalg.vector_norm(b5[r] - Dx[r]) / torch.linalg.vector_norm(b5[r])) <= cfg.tol
+    # oracle check of D on a patch around the source-free region and of the 4D projection rule on it
+    origin = (4, 6, 8, 10)
+    idx = torch.from_numpy(patch_indices(cfg.dims, origin)).cuda()
+    pp = oracle.Params(dims=(8,) * 4, Ls=cfg.Ls, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=cfg.mf, bc=(1, 1, 1, 1))
+    cols = [0, 5, 11]
+    Do = oracle.D(pp, U[:, idx].cpu().numpy(), x5[cols][:, :, idx].cpu().numpy()).reshape(3, cfg.Ls, 8, 8, 8, 8, 12)
+    Dg = Dx[cols][:, :, idx].cpu().numpy().reshape(3, cfg.Ls, 8, 8, 8, 8, 12)
+    c = slice(2, 6)
+    assert rel(Dg[:, :, c, c, c, c], Do[:, :, c, c, c, c]) <= 1e-12
+    q = ctx.mdwf_wall_project(x5)
+    qo = oracle.wall_project(pp, x5[cols][:, :, idx].cpu().numpy())
+    assert np.array_equal(q[cols][:, idx].cpu().numpy(), qo)
+
+
+def test_c4_fh_chain_full_size():
+    """config 4: 32^3x48, Ls=12: smeared 12-column source -> S ; gamma_z gamma_5 S on all t ; S_FH ; C(t) with and
+    without the insertion.  Solves are checked through the fp64 residual of the 5D systems (sampled columns), the
+    sequential source and one timeslice of each contraction against the oracle's literal sums."""
+    import paper_1810_01609_b200 as mdwf
+    cfg = synth.CONFIGS[4]
+    ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
+    U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(4, 1), device="cuda")
+    ctx.mdwf_load_gauge(U, 64, 18)
+    ctx.mdwf_load_gauge(U, 16, 12)
+    eta = synth.gaussian_smeared_sources_4d(cfg.dims, width=3.0).cuda()
+    kw = dict(tol=cfg.tol, inner_prec=16, recon=12, src_kind=1, out_kind=1)
+    S, r1 = ctx.mdwf_solve(eta, **kw)
+    G = oracle.gamma(2) @ oracle.gamma(4)
+    seq = ctx.mdwf_seq_source(S, G)
+    SFH, r2 = ctx.mdwf_solve(seq, **kw)
+    assert r1.status == mdwf.OK and r2.status == mdwf.OK, (r1, r2)
+    assert max(r1.true_resid) <= cfg.tol and max(r2.true_resid) <= cfg.tol
+    # sequential source: exact signed permutation of the input, all columns
+    Sn = S[:2].cpu().numpy()
+    assert rel(seq[:2].cpu().numpy(), oracle.seq_source(cfg.dims, Sn, G)) <= 1e-15
+    # 5D residual of two columns of the second solve, by the fp64 FULL operator
+    x5, r3 = ctx.mdwf_solve(seq[3:5].contiguous(), tol=cfg.tol, inner_prec=16, recon=12, src_kind=1, out_kind=0)
+    b5 = ctx.mdwf_wall_inject(seq[3:5].contiguous())
+    Dx = ctx.mdwf_dslash(mdwf.OP_FULL, x5, prec=64, recon=18)
+    for r in range(2):
+        assert float(torch.linalg.vector_norm(b5[r] - Dx[r]) / torch.linalg.vector_norm(b5[r])) <= cfg.tol
+    assert rel(ctx.mdwf_wall_project(x5).cpu().numpy(), SFH[3:5].cpu().numpy()) <= 1e-6
+    # contractions: one timeslice by the oracle's literal loops
+    P = 0.5 * (np.eye(4) + oracle.gamma(3))
+    c0 = ctx.mdwf_nucleon_2pt(S, S, S, P).cpu().numpy()
+    cfh = (ctx.mdwf_nucleon_2pt(SFH, S, S, P) + ctx.mdwf_nucleon_2pt(S, S, SFH, P) - ctx.mdwf_nucleon_2pt(S, SFH, S, P)).cpu().numpy()
+    t = 5
+    Sh, Fh = S.cpu().numpy(), SFH.cpu().numpy()
+    o0 = oracle.nucleon_2pt(cfg.dims, Sh, Sh, Sh, P, t_lo=t, t_hi=t)[t]
+    ofh = (oracle.nucleon_2pt(cfg.dims, Fh, Sh, Sh, P, t_lo=t, t_hi=t)[t] + oracle.nucleon_2pt(cfg.dims, Sh, Sh, Fh, P, t_lo=t, t_hi=t)[t]
+           - oracle.nucleon_2pt(cfg.dims, Sh, Fh, Sh, P, t_lo=t, t_hi=t)[t])
+    assert abs(c0[t] - o0) <= 1e-11 * abs(o0) and abs(cfh[t] - ofh) <= 1e-11 * abs(ofh)
+    assert np.isfinite(c0).all() and np.isfinite(cfh).all()
