@@ -60,6 +60,47 @@ static void build_matrices(int Ls, double M5, double b5, double c5, double mf, s
     }
 }
 
+// The structured form of the same operators that the kernels apply (LsOp, mdwf_hop.cuh).
+static void build_lsops(int Ls, double M5, double b5, double c5, double mf, LsOp ops[MAT_COUNT]) {
+    const double a = b5 * (4.0 - M5) + 1.0, d = c5 * (4.0 - M5) - 1.0, kappa = -d / a;
+    LsOp base;
+    base.kind = 1; base.dag = 0; base.c0 = 0; base.c1 = 0;
+    base.kappa = kappa; base.inv_a = 1.0 / a; base.mf = mf;
+    base.gfac = mf / (a * (1.0 + mf * std::pow(kappa, Ls)));
+    for (int dag = 0; dag < 2; ++dag) {
+        LsOp o = base;
+        o.dag = dag;
+        o.kind = 1; o.c0 = b5; o.c1 = c5; ops[MAT_A + 4 * dag] = o;
+        o.kind = 1; o.c0 = a; o.c1 = d; ops[MAT_M5 + 4 * dag] = o;
+        o.kind = 2; o.c0 = 0.0; o.c1 = 1.0; ops[MAT_M5INV + 4 * dag] = o;
+        if (d != 0.0) { o.kind = 2; o.c0 = c5 / d; o.c1 = b5 - c5 * a / d; }     // (b5 + c5 L)/(a + d L)
+        else { o.kind = 1; o.c0 = b5 / a; o.c1 = c5 / a; }
+        ops[MAT_AM5INV + 4 * dag] = o;
+    }
+}
+// host emulation of apply_ls on one chirality column (for the self-test): out = op(v), v[s], chi 0 = P+
+static void lsop_host(const LsOp& op, int Ls, int chi, const std::vector<double>& v, std::vector<double>& out) {
+    out.assign(Ls, 0.0);
+    if (op.kind == 1) {
+        for (int s = 0; s < Ls; ++s) {
+            const int sm = s == 0 ? Ls - 1 : s - 1, sp = s == Ls - 1 ? 0 : s + 1;
+            const double fm = s == 0 ? -op.mf : 1.0, fp = s == Ls - 1 ? -op.mf : 1.0;
+            const bool take_minus = (chi == 0) != (op.dag != 0);      // P+ takes s-1 (L), s+1 (L^dag)
+            out[s] = op.c0 * v[s] + op.c1 * (take_minus ? fm * v[sm] : fp * v[sp]);
+        }
+        return;
+    }
+    const bool fwd = (chi == 0) != (op.dag != 0);
+    std::vector<double> P(Ls);
+    double run = 0.0;
+    for (int k = 0; k < Ls; ++k) { const int s = fwd ? k : Ls - 1 - k; run = v[s] + op.kappa * run; P[s] = run; }
+    const double T = P[fwd ? Ls - 1 : 0];
+    for (int s = 0; s < Ls; ++s) {
+        const int k = fwd ? s : Ls - 1 - s;
+        out[s] = op.c0 * v[s] + op.c1 * (op.inv_a * P[s] - op.gfac * std::pow(op.kappa, k + 1) * T);
+    }
+}
+
 // z-slab depth: largest multiple of the tile depth tz dividing Z whose fp32 input slab XH*Y*zc*Ls*96 bytes stays
 // under ~9 MB, so that the three t-consecutive slabs a row of tiles touches (plus the streamed output) live in
 // L2 (measured on B200: 48^3x64 Ls=10 is fastest at zc = 8)
@@ -128,7 +169,6 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     c->M5 = M5; c->b5 = b5; c->c5 = c5; c->mf = mf;
     c->partial = nullptr; c->dscal = nullptr; c->hscal = nullptr; c->launches = 0; c->prof_on = 0;
     for (int i = 0; i < 3; ++i) { c->prof_ms[i] = c->prof_bytes[i] = c->prof_flops[i] = 0.0; c->prof_n[i] = 0; }
-    for (int i = 0; i < MAT_COUNT; ++i) c->mat_d[i] = c->mat_f[i] = nullptr;
     *out = c;   // returned even on failure so that mdwf_last_error can be read; caller destroys it
     long long v4 = 1;
     for (int m = 0; m < 4; ++m) {
@@ -163,17 +203,7 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     MDWF_CUDA(c, cudaMalloc(&c->dscal, sizeof(double) * 8 * 64));
     MDWF_CUDA(c, cudaMemset(c->dscal, 0, sizeof(double) * 8 * 64));
     MDWF_CUDA(c, cudaHostAlloc(&c->hscal, sizeof(double) * 8 * 64, cudaHostAllocDefault));
-    std::vector<double> mats[MAT_COUNT];
-    build_matrices(g.Ls, M5, b5, c5, mf, mats);
-    for (int i = 0; i < MAT_COUNT; ++i) {
-        const size_t n = mats[i].size();
-        std::vector<float> mf32(n);
-        for (size_t k = 0; k < n; ++k) mf32[k] = (float)mats[i][k];
-        MDWF_CUDA(c, cudaMalloc(&c->mat_d[i], n * sizeof(double)));
-        MDWF_CUDA(c, cudaMalloc(&c->mat_f[i], n * sizeof(float)));
-        MDWF_CUDA(c, cudaMemcpy(c->mat_d[i], mats[i].data(), n * sizeof(double), cudaMemcpyHostToDevice));
-        MDWF_CUDA(c, cudaMemcpy(c->mat_f[i], mf32.data(), n * sizeof(float), cudaMemcpyHostToDevice));
-    }
+    build_lsops(g.Ls, M5, b5, c5, mf, c->lsop);
     return MDWF_OK;
 }
 
@@ -181,7 +211,6 @@ int mdwf_destroy(mdwf_ctx* c) {
     if (!c) return MDWF_OK;
     for (size_t i = 0; i < c->gauges.size(); ++i) { cudaFree(c->gauges[i].v[0]); cudaFree(c->gauges[i].v[1]); }
     for (auto& kv : c->temps) for (mdwf_field* f : kv.second) free_field(f);
-    for (int i = 0; i < MAT_COUNT; ++i) { if (c->mat_d[i]) cudaFree(c->mat_d[i]); if (c->mat_f[i]) cudaFree(c->mat_f[i]); }
     prof_drain(c);
     for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
     if (c->partial) cudaFree(c->partial);
@@ -237,6 +266,18 @@ int mdwf_selftest_host(double M5, double b5, double c5, double mf) {
                     for (int id = 0; id < 4; ++id)
                         if (m[id + 4][ch * n + t * Ls + s] != m[id][ch * n + s * Ls + t]) return 3;
                 }
+        // 4: the structured operators the kernels apply reproduce the dense blocks column by column
+        LsOp ops[MAT_COUNT];
+        build_lsops(Ls, M5, b5, c5, mf, ops);
+        for (int id = 0; id < MAT_COUNT; ++id)
+            for (int ch = 0; ch < 2; ++ch)
+                for (int t = 0; t < Ls; ++t) {
+                    std::vector<double> e(Ls, 0.0), o;
+                    e[t] = 1.0;
+                    lsop_host(ops[id], Ls, ch, e, o);
+                    for (int s = 0; s < Ls; ++s)
+                        if (std::fabs(o[s] - m[id][ch * n + t * Ls + s]) > 1e-12) return 4;
+                }
     }
     return 0;
 }
@@ -276,7 +317,7 @@ int op_ls(const OpCtx& o, const SpinorView& out, const SpinorView& in, int mat, 
     LsArgs a;
     a.out = out; a.in = in;
     if (xin) a.xin = *xin; else { a.xin.v = nullptr; a.xin.n = nullptr; a.xin.rs = a.xin.rn = 0; }
-    a.G = mat >= 0 ? o.c->mat(mat, o.prec) : nullptr;
+    if (mat >= 0) a.op = o.c->lsop[mat]; else a.op.kind = 0;
     a.cx = cx; a.ch = ch; a.partial = partial; a.write = write; a.rl = rl;
     return launch_ls(o.c, o.prec, a, o.st);
 }
@@ -287,7 +328,7 @@ int op_hop(const OpCtx& o, const SpinorView& out, const SpinorView& in, int out_
     a.out = out; a.in = in;
     if (xin) a.xin = *xin; else { a.xin.v = nullptr; a.xin.n = nullptr; a.xin.rs = a.xin.rn = 0; }
     a.g.v[0] = o.gs->v[0]; a.g.v[1] = o.gs->v[1];
-    a.G = mat >= 0 ? o.c->mat(mat, o.prec) : nullptr;
+    if (mat >= 0) a.op = o.c->lsop[mat]; else a.op.kind = 0;
     a.cx = cx; a.ch = ch; a.partial = partial; a.par = out_par; a.nact = rl.nact;
     for (int i = 0; i < 64; ++i) a.rhs_list[i] = rl.rhs[i];
     const int fused = (mat >= 0 || xin || partial || ch != 1.0) ? 1 : 0;

@@ -78,9 +78,9 @@ template <typename S> static size_t g_smem(mdwf_ctx* c, bool useG) {
 int launch_ls(mdwf_ctx* c, int prec, LsArgs& a, cudaStream_t st) {
     const int grid = c->nblk * a.rl.nact;
     switch (prec) {
-        case 64: return launch_big_smem(c, ls_kernel<double>, grid, g_smem<double>(c, a.G != nullptr), st, a);
-        case 32: return launch_big_smem(c, ls_kernel<float>, grid, g_smem<float>(c, a.G != nullptr), st, a);
-        case 16: return launch_big_smem(c, ls_kernel<__half>, grid, g_smem<__half>(c, a.G != nullptr), st, a);
+        case 64: return launch_big_smem(c, ls_kernel<double>, grid, g_smem<double>(c, a.op.kind != 0), st, a);
+        case 32: return launch_big_smem(c, ls_kernel<float>, grid, g_smem<float>(c, a.op.kind != 0), st, a);
+        case 16: return launch_big_smem(c, ls_kernel<__half>, grid, g_smem<__half>(c, a.op.kind != 0), st, a);
     }
     MDWF_FAIL(c, MDWF_EINVAL, "bad precision %d", prec);
 }
@@ -156,9 +156,9 @@ int launch_cg_xr(mdwf_ctx* c, int prec_x, int prec, CgXrArgs& a, cudaStream_t st
 int launch_cg_p(mdwf_ctx* c, int prec, CgPArgs& a, cudaStream_t st) {
     const int grid = c->nblk * a.rl.nact;
     switch (prec) {
-        case 64: return launch_big_smem(c, cg_update_p_kernel<double>, grid, g_smem<double>(c, a.G != nullptr), st, a);
-        case 32: return launch_big_smem(c, cg_update_p_kernel<float>, grid, g_smem<float>(c, a.G != nullptr), st, a);
-        case 16: return launch_big_smem(c, cg_update_p_kernel<__half>, grid, g_smem<__half>(c, a.G != nullptr), st, a);
+        case 64: return launch_big_smem(c, cg_update_p_kernel<double>, grid, g_smem<double>(c, a.op.kind != 0), st, a);
+        case 32: return launch_big_smem(c, cg_update_p_kernel<float>, grid, g_smem<float>(c, a.op.kind != 0), st, a);
+        case 16: return launch_big_smem(c, cg_update_p_kernel<__half>, grid, g_smem<__half>(c, a.op.kind != 0), st, a);
     }
     MDWF_FAIL(c, MDWF_EINVAL, "bad precision %d", prec);
 }

@@ -16,7 +16,7 @@ struct RhsList {
 // out = cx*xin + ch * G in   (G == nullptr: identity), optional sum |out|^2, optional no store
 struct LsArgs {
     SpinorView out, in, xin;
-    const void* G;
+    LsOp op;
     double cx, ch;
     double* partial;
     int write;
@@ -35,7 +35,7 @@ __global__ void __launch_bounds__(256) ls_kernel(const Geom g, const LsArgs a) {
 #pragma unroll
         for (int i = 0; i < 24; ++i) acc[i] = 0;
     }
-    if (a.G != nullptr) apply_G<T>(acc, a.G, g.Ls, smem_raw);
+    if (a.op.kind != 0) apply_ls<T>(acc, a.op, g.Ls, smem_raw);
     const T ch = (T)a.ch, cx = (T)a.cx;
     if (a.xin.v != nullptr && live) {
         T xv[24];
@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(256) cg_update_xr_kernel(const Geom g, const C
 // the leading s-direction factor of the next operator application, fused to save one pass)
 struct CgPArgs {
     SpinorView p, r, q;
-    const void* G;
+    LsOp op;
     const double* rr_new;
     const double* rr_old;
     RhsList rl;
@@ -168,8 +168,8 @@ __global__ void __launch_bounds__(256) cg_update_p_kernel(const Geom g, const Cg
         for (int i = 0; i < 24; ++i) pv[i] = rv[i] + beta * pv[i];
         store_spinor<S>(a.p, rhs, idx, g.N5h, pv);
     }
-    if (a.G != nullptr) {
-        apply_G<T>(pv, a.G, g.Ls, smem_raw);
+    if (a.op.kind != 0) {
+        apply_ls<T>(pv, a.op, g.Ls, smem_raw);
         if (live) store_spinor<S>(a.q, rhs, idx, g.N5h, pv);
     }
 }

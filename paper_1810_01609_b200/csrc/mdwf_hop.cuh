@@ -101,24 +101,34 @@ template <typename T> struct alignas(16) Pack16 {
     T d[N];
 };
 
-// acc(s) <- sum_{s'} G_chi[s][s'] acc(s') over the Ls threads of one (site, rhs) group, through shared
-// memory.  G: device Gt[chi][s'][s] (chi = 0: spins 0,1 = P+, chi = 1: spins 2,3 = P-).  Every thread of
-// the block must call it (block-wide barriers); blockDim.x is a multiple of Ls.
-// smem needed: smem_bytes_G<T>(Ls, nthreads).
+// s-direction operator of a fused epilogue / site-local kernel (SURVEY 8 Notation):
+//   kind 1:  out = c0 v + c1 L v      (A = b5 + c5 L, M5 = a + d L;  dag: L -> L^dag)
+//   kind 2:  out = c0 v + c1 M5^-1 v  (M5^-1, and A M5^-1 = c5/d + (b5 - c5 a/d) M5^-1;  dag: M5^-dag)
+// with (L v)_s = P- v_{s+1} + P+ v_{s-1}, wraps multiplied by -mf, and M5^-1 through its closed form as a
+// first-order recurrence: for the "forward" chirality  P_s = v_s + kappa P_{s-1},  T = P_{Ls-1},
+//   (M5^-1 v)_s = P_s / a - gfac kappa^{s+1} T,   gfac = mf / (a (1 + mf kappa^Ls)),  kappa = -d/a,
+// and mirrored in s for the other chirality (P+ is forward for M5^-1, P- for M5^-dag).  O(Ls) work per site
+// instead of the O(Ls^2) of a dense Ls x Ls multiply.
+struct LsOp {
+    int kind, dag;
+    double c0, c1, kappa, inv_a, gfac, mf;
+};
+// shared memory: Ls reals (kappa powers) rounded up, then one 28-real row per thread (+4 per site group)
 template <typename T> __host__ __device__ inline int smem_reals_G(int Ls, int nthreads) {
-    return ((2 * Ls * Ls + 3) & ~3) + (nthreads / Ls) * (Ls * 28 + 4);
+    return ((Ls + 3) & ~3) + (nthreads / Ls) * (Ls * 28 + 4);
 }
+// Every thread of the block must call it (block-wide barriers); blockDim.x is a multiple of Ls; the Ls threads of
+// a (site, rhs) group are consecutive.
 template <typename T>
-__device__ __forceinline__ void apply_G(T acc[24], const void* G, int Ls, unsigned char* smem_raw) {
-    T* Gs = reinterpret_cast<T*>(smem_raw);
-    const int gsz = (2 * Ls * Ls + 3) & ~3;
-    T* buf = Gs + gsz;
-    for (int i = threadIdx.x; i < 2 * Ls * Ls; i += blockDim.x) Gs[i] = reinterpret_cast<const T*>(G)[i];
-    const int grp = threadIdx.x / Ls, sl = threadIdx.x - grp * Ls;
-    const int gstride = Ls * 28 + 4;   // 28-real rows (+4 per group): conflict-free 16-byte accesses
+__device__ __forceinline__ void apply_ls(T acc[24], const LsOp& op, int Ls, unsigned char* smem_raw) {
     typedef Pack16<T> P;
     constexpr int NP = 24 / P::N;
-    P* mine = reinterpret_cast<P*>(buf + grp * gstride + sl * 28);
+    T* kp = reinterpret_cast<T*>(smem_raw);
+    T* buf = kp + ((Ls + 3) & ~3);
+    const int grp = threadIdx.x / Ls, sl = threadIdx.x - grp * Ls;
+    const int gstride = Ls * 28 + 4;   // 28-real rows (+4 per group): conflict-free 16-byte accesses
+    T* grow = buf + grp * gstride;
+    P* mine = reinterpret_cast<P*>(grow + sl * 28);
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
         P t;
@@ -126,18 +136,51 @@ __device__ __forceinline__ void apply_G(T acc[24], const void* G, int Ls, unsign
         for (int e = 0; e < P::N; ++e) t.d[e] = acc[q * P::N + e];
         mine[q] = t;
     }
+    if (op.kind == 2 && (int)threadIdx.x < Ls) {
+        T v = (T)op.kappa;
+        for (int i = 0; i < (int)threadIdx.x; ++i) v *= (T)op.kappa;
+        kp[threadIdx.x] = v;            // kappa^{k+1}
+    }
     __syncthreads();
-#pragma unroll
-    for (int i = 0; i < 24; ++i) acc[i] = 0;
-    const T* grow = buf + grp * gstride;
-    for (int sp = 0; sp < Ls; ++sp) {
-        const T gp = Gs[sp * Ls + sl], gm = Gs[Ls * Ls + sp * Ls + sl];
-        const P* src = reinterpret_cast<const P*>(grow + sp * 28);
+    const T c0 = (T)op.c0, c1 = (T)op.c1;
+    if (op.kind == 1) {
+        const int sm = sl == 0 ? Ls - 1 : sl - 1, sp = sl == Ls - 1 ? 0 : sl + 1;
+        const T fm = c1 * (sl == 0 ? (T)(-op.mf) : (T)1), fp = c1 * (sl == Ls - 1 ? (T)(-op.mf) : (T)1);
+        const P* up = reinterpret_cast<const P*>(grow + (op.dag ? sp : sm) * 28);   // source row of the P+ components
+        const P* lo = reinterpret_cast<const P*>(grow + (op.dag ? sm : sp) * 28);   // source row of the P- components
+        const T fu = op.dag ? fp : fm, fl = op.dag ? fm : fp;
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
-            const P t = src[q];
+            const bool plus = q * P::N < 12;
+            const P t = plus ? up[q] : lo[q];
 #pragma unroll
-            for (int e = 0; e < P::N; ++e) acc[q * P::N + e] += (q * P::N + e < 12 ? gp : gm) * t.d[e];
+            for (int e = 0; e < P::N; ++e) acc[q * P::N + e] = c0 * acc[q * P::N + e] + (plus ? fu : fl) * t.d[e];
+        }
+    } else {
+        const T kap = (T)op.kappa;
+        for (int col = sl; col < NP; col += Ls) {
+            const bool fwd = (col * P::N < 12) != (op.dag != 0);
+            P run;
+#pragma unroll
+            for (int e = 0; e < P::N; ++e) run.d[e] = 0;
+            for (int k = 0; k < Ls; ++k) {
+                P* row = reinterpret_cast<P*>(grow + (fwd ? k : Ls - 1 - k) * 28) + col;
+                const P v = *row;
+#pragma unroll
+                for (int e = 0; e < P::N; ++e) run.d[e] = v.d[e] + kap * run.d[e];
+                *row = run;
+            }
+        }
+        __syncthreads();
+        const T ia = c1 * (T)op.inv_a;
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            const bool fwd = (q * P::N < 12) != (op.dag != 0);
+            const P ps = mine[q];
+            const P tt = reinterpret_cast<const P*>(grow + (fwd ? Ls - 1 : 0) * 28)[q];
+            const T gk = -c1 * (T)op.gfac * kp[fwd ? sl : Ls - 1 - sl];
+#pragma unroll
+            for (int e = 0; e < P::N; ++e) acc[q * P::N + e] = c0 * acc[q * P::N + e] + ia * ps.d[e] + gk * tt.d[e];
         }
     }
     __syncthreads();
@@ -222,7 +265,7 @@ __device__ __forceinline__ void leg2(const SpinorView& in, int rhs, int N5h, int
 struct HopArgs {
     SpinorView out, in, xin;   // xin.v == nullptr -> no xpay term
     GaugeView g;
-    const void* G;             // device: 2*Ls*Ls reals of the compute type, Gt[chi][s'][s]; nullptr -> identity
+    LsOp op;                   // s-direction factor applied to H(in); kind 0 -> none
     double cx, ch;
     double* partial;           // nullptr or [nact][nblk_per_rhs] per-block sum |out|^2 (fixed order)
     int par;                   // parity of the output sites
@@ -329,7 +372,7 @@ __global__ void __launch_bounds__(256, (sizeof(typename Store<S>::real) == 8 ? 1
         return;
     }
     // ---- fused epilogue: s-direction matrix, xpay, optional |out|^2 ---------------------------
-    if (a.G != nullptr) apply_G<T>(acc, a.G, g.Ls, smem_epi);
+    if (a.op.kind != 0) apply_ls<T>(acc, a.op, g.Ls, smem_epi);
     const T ch = (T)a.ch;
     if (a.xin.v != nullptr) {
         if (live) {
@@ -345,11 +388,13 @@ __global__ void __launch_bounds__(256, (sizeof(typename Store<S>::real) == 8 ? 1
     }
     if (live) store_spinor<S, MDWF_HOP_STCS>(a.out, rhs, idx, g.N5h, acc);
     if (a.partial != nullptr) {
-        double s2 = 0.0;
+        // the 24 squares of one site are summed in the compute type, everything above in fp64
+        T s24 = 0;
         if (live) {
 #pragma unroll
-            for (int i = 0; i < 24; ++i) s2 += (double)acc[i] * (double)acc[i];
+            for (int i = 0; i < 24; ++i) s24 = fma_<T>(acc[i], acc[i], s24);
         }
+        const double s2 = (double)s24;
         block_sum_store(s2, smem_epi, a.partial + (long long)slot * (gridDim.x / a.nact) + tile);
     }
 }

@@ -27,7 +27,7 @@ static int launch_hop_SR(mdwf_ctx* c, int dagger, int fused, HopArgs& a, cudaStr
     size_t smem = 0;
     if (fused) {
         smem = (size_t)c->block * sizeof(double);
-        if (a.G) smem = std::max(smem, (size_t)smem_reals_G<T>(c->g.Ls, c->block) * sizeof(T));
+        if (a.op.kind) smem = std::max(smem, (size_t)smem_reals_G<T>(c->g.Ls, c->block) * sizeof(T));
     }
     smem += smem_bytes_links<T>(c->block / c->g.Ls);
     if (fused) {

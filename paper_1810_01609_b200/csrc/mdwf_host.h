@@ -32,8 +32,7 @@ struct mdwf_ctx {
     int block;                 // threads per block: a multiple of Ls, <= 256
     int nblk;                  // blocks per rhs = ceil(N5h / block)
     std::vector<GaugeSet> gauges;
-    void* mat_d[MAT_COUNT];
-    void* mat_f[MAT_COUNT];
+    mdwf::LsOp lsop[MAT_COUNT];
     double* partial;           // [64][nblk] per-block partial sums
     double* dscal;             // device scalars [8][64]
     double* hscal;             // pinned host mirror [8][64]
@@ -54,7 +53,6 @@ struct mdwf_ctx {
             if (gauges[i].prec == prec && gauges[i].recon == recon) return &gauges[i];
         return nullptr;
     }
-    const void* mat(int id, int prec) const { return prec == 64 ? mat_d[id] : mat_f[id]; }
 };
 
 #define MDWF_FAIL(ctx, code, ...)                          \

@@ -226,7 +226,7 @@ static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_o
             if (act.nact == 0) break;
         }
         CgPArgs q;
-        q.p = p; q.r = r; q.q = none; q.G = nullptr; q.rr_new = S.dsc(rrNew); q.rr_old = S.dsc(rrOld); q.rl = act;
+        q.p = p; q.r = r; q.q = none; q.op.kind = 0; q.rr_new = S.dsc(rrNew); q.rr_old = S.dsc(rrOld); q.rl = act;
         if ((rc = launch_cg_p(c, S.prec, q, st))) break;
         std::swap(rrOld, rrNew);
     }
