@@ -209,7 +209,7 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
 
 int mdwf_destroy(mdwf_ctx* c) {
     if (!c) return MDWF_OK;
-    for (size_t i = 0; i < c->gauges.size(); ++i) { cudaFree(c->gauges[i].v[0]); cudaFree(c->gauges[i].v[1]); }
+    for (size_t i = 0; i < c->gauges.size(); ++i) free_gauge(&c->gauges[i]);
     for (auto& kv : c->temps) for (mdwf_field* f : kv.second) free_field(f);
     prof_drain(c);
     for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
@@ -298,8 +298,7 @@ int mdwf_load_gauge(mdwf_ctx* c, const void* U, int store_prec, int recon, void*
     if (rc) return rc;
     for (size_t i = 0; i < c->gauges.size(); ++i)
         if (c->gauges[i].prec == store_prec && c->gauges[i].recon == recon) {
-            cudaFree(c->gauges[i].v[0]);
-            cudaFree(c->gauges[i].v[1]);
+            free_gauge(&c->gauges[i]);
             c->gauges[i] = gs;
             return MDWF_OK;
         }
@@ -328,6 +327,7 @@ int op_hop(const OpCtx& o, const SpinorView& out, const SpinorView& in, int out_
     a.out = out; a.in = in;
     if (xin) a.xin = *xin; else { a.xin.v = nullptr; a.xin.n = nullptr; a.xin.rs = a.xin.rn = 0; }
     a.g.v[0] = o.gs->v[0]; a.g.v[1] = o.gs->v[1];
+    for (int p = 0; p < 2; ++p) { a.g.prep[p] = reinterpret_cast<const float4*>(o.gs->prep[p]); a.g.nbr[p] = o.gs->nbr[p]; }
     if (mat >= 0) a.op = o.c->lsop[mat]; else a.op.kind = 0;
     a.cx = cx; a.ch = ch; a.partial = partial; a.par = out_par; a.nact = rl.nact;
     for (int i = 0; i < 64; ++i) a.rhs_list[i] = rl.rhs[i];
@@ -341,10 +341,10 @@ int op_hop(const OpCtx& o, const SpinorView& out, const SpinorView& in, int out_
 //   Mhat^dag v : t1 = M5^-dag v ; t2 = (A M5^-1)^dag H^dag t1 ; out = v - 1/4 A^dag H^dag t2
 //   Dhat^dag v : t2 = (A M5^-1)^dag H^dag v ; t1 = M5^dag v ; out = t1 - 1/4 A^dag H^dag t2
 int op_schur(const OpCtx& o, const SpinorView& out, const SpinorView& in, int par, int dagger, int symmetric,
-             const SpinorView& t1, const SpinorView& t2, const RhsList& rl, double* partial) {
+             const SpinorView& t1, const SpinorView& t2, const RhsList& rl, double* partial, int first_factor_done) {
     int rc;
     if (!dagger) {
-        if ((rc = op_ls(o, t1, in, MAT_A, nullptr, 0.0, 1.0, rl))) return rc;
+        if (!first_factor_done && (rc = op_ls(o, t1, in, MAT_A, nullptr, 0.0, 1.0, rl))) return rc;
         if ((rc = op_hop(o, t2, t1, 1 - par, 0, MAT_AM5INV, nullptr, 0.0, 1.0, rl))) return rc;
         if (symmetric) return op_hop(o, out, t2, par, 0, MAT_M5INV, &in, 1.0, -0.25, rl, partial);
         if ((rc = op_ls(o, t1, in, MAT_M5, nullptr, 0.0, 1.0, rl))) return rc;

@@ -71,6 +71,10 @@ struct SpinorView {
 
 struct GaugeView {
     const void* v[2];   // per parity of the link's base site; [mu][c][xh] vectors
+    // optional "prepared" stencil links (fp16 storage only): per OUTPUT parity, per site the 8 legs as 20 fp32 each
+    // (reconstructed, daggered for backward legs, bc sign folded) and the 8 neighbour half-indices
+    const float4* prep[2];
+    const int* nbr[2];
 };
 
 // ---------------------------------------------------------------------------------------------

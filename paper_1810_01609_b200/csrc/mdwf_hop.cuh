@@ -211,7 +211,13 @@ __device__ __forceinline__ void block_sum_store(double v, unsigned char* smem_ra
 #define MDWF_HOP_STCS true
 #endif
 #ifndef MDWF_HOP_MINB
-#define MDWF_HOP_MINB 3
+#define MDWF_HOP_MINB 3      // fp16 storage: 80 registers, 3 blocks/SM
+#endif
+#ifndef MDWF_HOP_MINB32
+#define MDWF_HOP_MINB32 4    // fp32: 64 registers, 4 blocks/SM (measured faster: latency-bound gathers)
+#endif
+#ifndef MDWF_HOP_MINB64
+#define MDWF_HOP_MINB64 2    // fp64: 128 registers, 2 blocks/SM (measured: 6.6 -> 5.8 ms on 48^3x64x10)
 #endif
 #define MDWF_LROW 20
 #define MDWF_LSITE (8 * MDWF_LROW + 4)
@@ -291,8 +297,43 @@ __device__ __forceinline__ SiteCoord decode_site(const Geom& g, int par, uint32_
     return c;
 }
 
+// Leg l (mu = l>>1, forward for even l) of site c: the link as the stencil multiplies it -- reconstructed from
+// the packed format, daggered for backward legs, times the boundary sign -- as 18 (+2 pad) reals; returns the
+// neighbour's half-index.
+template <typename S, int R>
+__device__ __forceinline__ int stage_link(const Geom& g, const GaugeView& gv, int par, const SiteCoord& c, int l,
+                                          typename Store<S>::real V[MDWF_LROW]) {
+    typedef typename Store<S>::real T;
+    const int mu = l >> 1, xh = c.xh;
+    const bool fwd = (l & 1) == 0;
+    int n;
+    bool wrap;
+    if (mu == 0) {
+        if (fwd) { wrap = (c.o == 1 && c.xx == g.XH - 1); n = wrap ? xh - (g.XH - 1) : xh + c.o; }
+        else { wrap = (c.o == 0 && c.xx == 0); n = wrap ? xh + (g.XH - 1) : xh - (1 - c.o); }
+    } else {
+        const int cm = mu == 1 ? c.y : mu == 2 ? c.z : c.t;
+        const int Lm = mu == 1 ? g.Y : mu == 2 ? g.Z : g.T;
+        const int sm = mu == 1 ? g.XH : mu == 2 ? g.XH * g.Y : g.XH * g.Y * g.Z;
+        if (fwd) { wrap = cm == Lm - 1; n = wrap ? xh - (Lm - 1) * sm : xh + sm; }
+        else { wrap = cm == 0; n = wrap ? xh + (Lm - 1) * sm : xh - sm; }
+    }
+    const T sgn = wrap ? (T)g.bc[mu] : (T)1;
+    T U[18];
+    load_link<S, R>(fwd ? gv.v[par] : gv.v[1 - par], mu, fwd ? xh : n, g.Vh, U);
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc) {
+            V[(r * 3 + cc) * 2] = sgn * (fwd ? U[(r * 3 + cc) * 2] : U[(cc * 3 + r) * 2]);
+            V[(r * 3 + cc) * 2 + 1] = sgn * (fwd ? U[(r * 3 + cc) * 2 + 1] : -U[(cc * 3 + r) * 2 + 1]);
+        }
+    V[18] = V[19] = 0;
+    return n;
+}
+
 template <typename S, int R, bool DAG, bool FUSED>
-__global__ void __launch_bounds__(256, (sizeof(typename Store<S>::real) == 8 ? 1 : MDWF_HOP_MINB)) hop_kernel(const Geom g, const HopArgs a) {
+__global__ void __launch_bounds__(256, (sizeof(S) == 8 ? MDWF_HOP_MINB64 : sizeof(S) == 4 ? MDWF_HOP_MINB32 : MDWF_HOP_MINB)) hop_kernel(const Geom g, const HopArgs a) {
     typedef typename Store<S>::real T;
     typedef Pack16<T> P;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -305,44 +346,35 @@ __global__ void __launch_bounds__(256, (sizeof(typename Store<S>::real) == 8 ? 1
     const int tile = blockIdx.x / a.nact;
     const int rhs = a.rhs_list[slot];
     // ---- stage the block's links and neighbour table --------------------------------------------------
-    for (int task = threadIdx.x; task < nsite * 8; task += blockDim.x) {
-        const int i = task >> 3, l = task & 7, mu = l >> 1;
-        const bool fwd = (l & 1) == 0;
-        const SiteCoord c = decode_site(g, a.par, (uint32_t)tile, (uint32_t)i);
-        const int xh = c.xh;
-        int n;
-        bool wrap;
-        if (mu == 0) {
-            if (fwd) { wrap = (c.o == 1 && c.xx == g.XH - 1); n = wrap ? xh - (g.XH - 1) : xh + c.o; }
-            else { wrap = (c.o == 0 && c.xx == 0); n = wrap ? xh + (g.XH - 1) : xh - (1 - c.o); }
-        } else {
-            const int cm = mu == 1 ? c.y : mu == 2 ? c.z : c.t;
-            const int Lm = mu == 1 ? g.Y : mu == 2 ? g.Z : g.T;
-            const int sm = mu == 1 ? g.XH : mu == 2 ? g.XH * g.Y : g.XH * g.Y * g.Z;
-            if (fwd) { wrap = cm == Lm - 1; n = wrap ? xh - (Lm - 1) * sm : xh + sm; }
-            else { wrap = cm == 0; n = wrap ? xh + (Lm - 1) * sm : xh - sm; }
+    if (Store<S>::HALF && a.g.prep[a.par] != nullptr) {
+        // prepared links: a block's sites are a consecutive xh range, so this is a coalesced copy of
+        // nsite*640 bytes (+ 32 bytes of neighbour indices per site); see stage_link()
+        const int xh0 = decode_site(g, a.par, (uint32_t)tile, 0u).xh;
+        const float4* src = a.g.prep[a.par] + (long long)xh0 * 40;
+        float4* dst = reinterpret_cast<float4*>(links);
+        for (int v = threadIdx.x; v < nsite * 40; v += blockDim.x) dst[v + v / 40] = __ldg(src + v);
+        const int* ns = a.g.nbr[a.par] + (long long)xh0 * 8;
+        for (int w = threadIdx.x; w < nsite * 8; w += blockDim.x) {
+            tab[(w >> 3) * 12 + (w & 7)] = __ldg(ns + w);
+            if ((w & 7) == 0) tab[(w >> 3) * 12 + 8] = xh0 + (w >> 3);
         }
-        const T sgn = wrap ? (T)g.bc[mu] : (T)1;
-        T U[18], V[MDWF_LROW];
-        load_link<S, R>(fwd ? a.g.v[a.par] : a.g.v[1 - a.par], mu, fwd ? xh : n, g.Vh, U);
+    } else {
+        for (int task = threadIdx.x; task < nsite * 8; task += blockDim.x) {
+            const int i = task >> 3, l = task & 7;
+            const SiteCoord c = decode_site(g, a.par, (uint32_t)tile, (uint32_t)i);
+            T V[MDWF_LROW];
+            const int n = stage_link<S, R>(g, a.g, a.par, c, l, V);
+            P* dst = reinterpret_cast<P*>(links + i * MDWF_LSITE + l * MDWF_LROW);
 #pragma unroll
-        for (int r = 0; r < 3; ++r)
+            for (int q = 0; q < MDWF_LROW / P::N; ++q) {
+                P t;
 #pragma unroll
-            for (int cc = 0; cc < 3; ++cc) {
-                V[(r * 3 + cc) * 2] = sgn * (fwd ? U[(r * 3 + cc) * 2] : U[(cc * 3 + r) * 2]);
-                V[(r * 3 + cc) * 2 + 1] = sgn * (fwd ? U[(r * 3 + cc) * 2 + 1] : -U[(cc * 3 + r) * 2 + 1]);
+                for (int e = 0; e < P::N; ++e) t.d[e] = V[q * P::N + e];
+                dst[q] = t;
             }
-        V[18] = V[19] = 0;
-        P* dst = reinterpret_cast<P*>(links + i * MDWF_LSITE + l * MDWF_LROW);
-#pragma unroll
-        for (int q = 0; q < MDWF_LROW / P::N; ++q) {
-            P t;
-#pragma unroll
-            for (int e = 0; e < P::N; ++e) t.d[e] = V[q * P::N + e];
-            dst[q] = t;
+            tab[i * 12 + l] = n;
+            if (l == 0) tab[i * 12 + 8] = c.xh;
         }
-        tab[i * 12 + l] = n;
-        if (l == 0) tab[i * 12 + 8] = xh;
     }
     __syncthreads();
     // ---- the stencil: one thread per (site, s) -----------------------------------------------------------

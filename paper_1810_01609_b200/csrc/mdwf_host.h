@@ -14,6 +14,8 @@ struct GaugeSet {
     int prec, recon;
     void* v[2];
     size_t bytes_per_parity;
+    float* prep[2];     // prepared stencil links (prec 16 only), else nullptr
+    int* nbr[2];
 };
 
 struct mdwf_field {
@@ -94,6 +96,7 @@ int launch_cg_p(mdwf_ctx* c, int prec, CgPArgs& a, cudaStream_t st);
 int launch_finish(mdwf_ctx* c, const RhsList& rl, double* out, double* out2, cudaStream_t st);
 int launch_pack(mdwf_ctx* c, int prec, bool unpack, PackArgs& a, cudaStream_t st);
 int pack_gauge(mdwf_ctx* c, const void* U, int prec, int recon, GaugeSet* gs, cudaStream_t st);
+void free_gauge(GaugeSet* gs);
 
 // ---- composite operators on packed fields (solver + API) ------------------------------------------
 struct OpCtx {
@@ -110,7 +113,8 @@ int op_hop(const OpCtx& o, const SpinorView& out, const SpinorView& in, int out_
 // Schur operator: out = Dhat/Mhat (dagger) in, parity p; t1, t2 are work fields; if partial != nullptr the
 // per-block |out|^2 sums are written there (to be finished with launch_finish)
 int op_schur(const OpCtx& o, const SpinorView& out, const SpinorView& in, int par, int dagger, int symmetric,
-             const SpinorView& t1, const SpinorView& t2, const RhsList& rl, double* partial = nullptr);
+             const SpinorView& t1, const SpinorView& t2, const RhsList& rl, double* partial = nullptr,
+             int first_factor_done = 0);   // non-dagger only: t1 already holds A*in (fused into the CG p-update)
 
 int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_opts* opts, mdwf_solve_info* info,
                cudaStream_t st, bool host_buffers);

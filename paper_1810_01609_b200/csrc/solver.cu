@@ -182,6 +182,7 @@ static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_o
         AxpbyArgs cp;
         cp.out = p; cp.a = r; cp.b = none; cp.ca = 1.0; cp.cb = 0.0; cp.partial = nullptr; cp.rl = act;
         if ((rc = launch_axpby(c, S.prec, S.prec, S.prec, cp, st))) return rc;
+        if ((rc = op_ls(S.lo, t, p, MAT_A, nullptr, 0.0, 1.0, act))) return rc;   // q = A p (later fused into the p-update)
         std::swap(rrOld, rrNew);   // dsc(rrOld) = |r_0|^2
     }
     cudaEvent_t e0, e1;
@@ -193,7 +194,7 @@ static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_o
     while (act.nact > 0 && rc == MDWF_OK) {
         if (!open) { cudaEventRecord(e0, st); open = true; }
         // t = S p, pAp = |t|^2 ; Ap = S^dag t   (out may alias the first work field, see op_schur)
-        if ((rc = op_schur(S.lo, t, p, par, 0, sym, t, wb, act, c->partial))) break;
+        if ((rc = op_schur(S.lo, t, p, par, 0, sym, t, wb, act, c->partial, 1))) break;   // t holds A p on entry
         if ((rc = launch_finish(c, act, S.dsc(SC_PAP), S.hsc(SC_PAP), st))) break;
         if ((rc = op_schur(S.lo, wa, t, par, 1, sym, wa, wb, act))) break;
         CgXrArgs u;
@@ -226,7 +227,7 @@ static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_o
             if (act.nact == 0) break;
         }
         CgPArgs q;
-        q.p = p; q.r = r; q.q = none; q.op.kind = 0; q.rr_new = S.dsc(rrNew); q.rr_old = S.dsc(rrOld); q.rl = act;
+        q.p = p; q.r = r; q.q = t; q.op = c->lsop[MAT_A]; q.rr_new = S.dsc(rrNew); q.rr_old = S.dsc(rrOld); q.rl = act;
         if ((rc = launch_cg_p(c, S.prec, q, st))) break;
         std::swap(rrOld, rrNew);
     }
