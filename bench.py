@@ -204,6 +204,15 @@ def run_ours(args):
             "frac": (pby / pms / 1e6) / hbm_peak if pms > 0 else None, "traffic": None, "peak_source": peak_src,
             "launches": pn, "avg_launch_ms": pms / pn if pn else None, "gflops": pfl / pms / 1e6 if pms > 0 else None,
             "share_of_step": pms / (ms_total if world == 1 else ms_step * args.steps)}
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic_r1.json")) as f:
+            tr = json.load(f).get("%s|inner%d|recon%d" % (cfg.name, inner, recon))
+        if tr and nrhs >= 1:
+            roof["traffic"] = tr["dram_bytes_per_launch"]
+            roof["traffic_source"] = tr["source"]
+            roof["algorithmic_bytes_per_launch"] = pby / pn if pn else None
+    except Exception:
+        pass
     h64 = prof[2]
     dsl = {"inner_hop_GBps": roof["achieved"], "inner_hop_GFLOPs": roof["gflops"],
            "fp64_hop_GBps": h64[1] / h64[0] / 1e6 if h64[0] > 0 else None,
