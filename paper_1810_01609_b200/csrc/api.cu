@@ -4,6 +4,8 @@
 #include <cmath>
 #include <cstring>
 #include <algorithm>
+#include <map>
+#include <cstdlib>
 
 using namespace mdwf;
 
@@ -60,6 +62,70 @@ static void build_matrices(int Ls, double M5, double b5, double c5, double mf, s
     }
 }
 
+// Compact 4D tiles for mdwf_hop_tile.cuh: choose a box Lx x Ly x Lz x Lt (Lx even) that divides the lattice, holds
+// exactly g.nsite output sites (so every kernel keeps the same thread <-> site blocking) and needs the fewest input
+// slots (box interior of the other parity + one-site halo); tabulate, for both parities of the box origin, the
+// local coordinates of outputs and slots and the slot of each leg.
+static int setup_tile4(mdwf_ctx* c) {
+    Geom& g = c->g;
+    g.q4nsite = 0; g.q4nslot = 0;
+    for (int i = 0; i < 4; ++i) g.q4L[i] = 1;
+    for (int p = 0; p < 2; ++p) { g.q4out[p] = nullptr; g.q4slot[p] = nullptr; g.q4nbr[p] = nullptr; }
+    const int dims[4] = {g.X, g.Y, g.Z, g.T};
+    int best[4] = {0, 0, 0, 0}, bestslots = 1 << 30;
+    for (int lx = 2; lx <= 8; lx += 2) for (int ly = 1; ly <= 6; ++ly) for (int lz = 1; lz <= 6; ++lz) for (int lt = 1; lt <= 6; ++lt) {
+        if (dims[0] % lx || dims[1] % ly || dims[2] % lz || dims[3] % lt) continue;
+        if (lx * ly * lz * lt != 2 * g.nsite) continue;
+        if ((ly * lz * lt) % 2 || (lx * lz * lt) % 2 || (lx * ly * lt) % 2 || (lx * ly * lz) % 2) continue;   // faces split evenly by parity
+        const int slots = g.nsite + ly * lz * lt + lx * lz * lt + lx * ly * lt + lx * ly * lz;
+        if (slots < bestslots && slots <= 255) { bestslots = slots; best[0] = lx; best[1] = ly; best[2] = lz; best[3] = lt; }
+    }
+    if (!best[0]) return MDWF_OK;      // no suitable box: the row-tile kernel is used
+    const int* L = best;
+    for (int pat = 0; pat < 2; ++pat) {
+        std::vector<int> outp, slotp;
+        std::vector<unsigned char> nbr;
+        std::map<int, int> slot_of;
+        auto pack = [](int x, int y, int z, int t) { return x | (y << 8) | (z << 16) | (t << 24); };
+        // interior input sites, then the halo, in (t, z, y, x) order over the extended box [-1, L]
+        for (int pass = 0; pass < 2; ++pass)
+            for (int t = -1; t <= L[3]; ++t) for (int z = -1; z <= L[2]; ++z) for (int y = -1; y <= L[1]; ++y) for (int x = -1; x <= L[0]; ++x) {
+                const int outside = (x < 0 || x >= L[0]) + (y < 0 || y >= L[1]) + (z < 0 || z >= L[2]) + (t < 0 || t >= L[3]);
+                if (outside != pass) continue;                       // pass 0: interior, pass 1: faces (exactly one coordinate out)
+                if (((x + y + z + t + pat) & 1) == 0) continue;      // inputs have the other parity (x+..+pat odd; -1 is odd too)
+                const int key = pack(x + 1, y + 1, z + 1, t + 1);
+                slot_of[key] = (int)slotp.size();
+                slotp.push_back(key);
+            }
+        for (int t = 0; t < L[3]; ++t) for (int z = 0; z < L[2]; ++z) for (int y = 0; y < L[1]; ++y) for (int x = 0; x < L[0]; ++x) {
+            if ((x + y + z + t + pat) & 1) continue;
+            outp.push_back(pack(x, y, z, t));
+            for (int mu = 0; mu < 4; ++mu)
+                for (int dir = 0; dir < 2; ++dir) {
+                    int cc[4] = {x, y, z, t};
+                    cc[mu] += dir == 0 ? 1 : -1;
+                    const auto it = slot_of.find(pack(cc[0] + 1, cc[1] + 1, cc[2] + 1, cc[3] + 1));
+                    if (it == slot_of.end()) MDWF_FAIL(c, MDWF_EINVAL, "internal: 4D tile table is inconsistent");
+                    nbr.push_back((unsigned char)it->second);
+                }
+        }
+        if ((int)outp.size() != g.nsite || (int)slotp.size() != bestslots) MDWF_FAIL(c, MDWF_EINVAL, "internal: 4D tile counts (%zu, %zu)", outp.size(), slotp.size());
+        void *d0, *d1, *d2;
+        MDWF_CUDA(c, cudaMalloc(&d0, outp.size() * 4));
+        MDWF_CUDA(c, cudaMalloc(&d1, slotp.size() * 4));
+        MDWF_CUDA(c, cudaMalloc(&d2, nbr.size()));
+        MDWF_CUDA(c, cudaMemcpy(d0, outp.data(), outp.size() * 4, cudaMemcpyHostToDevice));
+        MDWF_CUDA(c, cudaMemcpy(d1, slotp.data(), slotp.size() * 4, cudaMemcpyHostToDevice));
+        MDWF_CUDA(c, cudaMemcpy(d2, nbr.data(), nbr.size(), cudaMemcpyHostToDevice));
+        c->q4dev[3 * pat] = d0; c->q4dev[3 * pat + 1] = d1; c->q4dev[3 * pat + 2] = d2;
+        g.q4out[pat] = (const int*)d0; g.q4slot[pat] = (const int*)d1; g.q4nbr[pat] = (const unsigned char*)d2;
+    }
+    for (int i = 0; i < 4; ++i) g.q4L[i] = L[i];
+    g.q4nsite = g.nsite; g.q4nslot = bestslots;
+    g.q4dTx = make_fastdiv(g.X / L[0]); g.q4dTy = make_fastdiv(g.Y / L[1]); g.q4dTt = make_fastdiv(g.T / L[3]);
+    return MDWF_OK;
+}
+
 // The structured form of the same operators that the kernels apply (LsOp, mdwf_hop.cuh).
 static void build_lsops(int Ls, double M5, double b5, double c5, double mf, LsOp ops[MAT_COUNT]) {
     const double a = b5 * (4.0 - M5) + 1.0, d = c5 * (4.0 - M5) - 1.0, kappa = -d / a;
@@ -106,10 +172,11 @@ static void lsop_host(const LsOp& op, int Ls, int chi, const std::vector<double>
 // L2 (measured on B200: 48^3x64 Ls=10 is fastest at zc = 8)
 static int pick_zc(const mdwf_ctx* c, int want) {
     const Geom& g = c->g;
-    if (want > 0 && g.Z % want == 0 && want % g.tz == 0) return want;
-    int best = g.tz;
+    const int lz = g.q4nsite > 0 ? g.q4L[2] : 1;
+    if (want > 0 && g.Z % want == 0 && want % g.tz == 0 && want % lz == 0) return want;
+    int best = 0;
     for (int z = g.tz; z <= g.Z; z += g.tz)
-        if (g.Z % z == 0 && (double)g.XH * g.Y * z * g.Ls * 96.0 <= 9.0e6) best = z;
+        if (g.Z % z == 0 && z % lz == 0 && (best == 0 || (double)g.XH * g.Y * z * g.Ls * 96.0 <= 9.0e6)) best = z;
     return best;
 }
 static void set_zc(mdwf_ctx* c, int zc) {
@@ -119,6 +186,7 @@ static void set_zc(mdwf_ctx* c, int zc) {
     g.dSlab = make_fastdiv((uint32_t)(g.XH * g.Y * zc));
     g.dTslab = make_fastdiv((uint32_t)(g.XH * g.Y * zc) * (uint32_t)g.T);
     g.dnTzs = make_fastdiv((uint32_t)(zc / g.tz));
+    g.q4dTzs = make_fastdiv((uint32_t)(zc / (g.q4nsite > 0 ? g.q4L[2] : 1)));
 }
 // Sites of a block: a box txh*ty*tz*tt (x fastest) that divides the lattice, filled greedily along x, then y, z, t
 // up to min(256/Ls, 32) sites, i.e. (nearly) whole x-rows in storage order.  Compact 4D boxes (e.g. 4x4x2x2) were
@@ -167,7 +235,8 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     mdwf_ctx* c = new mdwf_ctx;
     c->geo = *geo;
     c->M5 = M5; c->b5 = b5; c->c5 = c5; c->mf = mf;
-    c->partial = nullptr; c->dscal = nullptr; c->hscal = nullptr; c->launches = 0; c->prof_on = 0;
+    c->partial = nullptr; c->dscal = nullptr; c->hscal = nullptr; c->launches = 0; c->prof_on = 0; c->use_tiled = 0;
+    for (int i = 0; i < 6; ++i) c->q4dev[i] = nullptr;
     for (int i = 0; i < 3; ++i) { c->prof_ms[i] = c->prof_bytes[i] = c->prof_flops[i] = 0.0; c->prof_n[i] = 0; }
     *out = c;   // returned even on failure so that mdwf_last_error can be read; caller destroys it
     long long v4 = 1;
@@ -198,6 +267,11 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     for (int m = 0; m < 4; ++m) g.bc[m] = geo->bc[m];
     g.dLs = make_fastdiv(g.Ls); g.dXH = make_fastdiv(g.XH); g.dY = make_fastdiv(g.Y); g.dZ = make_fastdiv(g.Z);
     pick_tile(c, 0);
+    {
+        const int rc4 = setup_tile4(c);
+        if (rc4) return rc4;
+    }
+    c->use_tiled = getenv("MDWF_HOP_TILED") ? atoi(getenv("MDWF_HOP_TILED")) : 0;
     set_zc(c, pick_zc(c, 0));
     MDWF_CUDA(c, cudaMalloc(&c->partial, sizeof(double) * 64 * (size_t)c->nblk));
     MDWF_CUDA(c, cudaMalloc(&c->dscal, sizeof(double) * 8 * 64));
@@ -211,6 +285,7 @@ int mdwf_destroy(mdwf_ctx* c) {
     if (!c) return MDWF_OK;
     for (size_t i = 0; i < c->gauges.size(); ++i) free_gauge(&c->gauges[i]);
     for (auto& kv : c->temps) for (mdwf_field* f : kv.second) free_field(f);
+    for (int i = 0; i < 6; ++i) if (c->q4dev[i]) cudaFree(c->q4dev[i]);
     prof_drain(c);
     for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
     if (c->partial) cudaFree(c->partial);
@@ -286,6 +361,7 @@ int mdwf_set_tiling(mdwf_ctx* c, int zc) {
     if (!c) return MDWF_EINVAL;
     if (zc < 0 || (zc > 0 && (c->g.Z % zc != 0 || zc % c->g.tz != 0)))
         MDWF_FAIL(c, MDWF_EINVAL, "zc = %d must divide Z = %d and be a multiple of the tile depth %d", zc, c->g.Z, c->g.tz);
+    if (zc > 0 && c->g.q4nsite > 0 && zc % c->g.q4L[2] != 0) MDWF_FAIL(c, MDWF_EINVAL, "zc = %d must be a multiple of the 4D tile depth %d", zc, c->g.q4L[2]);
     set_zc(c, pick_zc(c, zc));
     return MDWF_OK;
 }

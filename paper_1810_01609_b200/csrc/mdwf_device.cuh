@@ -59,6 +59,14 @@ struct Geom {
     int txh, ty, tz, tt, nsite;
     FastDiv dtxh, dty, dtz;             // in-tile decode
     FastDiv dnTx, dnTy, dnTzs, dnTt;    // tile-index decode: tiles per row, per column, per slab depth, per T
+    // compact 4D tiles with shared-memory staged neighbours (mdwf_hop_tile.cuh); q4nsite == 0 -> not available.
+    // q4L: box extents in lattice sites; tables per parity pattern of the box origin: packed local coordinates of
+    // the output sites, of the input slots (+1, so the halo fits), and the slot of each of the 8 legs.
+    int q4L[4], q4nsite, q4nslot;
+    const int* q4out[2];
+    const int* q4slot[2];
+    const unsigned char* q4nbr[2];
+    FastDiv q4dTx, q4dTy, q4dTzs, q4dTt;
 };
 
 // one packed spinor field set (nrhs fields of one parity)

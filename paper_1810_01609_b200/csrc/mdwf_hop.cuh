@@ -219,21 +219,23 @@ __device__ __forceinline__ void block_sum_store(double v, unsigned char* smem_ra
 #ifndef MDWF_HOP_MINB64
 #define MDWF_HOP_MINB64 2    // fp64: 128 registers, 2 blocks/SM (measured: 6.6 -> 5.8 ms on 48^3x64x10)
 #endif
+#ifndef MDWF_TILE_MINB32
+#define MDWF_TILE_MINB32 2
+#endif
+#ifndef MDWF_TILE_MINB16
+#define MDWF_TILE_MINB16 3
+#endif
 #define MDWF_LROW 20
 #define MDWF_LSITE (8 * MDWF_LROW + 4)
 template <typename T> __host__ __device__ inline size_t smem_bytes_links(int nsite) {
     return (size_t)nsite * (MDWF_LSITE * sizeof(T) + 12 * sizeof(int));
 }
 
-// one stencil leg from staged data: U (smem, already U or U^dag, sign folded), neighbour 5D index nidx
-template <typename S, int MU, bool FWD, bool DAG>
-__device__ __forceinline__ void leg2(const SpinorView& in, int rhs, int N5h, int nidx,
-                                     const typename Store<S>::real* __restrict__ Us,
-                                     typename Store<S>::real acc[24]) {
-    typedef typename Store<S>::real T;
+// one stencil leg from staged data: neighbour spinor v (unscaled, scale sc), U (smem, already U or U^dag, bc sign
+// folded): acc += sc * rebuild( U * project(v) )
+template <typename T, int MU, bool FWD, bool DAG>
+__device__ __forceinline__ void leg_core(const T v[24], T sc, const T* __restrict__ Us, T acc[24]) {
     constexpr int SGN = (FWD ? -1 : 1) * (DAG ? -1 : 1);
-    T v[24], sc;
-    load_raw<S>(in, rhs, nidx, N5h, v, sc);
     T h[12], w[12], U[MDWF_LROW];
     project<MU, SGN, T>(v, h);
     typedef Pack16<T> P;
@@ -266,6 +268,17 @@ __device__ __forceinline__ void leg2(const SpinorView& in, int rhs, int N5h, int
             acc[18 + c * 2] = fma_<T>(cs, w1r, acc[18 + c * 2]); acc[18 + c * 2 + 1] = fma_<T>(cs, w1i, acc[18 + c * 2 + 1]);
         }
     }
+}
+
+// the same with the neighbour gathered from global memory (5D index nidx)
+template <typename S, int MU, bool FWD, bool DAG>
+__device__ __forceinline__ void leg2(const SpinorView& in, int rhs, int N5h, int nidx,
+                                     const typename Store<S>::real* __restrict__ Us,
+                                     typename Store<S>::real acc[24]) {
+    typedef typename Store<S>::real T;
+    T v[24], sc;
+    load_raw<S>(in, rhs, nidx, N5h, v, sc);
+    leg_core<T, MU, FWD, DAG>(v, sc, Us, acc);
 }
 
 struct HopArgs {

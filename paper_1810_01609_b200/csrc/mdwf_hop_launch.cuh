@@ -2,6 +2,7 @@
 // hop_f64.cu / hop_f32.cu / hop_f16.cu so the three compile in parallel.
 #pragma once
 #include "mdwf_host.h"
+#include "mdwf_hop_tile.cuh"
 #include <set>
 
 namespace mdwf {
@@ -11,7 +12,7 @@ static inline int launch_with_smem(mdwf_ctx* c, K kern, int grid, int block, siz
                                    const Geom& g, const HopArgs& a) {
     static std::set<const void*> raised;
     if (smem > 48 * 1024 && !raised.count((const void*)kern)) {
-        MDWF_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        MDWF_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         raised.insert((const void*)kern);
     }
     kern<<<grid, block, smem, st>>>(g, a);
@@ -28,6 +29,17 @@ static int launch_hop_SR(mdwf_ctx* c, int dagger, int fused, HopArgs& a, cudaStr
     if (fused) {
         smem = (size_t)c->block * sizeof(double);
         if (a.op.kind) smem = std::max(smem, (size_t)smem_reals_G<T>(c->g.Ls, c->block) * sizeof(T));
+    }
+    if (c->use_tiled && c->g.q4nsite > 0 && sizeof(T) == 4) {
+        // shared-memory staged 4D tiles; the epilogue reuses the spinor staging area
+        const size_t st_bytes = smem_bytes_tile<S>(c->g.q4nsite, c->g.q4nslot, c->g.Ls);
+        const size_t need = std::max(st_bytes, smem);
+        if (fused) {
+            if (dagger) return launch_with_smem(c, hop_tile_kernel<S, R, true, true>, grid, c->block, need, st, c->g, a);
+            return launch_with_smem(c, hop_tile_kernel<S, R, false, true>, grid, c->block, need, st, c->g, a);
+        }
+        if (dagger) return launch_with_smem(c, hop_tile_kernel<S, R, true, false>, grid, c->block, need, st, c->g, a);
+        return launch_with_smem(c, hop_tile_kernel<S, R, false, false>, grid, c->block, need, st, c->g, a);
     }
     smem += smem_bytes_links<T>(c->block / c->g.Ls);
     if (fused) {

@@ -50,6 +50,8 @@ struct mdwf_ctx {
     double prof_ms[3], prof_bytes[3], prof_flops[3];
     long long prof_n[3];
     int sm_count;
+    int use_tiled;             // hop through mdwf_hop_tile.cuh (fp32/fp16 storage) when the geometry allows
+    void* q4dev[6];            // device tables of the 4D tiles (freed at destroy)
     const GaugeSet* find_gauge(int prec, int recon) const {
         for (size_t i = 0; i < gauges.size(); ++i)
             if (gauges[i].prec == prec && gauges[i].recon == recon) return &gauges[i];
