@@ -218,9 +218,12 @@ __device__ __forceinline__ void store_spinor_h(const SpinorView& f, int r, int i
     float m = 0.f;
 #pragma unroll
     for (int i = 0; i < 24; ++i) m = fmaxf(m, fabsf(v[i]));
-    const float inv = m > 0.f ? __fdividef(1.0f, m) : 0.f;
+    // sites whose largest component is below 1e-30 (far outside the support of a point source after a few
+    // iterations: denormal range, 1/m would overflow) are stored as exact zeros
+    const bool nz = m > 1e-30f;
+    const float inv = nz ? __fdividef(1.0f, m) : 0.f;
     char* p = const_cast<char*>(site_ptr<__half>(f, r, idx));
-    st_<CS>(reinterpret_cast<float*>(p - (idx & 31) * 12 + 3 * 512), m);
+    st_<CS>(reinterpret_cast<float*>(p - (idx & 31) * 12 + 3 * 512), nz ? m : 0.f);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         uint4 t;

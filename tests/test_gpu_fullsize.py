@@ -48,6 +48,81 @@ def patch_residual(cfg, p_big, U, x, b, origin, P=8):
     return rn, bn
 
 
+def test_c3_point_source_propagator_full_size():
+    """config 3: 24^3x64, Ls=8, 12 point sources, 16-bit inner CG to 1e-8, 4D in / 4D out (batched multi-rhs)."""
+    import paper_1810_01609_b200 as mdwf
+    cfg = synth.CONFIGS[3]
+    ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
+    U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(3, 1), device="cuda")
+    ctx.mdwf_load_gauge(U, 64, 18)
+    ctx.mdwf_load_gauge(U, 16, 12)
+    eta = synth.point_sources_4d(cfg.dims).cuda()
+    x5, res = ctx.mdwf_solve(eta, tol=cfg.tol, inner_prec=16, recon=12, src_kind=1, out_kind=0)
+    assert res.status == mdwf.OK, res
+    assert max(res.true_resid) <= cfg.tol
+    cols = [0, 5, 11]
+    b5 = ctx.mdwf_wall_inject(eta[cols].contiguous())
+    Dx = ctx.mdwf_dslash(mdwf.OP_FULL, x5[cols].contiguous(), prec=64, recon=18)
+    for r in range(3):
+        assert float(torch.linalg.vector_norm(b5[r] - Dx[r]) / torch.linalg.vector_norm(b5[r])) <= cfg.tol
+    # oracle check of D on a patch around the source-free region and of the 4D projection rule on it
+    origin = (4, 6, 8, 10)
+    idx = torch.from_numpy(patch_indices(cfg.dims, origin)).cuda()
+    pp = oracle.Params(dims=(8,) * 4, Ls=cfg.Ls, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=cfg.mf, bc=(1, 1, 1, 1))
+    Do = oracle.D(pp, U[:, idx].cpu().numpy(), x5[cols][:, :, idx].cpu().numpy()).reshape(3, cfg.Ls, 8, 8, 8, 8, 12)
+    Dg = Dx[:, :, idx].cpu().numpy().reshape(3, cfg.Ls, 8, 8, 8, 8, 12)
+    c = slice(2, 6)
+    # away from the source D x = 0 up to the residual, so the difference is measured against |x| on the core
+    xc = x5[cols][:, :, idx].cpu().numpy().reshape(3, cfg.Ls, 8, 8, 8, 8, 12)[:, :, c, c, c, c]
+    assert np.linalg.norm((Dg - Do)[:, :, c, c, c, c]) <= 1e-12 * np.linalg.norm(xc)
+    q = ctx.mdwf_wall_project(x5)
+    qo = oracle.wall_project(pp, x5[cols][:, :, idx].cpu().numpy())
+    assert np.array_equal(q[cols][:, idx].cpu().numpy(), qo)
+    ctx.mdwf_destroy()
+
+
+def test_c4_fh_chain_full_size():
+    """config 4: 32^3x48, Ls=12: smeared 12-column source -> S ; gamma_z gamma_5 S on all t ; S_FH ; C(t) with and
+    without the insertion.  Solves are checked through the fp64 residual of the 5D systems (sampled columns), the
+    sequential source and one timeslice of each contraction against the oracle's literal sums."""
+    import paper_1810_01609_b200 as mdwf
+    cfg = synth.CONFIGS[4]
+    ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
+    U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(4, 1), device="cuda")
+    ctx.mdwf_load_gauge(U, 64, 18)
+    ctx.mdwf_load_gauge(U, 16, 12)
+    eta = synth.gaussian_smeared_sources_4d(cfg.dims, width=3.0).cuda()
+    kw = dict(tol=cfg.tol, inner_prec=16, recon=12, src_kind=1, out_kind=1)
+    S, r1 = ctx.mdwf_solve(eta, **kw)
+    G = oracle.gamma(2) @ oracle.gamma(4)
+    seq = ctx.mdwf_seq_source(S, G)
+    SFH, r2 = ctx.mdwf_solve(seq, **kw)
+    assert r1.status == mdwf.OK and r2.status == mdwf.OK, (r1, r2)
+    assert max(r1.true_resid) <= cfg.tol and max(r2.true_resid) <= cfg.tol
+    # sequential source: exact signed permutation of the input, all columns
+    Sn = S[:2].cpu().numpy()
+    assert rel(seq[:2].cpu().numpy(), oracle.seq_source(cfg.dims, Sn, G)) <= 1e-15
+    # 5D residual of two columns of the second solve, by the fp64 FULL operator
+    x5, r3 = ctx.mdwf_solve(seq[3:5].contiguous(), tol=cfg.tol, inner_prec=16, recon=12, src_kind=1, out_kind=0)
+    b5 = ctx.mdwf_wall_inject(seq[3:5].contiguous())
+    Dx = ctx.mdwf_dslash(mdwf.OP_FULL, x5, prec=64, recon=18)
+    for r in range(2):
+        assert float(torch.linalg.vector_norm(b5[r] - Dx[r]) / torch.linalg.vector_norm(b5[r])) <= cfg.tol
+    assert rel(ctx.mdwf_wall_project(x5).cpu().numpy(), SFH[3:5].cpu().numpy()) <= 1e-6
+    # contractions: one timeslice by the oracle's literal loops
+    P = 0.5 * (np.eye(4) + oracle.gamma(3))
+    c0 = ctx.mdwf_nucleon_2pt(S, S, S, P).cpu().numpy()
+    cfh = (ctx.mdwf_nucleon_2pt(SFH, S, S, P) + ctx.mdwf_nucleon_2pt(S, S, SFH, P) - ctx.mdwf_nucleon_2pt(S, SFH, S, P)).cpu().numpy()
+    t = 5
+    Sh, Fh = S.cpu().numpy(), SFH.cpu().numpy()
+    o0 = oracle.nucleon_2pt(cfg.dims, Sh, Sh, Sh, P, t_lo=t, t_hi=t)[t]
+    ofh = (oracle.nucleon_2pt(cfg.dims, Fh, Sh, Sh, P, t_lo=t, t_hi=t)[t] + oracle.nucleon_2pt(cfg.dims, Sh, Sh, Fh, P, t_lo=t, t_hi=t)[t]
+           - oracle.nucleon_2pt(cfg.dims, Sh, Fh, Sh, P, t_lo=t, t_hi=t)[t])
+    assert abs(c0[t] - o0) <= 1e-11 * abs(o0) and abs(cfh[t] - ofh) <= 1e-11 * abs(ofh)
+    assert np.isfinite(c0).all() and np.isfinite(cfh).all()
+    ctx.mdwf_destroy()
+
+
 @pytest.fixture(scope="module")
 def c5():
     import paper_1810_01609_b200 as mdwf
@@ -56,7 +131,10 @@ def c5():
     U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(5, 1), device="cuda")
     for prec, recon in [(64, 18), (32, 12), (16, 12)]:
         ctx.mdwf_load_gauge(U, prec, recon)
-    return mdwf, cfg, ctx, U
+    yield mdwf, cfg, ctx, U
+    ctx.mdwf_destroy()
+    del U
+    torch.cuda.empty_cache()
 
 
 def test_c5_hop_two_slices_vs_oracle(c5):
@@ -101,73 +179,3 @@ def test_c5_solve_sampled_residual(c5):
         assert rel(Dg[:, :, c, c, c, c], Do[:, :, c, c, c, c]) <= 1e-12
         rn, bn = patch_residual(cfg, p_big, U, x, b, origin)
         assert (rn / bn <= 20 * cfg.tol).all(), (origin, rn / bn)
-
-
-def test_c3_point_source_propagator_full_size():
-    """config 3: 24^3x64, Ls=8, 12 point sources, 16-bit inner CG to 1e-8, 4D in / 4D out (batched multi-rhs)."""
-    import paper_1810_01609_b200 as mdwf
-    cfg = synth.CONFIGS[3]
-    ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
-    U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(3, 1), device="cuda")
-    ctx.mdwf_load_gauge(U, 64, 18)
-    ctx.mdwf_load_gauge(U, 16, 12)
-    eta = synth.point_sources_4d(cfg.dims).cuda()
-    x5, res = ctx.mdwf_solve(eta, tol=cfg.tol, inner_prec=16, recon=12, src_kind=1, out_kind=0)
-    assert res.status == mdwf.OK, res
-    b5 = ctx.mdwf_wall_inject(eta)
-    Dx = ctx.mdwf_dslash(mdwf.OP_FULL, x5, prec=64, recon=18)
-    for r in range(12):
-        assert float(torch.linalg.vector_norm(b5[r] - Dx[r]) / torch.linalg.vector_norm(b5[r])) <= cfg.tol
-    # oracle check of D on a patch around the source-free region and of the 4D projection rule on it
-    origin = (4, 6, 8, 10)
-    idx = torch.from_numpy(patch_indices(cfg.dims, origin)).cuda()
-    pp = oracle.Params(dims=(8,) * 4, Ls=cfg.Ls, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=cfg.mf, bc=(1, 1, 1, 1))
-    cols = [0, 5, 11]
-    Do = oracle.D(pp, U[:, idx].cpu().numpy(), x5[cols][:, :, idx].cpu().numpy()).reshape(3, cfg.Ls, 8, 8, 8, 8, 12)
-    Dg = Dx[cols][:, :, idx].cpu().numpy().reshape(3, cfg.Ls, 8, 8, 8, 8, 12)
-    c = slice(2, 6)
-    assert rel(Dg[:, :, c, c, c, c], Do[:, :, c, c, c, c]) <= 1e-12
-    q = ctx.mdwf_wall_project(x5)
-    qo = oracle.wall_project(pp, x5[cols][:, :, idx].cpu().numpy())
-    assert np.array_equal(q[cols][:, idx].cpu().numpy(), qo)
-
-
-def test_c4_fh_chain_full_size():
-    """config 4: 32^3x48, Ls=12: smeared 12-column source -> S ; gamma_z gamma_5 S on all t ; S_FH ; C(t) with and
-    without the insertion.  Solves are checked through the fp64 residual of the 5D systems (sampled columns), the
-    sequential source and one timeslice of each contraction against the oracle's literal sums."""
-    import paper_1810_01609_b200 as mdwf
-    cfg = synth.CONFIGS[4]
-    ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
-    U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(4, 1), device="cuda")
-    ctx.mdwf_load_gauge(U, 64, 18)
-    ctx.mdwf_load_gauge(U, 16, 12)
-    eta = synth.gaussian_smeared_sources_4d(cfg.dims, width=3.0).cuda()
-    kw = dict(tol=cfg.tol, inner_prec=16, recon=12, src_kind=1, out_kind=1)
-    S, r1 = ctx.mdwf_solve(eta, **kw)
-    G = oracle.gamma(2) @ oracle.gamma(4)
-    seq = ctx.mdwf_seq_source(S, G)
-    SFH, r2 = ctx.mdwf_solve(seq, **kw)
-    assert r1.status == mdwf.OK and r2.status == mdwf.OK, (r1, r2)
-    assert max(r1.true_resid) <= cfg.tol and max(r2.true_resid) <= cfg.tol
-    # sequential source: exact signed permutation of the input, all columns
-    Sn = S[:2].cpu().numpy()
-    assert rel(seq[:2].cpu().numpy(), oracle.seq_source(cfg.dims, Sn, G)) <= 1e-15
-    # 5D residual of two columns of the second solve, by the fp64 FULL operator
-    x5, r3 = ctx.mdwf_solve(seq[3:5].contiguous(), tol=cfg.tol, inner_prec=16, recon=12, src_kind=1, out_kind=0)
-    b5 = ctx.mdwf_wall_inject(seq[3:5].contiguous())
-    Dx = ctx.mdwf_dslash(mdwf.OP_FULL, x5, prec=64, recon=18)
-    for r in range(2):
-        assert float(torch.linalg.vector_norm(b5[r] - Dx[r]) / torch.linalg.vector_norm(b5[r])) <= cfg.tol
-    assert rel(ctx.mdwf_wall_project(x5).cpu().numpy(), SFH[3:5].cpu().numpy()) <= 1e-6
-    # contractions: one timeslice by the oracle's literal loops
-    P = 0.5 * (np.eye(4) + oracle.gamma(3))
-    c0 = ctx.mdwf_nucleon_2pt(S, S, S, P).cpu().numpy()
-    cfh = (ctx.mdwf_nucleon_2pt(SFH, S, S, P) + ctx.mdwf_nucleon_2pt(S, S, SFH, P) - ctx.mdwf_nucleon_2pt(S, SFH, S, P)).cpu().numpy()
-    t = 5
-    Sh, Fh = S.cpu().numpy(), SFH.cpu().numpy()
-    o0 = oracle.nucleon_2pt(cfg.dims, Sh, Sh, Sh, P, t_lo=t, t_hi=t)[t]
-    ofh = (oracle.nucleon_2pt(cfg.dims, Fh, Sh, Sh, P, t_lo=t, t_hi=t)[t] + oracle.nucleon_2pt(cfg.dims, Sh, Sh, Fh, P, t_lo=t, t_hi=t)[t]
-           - oracle.nucleon_2pt(cfg.dims, Sh, Fh, Sh, P, t_lo=t, t_hi=t)[t])
-    assert abs(c0[t] - o0) <= 1e-11 * abs(o0) and abs(cfh[t] - ofh) <= 1e-11 * abs(ofh)
-    assert np.isfinite(c0).all() and np.isfinite(cfh).all()

@@ -103,3 +103,42 @@ def test_not_converged_is_reported():
     b = synth.gaussian_spinor(cfg.dims, cfg.Ls, 1, synth.seed_for(1, 2))
     x, res = ctx.mdwf_solve(b.cuda(), tol=1e-10, inner_prec=64, recon=18, max_iter=3)
     assert res.status == mdwf.NOT_CONVERGED and res.rhs_status[0] == mdwf.NOT_CONVERGED
+
+
+def test_edge_cases_zero_rhs_max_batch_and_ls1():
+    """degenerate inputs: an all-zero rhs inside a batch (solution 0, converged at once), the maximum batch of 64 rhs
+    through mdwf_dslash, and Ls = 1 (L has only the -mf wraps, A21) solved in the asymmetric form on parity 1."""
+    import paper_1810_01609_b200 as mdwf
+    cfg = synth.CONFIGS[1]
+    p = oracle.Params(dims=cfg.dims, Ls=cfg.Ls, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=cfg.mf, bc=cfg.bc)
+    U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(1, 1))
+    ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
+    ctx.mdwf_load_gauge(U.cuda(), 64, 18)
+    ctx.mdwf_load_gauge(U.cuda(), 16, 12)
+    b = synth.gaussian_spinor(cfg.dims, cfg.Ls, 3, synth.seed_for(1, 4))
+    b[1] = 0
+    x, res = ctx.mdwf_solve(b.cuda(), tol=1e-9, inner_prec=16, recon=12)
+    assert res.status == mdwf.OK and res.iters[1] == 0
+    xn = x.cpu().numpy()
+    assert np.all(xn[1] == 0)
+    tr = oracle.true_residual(p, U.numpy(), xn[[0, 2]], b.numpy()[[0, 2]])
+    assert tr.max() <= 1e-9
+    # 64 rhs through the Dslash entry point
+    psi = synth.gaussian_spinor(cfg.dims, cfg.Ls, 64, synth.seed_for(1, 5)).numpy()
+    same = oracle.mask(p, psi, 0)
+    exp = oracle.to_half(oracle.schur(p, U.numpy(), same, 0, False, True), cfg.dims, 0)
+    got = ctx.mdwf_dslash(mdwf.OP_DHAT_SYM, torch.from_numpy(oracle.to_half(same, cfg.dims, 0)).cuda(), prec=64, recon=18)
+    assert rel(got.cpu().numpy(), exp) <= 1e-12
+    with pytest.raises(mdwf.MdwfError):
+        ctx.mdwf_dslash(mdwf.OP_HOP, torch.zeros((65, cfg.Ls, cfg.V4 // 2, 4, 3), dtype=torch.complex128, device="cuda"))
+    # Ls = 1
+    dims = (4, 2, 6, 4)
+    p1 = oracle.Params(dims=dims, Ls=1, M5=1.4, b5=1.2, c5=0.3, mf=0.2, bc=(1, -1, 1, -1))
+    U1 = synth.gauge_field(dims, 0.3, 77)
+    c1 = mdwf.Context(dims, 1, 1.4, 1.2, 0.3, 0.2, bc=(1, -1, 1, -1))
+    c1.mdwf_load_gauge(U1.cuda(), 64, 18)
+    c1.mdwf_load_gauge(U1.cuda(), 32, 8)
+    b1 = synth.gaussian_spinor(dims, 1, 2, 78)
+    x1, r1 = c1.mdwf_solve(b1.cuda(), tol=1e-10, inner_prec=32, recon=8, parity=1, symmetric=False)
+    assert r1.status == mdwf.OK
+    assert oracle.true_residual(p1, U1.numpy(), x1.cpu().numpy(), b1.numpy()).max() <= 1e-10
