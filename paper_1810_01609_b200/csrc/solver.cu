@@ -15,6 +15,7 @@
 #include <cmath>
 #include <algorithm>
 #include <cstring>
+#include <string>
 
 namespace mdwf {
 
@@ -305,7 +306,7 @@ int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_o
     if (opts->batch <= 0) {
         size_t fr = 0, tot = 0;
         MDWF_CUDA(c, cudaMemGetInfo(&fr, &tot));
-        const size_t per = per_rhs_bytes(g, S.prec, S.px) + (host_buffers ? in_per + out_per : 0);
+        const size_t per = per_rhs_bytes(g, S.prec, S.px) + (host_buffers ? 2 * (in_per + out_per) : 0);
         const size_t fit = (size_t)(0.92 * (double)fr) / per;
         if (fit < 1) MDWF_FAIL(c, MDWF_ENOMEM, "not enough free device memory for one rhs (%zu needed, %zu free)", per, fr);
         nb = (int)std::min<size_t>(fit, (size_t)nrhs);
@@ -318,38 +319,74 @@ int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_o
     const long long l0 = c->launches;
     double inner_ms = 0.0;
     int rc = MDWF_OK;
-    void *dbuf_in = nullptr, *dbuf_out = nullptr;
-    for (int r0 = 0; r0 < nrhs && rc == MDWF_OK; r0 += nb) {
-        S.nb = std::min(nb, nrhs - r0);
-        if (!host_buffers) {
+    if (!host_buffers) {
+        for (int r0 = 0; r0 < nrhs && rc == MDWF_OK; r0 += nb) {
+            S.nb = std::min(nb, nrhs - r0);
             rc = solve_batch(S, (double*)x, (const double*)b, opts, info, r0, &inner_ms);
-        } else {
-            // stage this batch through device buffers; copies are part of the call (mdwf.h)
-            if (!dbuf_in) {
-                if (cudaMalloc(&dbuf_in, in_per * nb) != cudaSuccess || cudaMalloc(&dbuf_out, out_per * nb) != cudaSuccess) {
-                    cudaGetLastError();
-                    c->err = "cudaMalloc of staging buffers failed";
-                    rc = MDWF_ENOMEM;
-                    break;
-                }
-            }
-            cudaError_t e = cudaMemcpyAsync(dbuf_in, (const char*)b + in_per * r0, in_per * S.nb, cudaMemcpyHostToDevice, st);
+        }
+    } else {
+        // Host buffers: every batch is staged through device buffers; the copies are part of the call (mdwf.h).
+        // Two buffer sets and a copy stream: the upload of batch k+1 and the download of batch k-1 overlap the
+        // solve of batch k (true overlap needs pinned host memory; pageable memory still gives correct results).
+        void *din[2] = {nullptr, nullptr}, *dout[2] = {nullptr, nullptr};
+        cudaStream_t cs = nullptr;
+        cudaEvent_t up[2] = {nullptr, nullptr}, down[2] = {nullptr, nullptr}, solved = nullptr;
+        const int nbatch = (nrhs + nb - 1) / nb, nset = nbatch > 1 ? 2 : 1;
+        cudaError_t e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
+        for (int k = 0; k < nset && e == cudaSuccess; ++k) {
+            e = cudaMalloc(&din[k], in_per * nb);
+            if (e == cudaSuccess) e = cudaMalloc(&dout[k], out_per * nb);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&up[k], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&down[k], cudaEventDisableTiming);
+        }
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&solved, cudaEventDisableTiming);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            c->err = std::string("staging buffers for host-buffer solve: ") + cudaGetErrorString(e);
+            rc = MDWF_ENOMEM;
+        }
+        auto upload = [&](int k) -> cudaError_t {     // batch k -> din[k % nset] on the copy stream
+            const int r0 = k * nb, n = std::min(nb, nrhs - r0);
+            cudaError_t ee = cudaMemcpyAsync(din[k % nset], (const char*)b + in_per * r0, in_per * n, cudaMemcpyHostToDevice, cs);
+            if (ee == cudaSuccess) ee = cudaEventRecord(up[k % nset], cs);
+            return ee;
+        };
+        if (rc == MDWF_OK && (e = upload(0)) != cudaSuccess) { c->err = cudaGetErrorString(e); rc = MDWF_ECUDA; }
+        for (int k = 0; k < nbatch && rc == MDWF_OK; ++k) {
+            const int r0 = k * nb, set = k % nset;
+            S.nb = std::min(nb, nrhs - r0);
+            e = cudaStreamWaitEvent(st, up[set], 0);                           // batch k is on the device
+            if (e == cudaSuccess && k >= nset) e = cudaStreamWaitEvent(st, down[set], 0);   // dout[set] has been drained
+            // din[(k+1) % nset] was last read by batch k-1, which has completed (solve_batch returns synchronised)
+            if (e == cudaSuccess && k + 1 < nbatch) e = upload(k + 1);
             if (e != cudaSuccess) { c->err = cudaGetErrorString(e); rc = MDWF_ECUDA; break; }
             mdwf_solve_info tmp;
             memset(&tmp, 0, sizeof(tmp));
-            rc = solve_batch(S, (double*)dbuf_out, (const double*)dbuf_in, opts, &tmp, 0, &inner_ms);
+            rc = solve_batch(S, (double*)dout[set], (const double*)din[set], opts, &tmp, 0, &inner_ms);
             if (rc) break;
             for (int i = 0; i < S.nb; ++i) {
                 info->iters[r0 + i] = tmp.iters[i]; info->reliable_updates[r0 + i] = tmp.reliable_updates[i];
                 info->status[r0 + i] = tmp.status[i]; info->true_resid[r0 + i] = tmp.true_resid[i];
             }
-            e = cudaMemcpyAsync((char*)x + out_per * r0, dbuf_out, out_per * S.nb, cudaMemcpyDeviceToHost, st);
-            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+            e = cudaEventRecord(solved, st);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, solved, 0);
+            if (e == cudaSuccess) e = cudaMemcpyAsync((char*)x + out_per * r0, dout[set], out_per * S.nb, cudaMemcpyDeviceToHost, cs);
+            if (e == cudaSuccess) e = cudaEventRecord(down[set], cs);
             if (e != cudaSuccess) { c->err = cudaGetErrorString(e); rc = MDWF_ECUDA; break; }
         }
+        if (cs) {
+            e = cudaStreamSynchronize(cs);
+            if (e != cudaSuccess && rc == MDWF_OK) { c->err = cudaGetErrorString(e); rc = MDWF_ECUDA; }
+        }
+        for (int k = 0; k < 2; ++k) {
+            if (din[k]) cudaFree(din[k]);
+            if (dout[k]) cudaFree(dout[k]);
+            if (up[k]) cudaEventDestroy(up[k]);
+            if (down[k]) cudaEventDestroy(down[k]);
+        }
+        if (solved) cudaEventDestroy(solved);
+        if (cs) cudaStreamDestroy(cs);
     }
-    if (dbuf_in) cudaFree(dbuf_in);
-    if (dbuf_out) cudaFree(dbuf_out);
     cudaEventRecord(e1, st);
     cudaEventSynchronize(e1);
     float ms = 0.f;
