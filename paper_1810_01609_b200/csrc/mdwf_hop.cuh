@@ -186,18 +186,25 @@ __device__ __forceinline__ void apply_ls(T acc[24], const LsOp& op, int Ls, unsi
     __syncthreads();
 }
 
-// fixed-order block sum (shared-memory tree: same order every run -> bit-reproducible); thread 0 stores.
-// smem needed: blockDim.x doubles.  Every thread of the block must call it.
+// fixed-order block sum (same order every run -> bit-reproducible); thread 0 stores.  Two-level: 32 strided
+// partial sums, then one serial pass.  smem needed: blockDim.x doubles.  Every thread of the block must call it.
 __device__ __forceinline__ void block_sum_store(double v, unsigned char* smem_raw, double* dst) {
     double* red = reinterpret_cast<double*>(smem_raw);
     __syncthreads();
     red[threadIdx.x] = v;
     __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
-        if ((int)threadIdx.x < o && (int)threadIdx.x + o < (int)blockDim.x) red[threadIdx.x] += red[threadIdx.x + o];
-        __syncthreads();
+    double a = 0.0;
+    if (threadIdx.x < 32)
+        for (int i = threadIdx.x; i < (int)blockDim.x; i += 32) a += red[i];
+    __syncthreads();
+    if (threadIdx.x < 32) red[threadIdx.x] = a;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tot = 0.0;
+        const int n = blockDim.x < 32 ? (int)blockDim.x : 32;
+        for (int i = 0; i < n; ++i) tot += red[i];
+        *dst = tot;
     }
-    if (threadIdx.x == 0) *dst = red[0];
 }
 
 // ---- links staged in shared memory ------------------------------------------------------------------
@@ -310,6 +317,42 @@ __device__ __forceinline__ SiteCoord decode_site(const Geom& g, int par, uint32_
     return c;
 }
 
+// Fused epilogue shared by hop_kernel and hop_tile_kernel:  out = cx * xin + ch * op(acc), streaming store, optional
+// fixed-order |out|^2 partial.  ch is folded into the s-direction coefficients and, for fp16 storage, the per-site
+// scale of xin into cx, so the xpay costs 24 FMAs.
+template <typename S>
+__device__ __forceinline__ void fused_epilogue(const Geom& g, const HopArgs& a, typename Store<S>::real acc[24], bool live,
+                                               int rhs, int idx, int slot, int tile, unsigned char* smem_epi) {
+    typedef typename Store<S>::real T;
+    if (a.op.kind != 0) {
+        LsOp op = a.op;
+        op.c0 *= a.ch;
+        op.c1 *= a.ch;
+        apply_ls<T>(acc, op, g.Ls, smem_epi);
+    } else {
+        const T ch = (T)a.ch;
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[i] *= ch;
+    }
+    if (a.xin.v != nullptr && live) {
+        T xv[24], sc;
+        load_raw<S>(a.xin, rhs, idx, g.N5h, xv, sc);
+        const T cxs = (T)a.cx * sc;
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[i] = fma_<T>(cxs, xv[i], acc[i]);
+    }
+    if (live) store_spinor<S, MDWF_HOP_STCS>(a.out, rhs, idx, g.N5h, acc);
+    if (a.partial != nullptr) {
+        // the 24 squares of one site are summed in the compute type, everything above in fp64 (PAPER.md:183)
+        T s24 = 0;
+        if (live) {
+#pragma unroll
+            for (int i = 0; i < 24; ++i) s24 = fma_<T>(acc[i], acc[i], s24);
+        }
+        block_sum_store((double)s24, smem_epi, a.partial + (long long)slot * (gridDim.x / a.nact) + tile);
+    }
+}
+
 // Leg l (mu = l>>1, forward for even l) of site c: the link as the stencil multiplies it -- reconstructed from
 // the packed format, daggered for backward legs, times the boundary sign -- as 18 (+2 pad) reals; returns the
 // neighbour's half-index.
@@ -416,32 +459,7 @@ __global__ void __launch_bounds__(256, (sizeof(S) == 8 ? MDWF_HOP_MINB64 : sizeo
         if (live) store_spinor<S, MDWF_HOP_STCS>(a.out, rhs, idx, g.N5h, acc);
         return;
     }
-    // ---- fused epilogue: s-direction matrix, xpay, optional |out|^2 ---------------------------
-    if (a.op.kind != 0) apply_ls<T>(acc, a.op, g.Ls, smem_epi);
-    const T ch = (T)a.ch;
-    if (a.xin.v != nullptr) {
-        if (live) {
-            T xv[24];
-            load_spinor<S>(a.xin, rhs, idx, g.N5h, xv);
-            const T cx = (T)a.cx;
-#pragma unroll
-            for (int i = 0; i < 24; ++i) acc[i] = cx * xv[i] + ch * acc[i];
-        }
-    } else {
-#pragma unroll
-        for (int i = 0; i < 24; ++i) acc[i] *= ch;
-    }
-    if (live) store_spinor<S, MDWF_HOP_STCS>(a.out, rhs, idx, g.N5h, acc);
-    if (a.partial != nullptr) {
-        // the 24 squares of one site are summed in the compute type, everything above in fp64 (PAPER.md:183)
-        T s24 = 0;
-        if (live) {
-#pragma unroll
-            for (int i = 0; i < 24; ++i) s24 = fma_<T>(acc[i], acc[i], s24);
-        }
-        const double s2 = (double)s24;
-        block_sum_store(s2, smem_epi, a.partial + (long long)slot * (gridDim.x / a.nact) + tile);
-    }
+    fused_epilogue<S>(g, a, acc, live, rhs, idx, slot, tile, smem_epi);
 }
 
 }  // namespace mdwf

@@ -169,29 +169,7 @@ hop_tile_kernel(const Geom g, const HopArgs a) {
     // ---- fused epilogue (the staged spinors are dead: their shared memory is reused) ------------------------
     __syncthreads();
     unsigned char* smem_epi = smem_raw;
-    if (a.op.kind != 0) apply_ls<T>(acc, a.op, g.Ls, smem_epi);
-    const T ch = (T)a.ch;
-    if (a.xin.v != nullptr) {
-        if (live) {
-            T xv[24];
-            load_spinor<S>(a.xin, rhs, idx, g.N5h, xv);
-            const T cx = (T)a.cx;
-#pragma unroll
-            for (int i = 0; i < 24; ++i) acc[i] = cx * xv[i] + ch * acc[i];
-        }
-    } else {
-#pragma unroll
-        for (int i = 0; i < 24; ++i) acc[i] *= ch;
-    }
-    if (live) store_spinor<S, MDWF_HOP_STCS>(a.out, rhs, idx, g.N5h, acc);
-    if (a.partial != nullptr) {
-        T s24 = 0;
-        if (live) {
-#pragma unroll
-            for (int i = 0; i < 24; ++i) s24 = fma_<T>(acc[i], acc[i], s24);
-        }
-        block_sum_store((double)s24, smem_epi, a.partial + (long long)slot_r * (gridDim.x / a.nact) + tile);
-    }
+    fused_epilogue<S>(g, a, acc, live, rhs, idx, slot_r, tile, smem_epi);
 }
 
 }  // namespace mdwf
