@@ -142,3 +142,40 @@ def test_edge_cases_zero_rhs_max_batch_and_ls1():
     x1, r1 = c1.mdwf_solve(b1.cuda(), tol=1e-10, inner_prec=32, recon=8, parity=1, symmetric=False)
     assert r1.status == mdwf.OK
     assert oracle.true_residual(p1, U1.numpy(), x1.cpu().numpy(), b1.numpy()).max() <= 1e-10
+
+
+def test_bit_reproducible_and_packed_api_and_profile():
+    """fixed-order reductions: two solves of the same input are bit-identical; the packed-field calls give
+    the same numbers as mdwf_dslash; the hop profiler counts launches and the documented algorithmic bytes."""
+    import paper_1810_01609_b200 as mdwf
+    dims, Ls = (8, 8, 4, 8), 10
+    cfg = synth.CONFIGS[5]
+    U = synth.gauge_field(dims, cfg.eps, 901).cuda()
+    ctx = mdwf.Context(dims, Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
+    ctx.mdwf_load_gauge(U, 64, 18)
+    ctx.mdwf_load_gauge(U, 16, 12)
+    b = synth.gaussian_spinor(dims, Ls, 3, 902).cuda()
+    x1, r1 = ctx.mdwf_solve(b, tol=1e-9, inner_prec=16, recon=12, batch=2)
+    x2, r2 = ctx.mdwf_solve(b, tol=1e-9, inner_prec=16, recon=12, batch=2)
+    assert r1.status == mdwf.OK and r1.iters == r2.iters
+    assert torch.equal(torch.view_as_real(x1), torch.view_as_real(x2))
+    # packed API == canonical API
+    V4 = int(np.prod(dims))
+    half = synth.gaussian_spinor(dims, Ls, 2, 903)[:, :, : V4 // 2].contiguous().cuda()
+    fin, fout = ctx.mdwf_field_create(16, 2), ctx.mdwf_field_create(16, 2)
+    fin.mdwf_field_pack(half)
+    ctx.mdwf_profile(True)
+    ctx.mdwf_dslash_packed(mdwf.OP_DHAT_SYM, fout, fin, parity=1, dagger=True, recon=12)
+    out = torch.empty_like(half)
+    fout.mdwf_field_unpack(out)
+    ms, by, fl, n = ctx.mdwf_profile_read(0)
+    ctx.mdwf_profile(False)
+    ref = ctx.mdwf_dslash(mdwf.OP_DHAT_SYM, half, parity=1, dagger=True, prec=16, recon=12)
+    assert torch.equal(torch.view_as_real(out), torch.view_as_real(ref))
+    n5 = (V4 // 2) * Ls * 2
+    assert n == 2 and ms > 0 and fl == 2 * 1320.0 * n5
+    assert by == (2 + 3) * 52.0 * n5 + 2 * 8 * 12 * 2 * (V4 // 2)      # one plain-input and one xpay-input fused hop
+    cb, cf = ctx.mdwf_dslash_cost(mdwf.OP_HOP, 16, 12, 2)
+    assert cb == 2 * 52.0 * n5 + 8 * 12 * 2 * (V4 // 2) and cf == 1320.0 * n5
+    with pytest.raises(mdwf.MdwfError):
+        ctx.mdwf_dslash_packed(mdwf.OP_HOP, fin, fin, recon=12)          # out must not alias in
