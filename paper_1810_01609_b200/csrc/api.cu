@@ -167,26 +167,33 @@ static void lsop_host(const LsOp& op, int Ls, int chi, const std::vector<double>
     }
 }
 
-// z-slab depth: largest multiple of the tile depth tz dividing Z whose fp32 input slab XH*Y*zc*Ls*96 bytes stays
-// under ~9 MB, so that the three t-consecutive slabs a row of tiles touches (plus the streamed output) live in
-// L2 (measured on B200: 48^3x64 Ls=10 is fastest at zc = 8)
-static int pick_zc(const mdwf_ctx* c, int want) {
+// z-slab depth (per storage precision): largest multiple of the tile depth tz dividing Z whose input slab
+// XH*Y*zc*Ls*(bytes per site) stays under ~9 MB, so that the three t-consecutive slabs a row of tiles touches (plus
+// the streamed output) live in L2 (measured on B200, 48^3x64 Ls=10: fp32 fastest at zc = 8,
+// fp64 at zc = 4, fp16 flat between 2 and 16)
+static int pick_zc(const mdwf_ctx* c, int want, double site_bytes) {
     const Geom& g = c->g;
-    const int lz = g.q4nsite > 0 ? g.q4L[2] : 1;
+    const int lz = (c->use_tiled && g.q4nsite > 0) ? g.q4L[2] : 1;   // only the opt-in tile kernel constrains zc
     if (want > 0 && g.Z % want == 0 && want % g.tz == 0 && want % lz == 0) return want;
     int best = 0;
     for (int z = g.tz; z <= g.Z; z += g.tz)
-        if (g.Z % z == 0 && z % lz == 0 && (best == 0 || (double)g.XH * g.Y * z * g.Ls * 96.0 <= 9.0e6)) best = z;
+        if (g.Z % z == 0 && z % lz == 0 && (best == 0 || (double)g.XH * g.Y * z * g.Ls * site_bytes <= 9.0e6)) best = z;
     return best;
 }
-static void set_zc(mdwf_ctx* c, int zc) {
-    Geom& g = c->g;
-    g.zc = zc;
-    g.dZc = make_fastdiv(zc);
-    g.dSlab = make_fastdiv((uint32_t)(g.XH * g.Y * zc));
-    g.dTslab = make_fastdiv((uint32_t)(g.XH * g.Y * zc) * (uint32_t)g.T);
-    g.dnTzs = make_fastdiv((uint32_t)(zc / g.tz));
-    g.q4dTzs = make_fastdiv((uint32_t)(zc / (g.q4nsite > 0 ? g.q4L[2] : 1)));
+static void set_zc(mdwf_ctx* c, int want) {
+    const double site_bytes[3] = {52.0, 96.0, 192.0};
+    for (int cls = 0; cls < 3; ++cls) {
+        Geom g = c->g;
+        const int zc = pick_zc(c, want, site_bytes[cls]);
+        g.zc = zc;
+        g.dZc = make_fastdiv(zc);
+        g.dSlab = make_fastdiv((uint32_t)(g.XH * g.Y * zc));
+        g.dTslab = make_fastdiv((uint32_t)(g.XH * g.Y * zc) * (uint32_t)g.T);
+        g.dnTzs = make_fastdiv((uint32_t)(zc / g.tz));
+        g.q4dTzs = make_fastdiv((uint32_t)std::max(1, zc / (g.q4nsite > 0 ? g.q4L[2] : 1)));
+        c->ghop[cls] = g;
+        if (cls == 1) c->g = g;
+    }
 }
 // Sites of a block: a box txh*ty*tz*tt (x fastest) that divides the lattice, filled greedily along x, then y, z, t
 // up to min(256/Ls, 32) sites, i.e. (nearly) whole x-rows in storage order.  Compact 4D boxes (e.g. 4x4x2x2) were
@@ -272,7 +279,7 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
         if (rc4) return rc4;
     }
     c->use_tiled = getenv("MDWF_HOP_TILED") ? atoi(getenv("MDWF_HOP_TILED")) : 0;
-    set_zc(c, pick_zc(c, 0));
+    set_zc(c, 0);
     MDWF_CUDA(c, cudaMalloc(&c->partial, sizeof(double) * 64 * (size_t)c->nblk));
     MDWF_CUDA(c, cudaMalloc(&c->dscal, sizeof(double) * 8 * 64));
     MDWF_CUDA(c, cudaMemset(c->dscal, 0, sizeof(double) * 8 * 64));
@@ -361,8 +368,8 @@ int mdwf_set_tiling(mdwf_ctx* c, int zc) {
     if (!c) return MDWF_EINVAL;
     if (zc < 0 || (zc > 0 && (c->g.Z % zc != 0 || zc % c->g.tz != 0)))
         MDWF_FAIL(c, MDWF_EINVAL, "zc = %d must divide Z = %d and be a multiple of the tile depth %d", zc, c->g.Z, c->g.tz);
-    if (zc > 0 && c->g.q4nsite > 0 && zc % c->g.q4L[2] != 0) MDWF_FAIL(c, MDWF_EINVAL, "zc = %d must be a multiple of the 4D tile depth %d", zc, c->g.q4L[2]);
-    set_zc(c, pick_zc(c, zc));
+    if (zc > 0 && c->use_tiled && c->g.q4nsite > 0 && zc % c->g.q4L[2] != 0) MDWF_FAIL(c, MDWF_EINVAL, "zc = %d must be a multiple of the 4D tile depth %d", zc, c->g.q4L[2]);
+    set_zc(c, zc);
     return MDWF_OK;
 }
 

@@ -31,6 +31,7 @@ struct mdwf_ctx {
     mdwf_geometry geo;
     double M5, b5, c5, mf;
     mdwf::Geom g;
+    mdwf::Geom ghop[3];        // the same with the hop traversal's z-slab depth for fp16 / fp32 / fp64 storage
     int block;                 // threads per block: a multiple of Ls, <= 256
     int nblk;                  // blocks per rhs = ceil(N5h / block)
     std::vector<GaugeSet> gauges;

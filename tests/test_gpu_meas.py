@@ -105,3 +105,45 @@ def test_fh_chain_small():
     c0o = oracle.nucleon_2pt(dims, So, So, So, P)
     cfho = (oracle.nucleon_2pt(dims, SFHo, So, So, P) + oracle.nucleon_2pt(dims, So, So, SFHo, P) - oracle.nucleon_2pt(dims, So, SFHo, So, P))
     assert rel(c0, c0o) <= 1e-5 and rel(cfh, cfho) <= 1e-5
+
+
+def test_static_limit_matches_golden_file():
+    import os
+    import paper_1810_01609_b200 as mdwf
+    vals = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "static_nucleon.txt")) as f:
+        for line in f:
+            if not line.startswith("#") and line.strip():
+                k, v = line.split()
+                vals[k] = float(v)
+    dims = (2, 2, 4, 2)
+    ctx = mdwf.Context(dims, 2, 1.3, 1.5, 0.5, 0.1)
+    V4 = int(np.prod(dims))
+    gt = oracle.gamma(3)
+    Pp, Pm = 0.5 * (np.eye(4) + gt), 0.5 * (np.eye(4) - gt)
+    S = np.zeros((12, V4, 4, 3), dtype=np.complex128)
+    for be in range(4):
+        for b in range(3):
+            for al in range(4):
+                S[3 * be + b, :, al, b] = Pp[al, be]
+    Sd = torch.from_numpy(S).cuda()
+    V3 = V4 // dims[3]
+    assert np.allclose(ctx.mdwf_nucleon_2pt(Sd, Sd, Sd, Pp).cpu().numpy(), vals["(1+gamma_t)/2"] * V3, atol=1e-10)
+    assert np.allclose(ctx.mdwf_nucleon_2pt(Sd, Sd, Sd, Pm).cpu().numpy(), vals["(1-gamma_t)/2"] * V3, atol=1e-10)
+
+
+@pytest.mark.parametrize("prec,tol", [(64, 0.0), (32, 1e-7), (16, 6e-4)])
+def test_pack_unpack_round_trip(prec, tol):
+    """layout round trip: canonical -> packed -> canonical; exact in fp64, storage rounding otherwise.
+    Ragged shape: N5h = 3*5*... not a multiple of the 32-site storage block."""
+    import paper_1810_01609_b200 as mdwf
+    dims, Ls = (6, 2, 2, 4), 5
+    ctx = mdwf.Context(dims, Ls, 1.3, 1.5, 0.5, 0.1)
+    Vh = int(np.prod(dims)) // 2
+    src = crandn((3, Ls, Vh, 4, 3), 4300).cuda()
+    f = ctx.mdwf_field_create(prec, 3)
+    f.mdwf_field_pack(src)
+    out = torch.zeros_like(src)
+    f.mdwf_field_unpack(out)
+    err = float((out - src).abs().max() / src.abs().max())
+    assert err <= tol, err
