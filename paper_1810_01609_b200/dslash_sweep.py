@@ -23,6 +23,44 @@ OPS = {"hop": mdwf.OP_HOP, "mhat": mdwf.OP_DHAT_SYM, "dhat": mdwf.OP_DHAT_ASYM, 
        "normal": mdwf.OP_NORMAL_SYM}
 
 
+def measurement_kernels(ctx, cfg, iters, peak):
+    """Feynman-Hellmann sequential source and nucleon two-point contraction on random 12-column 4D propagators
+    (SURVEY a10, a11): device time, algorithmic GB/s (seq source: read + write one propagator; contraction: read
+    three), and GFLOP/s of the contraction at ~2.0e4 flop per site."""
+    import numpy as np
+    g = torch.Generator(device="cuda").manual_seed(synth.seed_for(cfg.index, 9))
+    props = []
+    for _ in range(3):
+        S = torch.empty((12, cfg.V4, 4, 3), dtype=torch.complex128, device="cuda")
+        torch.view_as_real(S).normal_(0.0, 1.0, generator=g)
+        props.append(S)
+    out = torch.empty_like(props[0])
+    G = np.zeros((4, 4), dtype=np.complex128)
+    G[0, 2], G[1, 3], G[2, 0], G[3, 1] = 1j, -1j, 1j, -1j          # a signed permutation like gamma_z gamma_5
+    P = np.diag([1.0, 1.0, 0.0, 0.0]).astype(np.complex128)
+    pbytes = props[0].numel() * 16
+
+    def timed(fn):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(iters):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / iters
+
+    ms = timed(lambda: ctx.mdwf_seq_source(props[0], G, out=out))
+    print(json.dumps({"workload": cfg.name, "op": "seq_source", "ms": round(ms, 4), "GBps": round(2 * pbytes / ms / 1e6, 1),
+                      "frac_of_measured_hbm": round(2 * pbytes / ms / 1e6 / peak, 4)}), flush=True)
+    ms = timed(lambda: ctx.mdwf_nucleon_2pt(props[0], props[1], props[2], P))
+    print(json.dumps({"workload": cfg.name, "op": "nucleon_2pt", "ms": round(ms, 4), "GBps": round(3 * pbytes / ms / 1e6, 1),
+                      "GFLOPs": round(2.0e4 * cfg.V4 / ms / 1e6, 1),
+                      "frac_of_measured_hbm": round(3 * pbytes / ms / 1e6 / peak, 4)}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", type=int, default=2)
@@ -33,6 +71,7 @@ def main():
     ap.add_argument("--rotate", type=int, default=4)
     ap.add_argument("--zc", type=int, default=0)
     ap.add_argument("--dagger", type=int, default=0)
+    ap.add_argument("--meas", action="store_true", help="time the sequential-source and nucleon 2-pt kernels instead")
     a = ap.parse_args()
     cfg = synth.CONFIGS[a.config]
     peak = 6650.0
@@ -41,6 +80,9 @@ def main():
         peak = float(json.load(open(pk))["hbm_gbs"])
     ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
     ctx.mdwf_set_tiling(a.zc)
+    if a.meas:
+        measurement_kernels(ctx, cfg, a.iters, peak)
+        return
     U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(cfg.index, 1), device="cuda")
     fmts = [tuple(int(v) for v in f.split("x")) for f in a.formats.split(",")]
     for prec, recon in fmts:
