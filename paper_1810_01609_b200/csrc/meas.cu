@@ -108,7 +108,7 @@ __global__ void __launch_bounds__(256) seq_source_kernel(const SeqArgs a) {
 // Nucleon 2-pt (SURVEY O4 C-def), in the trace form
 //   C(t) = sum_x eps_{abc} eps_{a'b'c'} { tr[Q^{bb'} (Su1^{aa'})^T] tr[P Su2^{cc'}] - tr[(Q^{bb'})^T Su1^{ac'} P Su2^{ca'}] },
 //   Q^{bb'} = G Sd^{bb'} Gt,  G = C gamma5,  Gt = gamma_t G^dag gamma_t,  S^{ab}_{al be}(x) = S[3 be + b][x][al][a].
-// One block of 144 threads per site batch; thread = (colour-permutation pair e1,e2 ; spin index al').
+// One warp per site; the 144 work items (colour-permutation pair e1,e2 ; spin index al') are spread over the lanes.
 struct NucArgs {
     const double2 *Su1, *Sd, *Su2;
     double* partial;       // [T][nblk_t][2]
@@ -122,28 +122,32 @@ __device__ __forceinline__ double2 cfma(double2 a, double2 b, double2 c) {
     return make_double2(c.x + a.x * b.x - a.y * b.y, c.y + a.x * b.y + a.y * b.x);
 }
 
-__global__ void __launch_bounds__(144) nucleon_kernel(const NucArgs a) {
+#define MDWF_NUC_WARPS 4
+__constant__ int c_perm[6][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}, {0, 2, 1}, {2, 1, 0}, {1, 0, 2}};
+__constant__ double c_psign[6] = {1, 1, 1, -1, -1, -1};
+__global__ void __launch_bounds__(32 * MDWF_NUC_WARPS) nucleon_kernel(const NucArgs a) {
+    // One warp per site (only warp-level barriers); 144 work items per phase are spread over the 32 lanes.
     // prop element (sink spin al, sink colour ca, source spin be, source colour cb) at S[(3*be+cb)*12 + 3*al+ca]
-    __shared__ double2 s1[144], sd[144], s2[144], Q[144], W[144], trP[9];
-    __shared__ double redr[144], redi[144];
-    const int tid = threadIdx.x;
+    extern __shared__ __align__(16) unsigned char nuc_smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double2* base = reinterpret_cast<double2*>(nuc_smem) + warp * (5 * 144 + 16);
+    double2 *s1 = base, *sd = base + 144, *s2 = base + 288, *Q = base + 432, *W = base + 576, *trP = base + 720;
     const int t = blockIdx.y;
-    const int perm[6][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}, {0, 2, 1}, {2, 1, 0}, {1, 0, 2}};
-    const double psign[6] = {1, 1, 1, -1, -1, -1};
     double accr = 0.0, acci = 0.0;
-    for (long long xs = blockIdx.x; xs < a.V3; xs += a.nblk_t) {
+    const int wid = blockIdx.x * MDWF_NUC_WARPS + warp, nw = a.nblk_t * MDWF_NUC_WARPS;
+    for (long long xs = wid; xs < a.V3; xs += nw) {
         const long long x = (long long)t * a.V3 + xs;
-        {
-            const int col = tid / 12, k = tid % 12;
+        for (int i = lane; i < 144; i += 32) {
+            const int col = i / 12, k = i - col * 12;
             const long long off = ((long long)col * a.V4 + x) * 12 + k;
-            s1[tid] = a.Su1[off];
-            sd[tid] = a.Sd[off];
-            s2[tid] = a.Su2[off];
+            s1[i] = __ldg(a.Su1 + off);
+            sd[i] = __ldg(a.Sd + off);
+            s2[i] = __ldg(a.Su2 + off);
         }
-        __syncthreads();
-        {
-            // thread -> (b, b', al, al'):  Q^{bb'}_{al al'} = sum_{be,be'} G[al][be] Sd^{bb'}_{be be'} Gt[be'][al']
-            const int b = tid / 48, bp = (tid / 16) % 3, al = (tid / 4) % 4, alp = tid % 4;
+        __syncwarp();
+        for (int e = lane; e < 144; e += 32) {
+            // e -> (b, b', al, al'):  Q^{bb'}_{al al'} = sum_{be,be'} G[al][be] Sd^{bb'}_{be be'} Gt[be'][al']
+            const int b = e / 48, bp = (e / 16) % 3, al = (e / 4) % 4, alp = e % 4;
             double2 q = make_double2(0.0, 0.0);
 #pragma unroll
             for (int be = 0; be < 4; ++be) {
@@ -152,34 +156,36 @@ __global__ void __launch_bounds__(144) nucleon_kernel(const NucArgs a) {
 #pragma unroll
                 for (int bep = 0; bep < 4; ++bep) {
                     const double2 g2 = make_double2(a.Gt[2 * (4 * bep + alp)], a.Gt[2 * (4 * bep + alp) + 1]);
+                    if (g2.x == 0.0 && g2.y == 0.0) continue;
                     q = cfma(cmul(g1, g2), sd[(3 * bep + bp) * 12 + 3 * be + b], q);
                 }
             }
-            Q[tid] = q;     // index ((b*3+bp)*4+al)*4+alp
+            Q[e] = q;     // index ((b*3+bp)*4+al)*4+alp
             // W^{c a'}_{ga' al'} = sum_ga P[ga'][ga] Su2^{c a'}_{ga al'}   (same index pattern: c, a', ga', al')
             double2 w = make_double2(0.0, 0.0);
 #pragma unroll
             for (int ga = 0; ga < 4; ++ga) {
                 const double2 pp = make_double2(a.P[2 * (4 * al + ga)], a.P[2 * (4 * al + ga) + 1]);
+                if (pp.x == 0.0 && pp.y == 0.0) continue;
                 w = cfma(pp, s2[(3 * alp + bp) * 12 + 3 * ga + b], w);
             }
-            W[tid] = w;     // index ((c*3+a')*4+ga')*4+al'
-            if (tid < 9) {
-                const int c = tid / 3, cp = tid % 3;
-                double2 tr = make_double2(0.0, 0.0);
-                for (int gap = 0; gap < 4; ++gap)
-                    for (int ga = 0; ga < 4; ++ga)
-                        tr = cfma(make_double2(a.P[2 * (4 * gap + ga)], a.P[2 * (4 * gap + ga) + 1]),
-                                  s2[(3 * gap + cp) * 12 + 3 * ga + c], tr);
-                trP[tid] = tr;
-            }
+            W[e] = w;     // index ((c*3+a')*4+ga')*4+al'
         }
-        __syncthreads();
-        {
-            const int e = tid / 4, alp = tid % 4, e1 = e / 6, e2 = e % 6;
-            const int ca = perm[e1][0], cb = perm[e1][1], cc = perm[e1][2];
-            const int cap = perm[e2][0], cbp = perm[e2][1], ccp = perm[e2][2];
-            const double sg = psign[e1] * psign[e2];
+        if (lane < 9) {
+            const int c = lane / 3, cp = lane % 3;
+            double2 tr = make_double2(0.0, 0.0);
+            for (int gap = 0; gap < 4; ++gap)
+                for (int ga = 0; ga < 4; ++ga)
+                    tr = cfma(make_double2(a.P[2 * (4 * gap + ga)], a.P[2 * (4 * gap + ga) + 1]),
+                              s2[(3 * gap + cp) * 12 + 3 * ga + c], tr);
+            trP[lane] = tr;
+        }
+        __syncwarp();
+        for (int wi = lane; wi < 144; wi += 32) {
+            const int e = wi / 4, alp = wi % 4, e1 = e / 6, e2 = e % 6;
+            const int ca = c_perm[e1][0], cb = c_perm[e1][1], cc = c_perm[e1][2];
+            const int cap = c_perm[e2][0], cbp = c_perm[e2][1], ccp = c_perm[e2][2];
+            const double sg = c_psign[e1] * c_psign[e2];
             const double2* q = Q + (cb * 3 + cbp) * 16;
             // direct: sum_al Q_{al al'} Su1^{aa'}_{al al'}  * tr[P Su2^{cc'}]
             double2 d = make_double2(0.0, 0.0);
@@ -199,16 +205,17 @@ __global__ void __launch_bounds__(144) nucleon_kernel(const NucArgs a) {
             accr += sg * (d.x - ex.x);
             acci += sg * (d.y - ex.y);
         }
-        __syncthreads();
+        __syncwarp();
     }
-    redr[tid] = accr;
-    redi[tid] = acci;
-    __syncthreads();
-    if (tid == 0) {
-        double sr = 0.0, si = 0.0;
-        for (int i = 0; i < 144; ++i) { sr += redr[i]; si += redi[i]; }
-        a.partial[((long long)t * a.nblk_t + blockIdx.x) * 2] = sr;
-        a.partial[((long long)t * a.nblk_t + blockIdx.x) * 2 + 1] = si;
+    // fixed-order warp sum, one partial per warp
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        accr += __shfl_down_sync(0xffffffffu, accr, o);
+        acci += __shfl_down_sync(0xffffffffu, acci, o);
+    }
+    if (lane == 0) {
+        a.partial[((long long)t * nw + wid) * 2] = accr;
+        a.partial[((long long)t * nw + wid) * 2 + 1] = acci;
     }
 }
 
@@ -303,7 +310,7 @@ int mdwf_nucleon_2pt(mdwf_ctx* c, double* corr, const void* S_u1, const void* S_
     a.Su1 = (const double2*)S_u1; a.Sd = (const double2*)S_d; a.Su2 = (const double2*)S_u2;
     a.V4 = 2ll * c->g.Vh; a.V3 = a.V4 / c->g.T;
     const int T = c->g.T;
-    a.nblk_t = (int)std::min<long long>(a.V3, std::max(1, (c->sm_count * 8) / T));
+    a.nblk_t = (int)std::min<long long>((a.V3 + MDWF_NUC_WARPS - 1) / MDWF_NUC_WARPS, std::max(1, (c->sm_count * 16) / T));
     // C = gamma_y gamma_t, G = C gamma5, Gt = gamma_t G^dag gamma_t in the DeGrand-Rossi basis (SURVEY 8 Notation)
     const double gy[32] = {0,0, 0,0, 0,0, -1,0,   0,0, 0,0, 1,0, 0,0,   0,0, 1,0, 0,0, 0,0,   -1,0, 0,0, 0,0, 0,0};
     const double gt[32] = {0,0, 0,0, 1,0, 0,0,   0,0, 0,0, 0,0, 1,0,   1,0, 0,0, 0,0, 0,0,   0,0, 1,0, 0,0, 0,0};
@@ -319,12 +326,16 @@ int mdwf_nucleon_2pt(mdwf_ctx* c, double* corr, const void* S_u1, const void* S_
     memcpy(a.Gt, Gt, sizeof(Gt));
     memcpy(a.P, proj_host, sizeof(a.P));
     double* partial = nullptr;
-    MDWF_CUDA(c, cudaMallocAsync(&partial, sizeof(double) * 2 * T * a.nblk_t, st));
+    const int npart = a.nblk_t * MDWF_NUC_WARPS;
+    MDWF_CUDA(c, cudaMallocAsync(&partial, sizeof(double) * 2 * T * npart, st));
     a.partial = partial;
     dim3 grid(a.nblk_t, T);
-    nucleon_kernel<<<grid, 144, 0, st>>>(a);
+    const size_t nsm = (size_t)MDWF_NUC_WARPS * (5 * 144 + 16) * sizeof(double2);
+    static bool raised = false;
+    if (!raised) { MDWF_CUDA(c, cudaFuncSetAttribute(nucleon_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nsm)); raised = true; }
+    nucleon_kernel<<<grid, 32 * MDWF_NUC_WARPS, nsm, st>>>(a);
     MDWF_CUDA(c, cudaGetLastError());
-    nucleon_finish_kernel<<<(T + 63) / 64, 64, 0, st>>>(corr, partial, a.nblk_t, T, t0);
+    nucleon_finish_kernel<<<(T + 63) / 64, 64, 0, st>>>(corr, partial, npart, T, t0);
     MDWF_CUDA(c, cudaGetLastError());
     MDWF_CUDA(c, cudaFreeAsync(partial, st));
     c->launches += 2;
