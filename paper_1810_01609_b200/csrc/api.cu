@@ -171,8 +171,7 @@ static void lsop_host(const LsOp& op, int Ls, int chi, const std::vector<double>
 // XH*Y*zc*Ls*(bytes per site) stays under ~9 MB, so that the three t-consecutive slabs a row of tiles touches (plus
 // the streamed output) live in L2 (measured on B200, 48^3x64 Ls=10: fp32 fastest at zc = 8,
 // fp64 at zc = 4, fp16 flat between 2 and 16)
-static int pick_zc(const mdwf_ctx* c, int want, double site_bytes) {
-    const Geom& g = c->g;
+static int pick_zc(const mdwf_ctx* c, const Geom& g, int want, double site_bytes) {
     const int lz = (c->use_tiled && g.q4nsite > 0) ? g.q4L[2] : 1;   // only the opt-in tile kernel constrains zc
     if (want > 0 && g.Z % want == 0 && want % g.tz == 0 && want % lz == 0) return want;
     int best = 0;
@@ -183,25 +182,25 @@ static int pick_zc(const mdwf_ctx* c, int want, double site_bytes) {
 static void set_zc(mdwf_ctx* c, int want) {
     const double site_bytes[3] = {52.0, 96.0, 192.0};
     for (int cls = 0; cls < 3; ++cls) {
-        Geom g = c->g;
-        const int zc = pick_zc(c, want, site_bytes[cls]);
+        Geom& g = c->ghop[cls];
+        const int zc = pick_zc(c, g, want, site_bytes[cls]);
         g.zc = zc;
         g.dZc = make_fastdiv(zc);
         g.dSlab = make_fastdiv((uint32_t)(g.XH * g.Y * zc));
         g.dTslab = make_fastdiv((uint32_t)(g.XH * g.Y * zc) * (uint32_t)g.T);
         g.dnTzs = make_fastdiv((uint32_t)(zc / g.tz));
         g.q4dTzs = make_fastdiv((uint32_t)std::max(1, zc / (g.q4nsite > 0 ? g.q4L[2] : 1)));
-        c->ghop[cls] = g;
-        if (cls == 1) c->g = g;
     }
+    c->g = c->ghop[1];
 }
 // Sites of a block: a box txh*ty*tz*tt (x fastest) that divides the lattice, filled greedily along x, then y, z, t
-// up to min(256/Ls, 32) sites, i.e. (nearly) whole x-rows in storage order.  Compact 4D boxes (e.g. 4x4x2x2) were
-// measured SLOWER on B200 (profiles/README.md, "tile shape"): L1 does not keep the in-box neighbours long enough to
-// merge their eight uses, so the L2->SM traffic does not drop, while coalescing gets worse.
-static void pick_tile(mdwf_ctx* c, int) {
-    Geom& g = c->g;
-    const int cap = std::max(1, std::min(256 / g.Ls, 32));
+// up to `cap` sites, i.e. (nearly) whole x-rows in storage order.  Compact 4D boxes (e.g. 4x4x2x2) were measured
+// SLOWER on B200 (profiles/README.md, "tile shape").  cap: min(256/Ls, 32) sites for fp32/fp64 storage, min(128/Ls, 32)
+// for fp16 -- the issue-bound fp16 kernels stall less at their block barriers with ~128-thread blocks (measured
+// -5..7 % on the fused kernels), while fp32 prefers the larger ones.
+static void pick_tile(Geom& g, int cap) {
+    if (getenv("MDWF_MAX_SITES")) cap = std::min(cap, atoi(getenv("MDWF_MAX_SITES")));   // experiments
+    cap = std::max(1, cap);
     int best[4] = {1, 1, 1, 1};
     const int ext[4] = {g.XH, g.Y, g.Z, g.T};
     int n = 1;
@@ -217,8 +216,6 @@ static void pick_tile(mdwf_ctx* c, int) {
     g.nsite = g.txh * g.ty * g.tz * g.tt;
     g.dtxh = make_fastdiv(g.txh); g.dty = make_fastdiv(g.ty); g.dtz = make_fastdiv(g.tz);
     g.dnTx = make_fastdiv(g.XH / g.txh); g.dnTy = make_fastdiv(g.Y / g.ty); g.dnTt = make_fastdiv(g.T / g.tt);
-    c->block = g.nsite * g.Ls;
-    c->nblk = g.Vh / g.nsite;
 }
 
 static void prof_drain(mdwf_ctx* c) {
@@ -273,14 +270,24 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     g.N5h = g.Vh * g.Ls;
     for (int m = 0; m < 4; ++m) g.bc[m] = geo->bc[m];
     g.dLs = make_fastdiv(g.Ls); g.dXH = make_fastdiv(g.XH); g.dY = make_fastdiv(g.Y); g.dZ = make_fastdiv(g.Z);
-    pick_tile(c, 0);
+    pick_tile(g, std::min(256 / g.Ls, 32));
     {
-        const int rc4 = setup_tile4(c);
+        const int rc4 = setup_tile4(c);      // the (opt-in) 4D tiles follow the fp32 blocking
         if (rc4) return rc4;
     }
     c->use_tiled = getenv("MDWF_HOP_TILED") ? atoi(getenv("MDWF_HOP_TILED")) : 0;
+    int max_nblk = 0;
+    for (int cls = 0; cls < 3; ++cls) {
+        c->ghop[cls] = g;
+        if (cls == 0) pick_tile(c->ghop[cls], std::min(128 / g.Ls, 32));
+        c->blk_cls[cls] = c->ghop[cls].nsite * g.Ls;
+        c->nblk_cls[cls] = g.Vh / c->ghop[cls].nsite;
+        max_nblk = std::max(max_nblk, c->nblk_cls[cls]);
+    }
+    c->block = c->blk_cls[1];
+    c->nblk = c->nblk_cls[1];
     set_zc(c, 0);
-    MDWF_CUDA(c, cudaMalloc(&c->partial, sizeof(double) * 64 * (size_t)c->nblk));
+    MDWF_CUDA(c, cudaMalloc(&c->partial, sizeof(double) * 64 * (size_t)max_nblk));
     MDWF_CUDA(c, cudaMalloc(&c->dscal, sizeof(double) * 8 * 64));
     MDWF_CUDA(c, cudaMemset(c->dscal, 0, sizeof(double) * 8 * 64));
     MDWF_CUDA(c, cudaHostAlloc(&c->hscal, sizeof(double) * 8 * 64, cudaHostAllocDefault));
@@ -366,7 +373,7 @@ int mdwf_selftest_host(double M5, double b5, double c5, double mf) {
 
 int mdwf_set_tiling(mdwf_ctx* c, int zc) {
     if (!c) return MDWF_EINVAL;
-    if (zc < 0 || (zc > 0 && (c->g.Z % zc != 0 || zc % c->g.tz != 0)))
+    if (zc < 0 || (zc > 0 && (c->g.Z % zc != 0 || zc % c->ghop[0].tz != 0 || zc % c->ghop[1].tz != 0)))
         MDWF_FAIL(c, MDWF_EINVAL, "zc = %d must divide Z = %d and be a multiple of the tile depth %d", zc, c->g.Z, c->g.tz);
     if (zc > 0 && c->use_tiled && c->g.q4nsite > 0 && zc % c->g.q4L[2] != 0) MDWF_FAIL(c, MDWF_EINVAL, "zc = %d must be a multiple of the 4D tile depth %d", zc, c->g.q4L[2]);
     set_zc(c, zc);

@@ -48,21 +48,21 @@ int temp_field(mdwf_ctx* c, int prec, int nrhs, int slot, mdwf_field** out) {
     return MDWF_OK;
 }
 
-#define LAUNCH(kern, grid, smem, ...)                                   \
+#define LAUNCH(kern, grid, blk, smem, ...)                              \
     do {                                                                \
-        kern<<<(grid), c->block, (smem), st>>>(__VA_ARGS__);            \
+        kern<<<(grid), (blk), (smem), st>>>(__VA_ARGS__);               \
         MDWF_CUDA(c, cudaGetLastError());                               \
         c->launches++;                                                  \
     } while (0)
 
 template <typename K, typename A>
-static int launch_big_smem(mdwf_ctx* c, K kern, int grid, size_t smem, cudaStream_t st, const A& a) {
+static int launch_big_smem(mdwf_ctx* c, K kern, int grid, int blk, size_t smem, cudaStream_t st, const A& a) {
     static std::set<const void*> raised;
     if (smem > 48 * 1024 && !raised.count((const void*)kern)) {
         MDWF_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         raised.insert((const void*)kern);
     }
-    kern<<<grid, c->block, smem, st>>>(c->g, a);
+    kern<<<grid, blk, smem, st>>>(c->g, a);
     MDWF_CUDA(c, cudaGetLastError());
     c->launches++;
     return MDWF_OK;
@@ -70,17 +70,18 @@ static int launch_big_smem(mdwf_ctx* c, K kern, int grid, size_t smem, cudaStrea
 
 template <typename S> static size_t g_smem(mdwf_ctx* c, bool useG) {
     typedef typename Store<S>::real T;
-    size_t smem = (size_t)c->block * sizeof(double);
-    if (useG) smem = std::max(smem, (size_t)smem_reals_G<T>(c->g.Ls, c->block) * sizeof(T));
+    const int blk = c->blk_cls[sizeof(S) == 2 ? 0 : sizeof(S) == 4 ? 1 : 2];
+    size_t smem = (size_t)blk * sizeof(double);
+    if (useG) smem = std::max(smem, (size_t)smem_reals_G<T>(c->g.Ls, blk) * sizeof(T));
     return smem;
 }
 
 int launch_ls(mdwf_ctx* c, int prec, LsArgs& a, cudaStream_t st) {
-    const int grid = c->nblk * a.rl.nact;
+    const int grid = c->nblk_cls[cls_of(prec)] * a.rl.nact, blk = c->blk_cls[cls_of(prec)];
     switch (prec) {
-        case 64: return launch_big_smem(c, ls_kernel<double>, grid, g_smem<double>(c, a.op.kind != 0), st, a);
-        case 32: return launch_big_smem(c, ls_kernel<float>, grid, g_smem<float>(c, a.op.kind != 0), st, a);
-        case 16: return launch_big_smem(c, ls_kernel<__half>, grid, g_smem<__half>(c, a.op.kind != 0), st, a);
+        case 64: return launch_big_smem(c, ls_kernel<double>, grid, blk, g_smem<double>(c, a.op.kind != 0), st, a);
+        case 32: return launch_big_smem(c, ls_kernel<float>, grid, blk, g_smem<float>(c, a.op.kind != 0), st, a);
+        case 16: return launch_big_smem(c, ls_kernel<__half>, grid, blk, g_smem<__half>(c, a.op.kind != 0), st, a);
     }
     MDWF_FAIL(c, MDWF_EINVAL, "bad precision %d", prec);
 }
@@ -116,12 +117,13 @@ int launch_hop(mdwf_ctx* c, int prec, int recon, int dagger, int fused, HopArgs&
 
 template <typename SO, typename SA>
 static int axpby_b(mdwf_ctx* c, int pb, AxpbyArgs& a, cudaStream_t st) {
-    const int grid = c->nblk * a.rl.nact;
-    const size_t smem = (size_t)c->block * sizeof(double);
+    const int cls = sizeof(SO) == 2 ? 0 : sizeof(SO) == 4 ? 1 : 2;      // blocked like the output's storage class
+    const int grid = c->nblk_cls[cls] * a.rl.nact, blk = c->blk_cls[cls];
+    const size_t smem = (size_t)blk * sizeof(double);
     switch (pb) {
-        case 64: LAUNCH((axpby_kernel<SO, SA, double>), grid, smem, c->g, a); return MDWF_OK;
-        case 32: LAUNCH((axpby_kernel<SO, SA, float>), grid, smem, c->g, a); return MDWF_OK;
-        case 16: LAUNCH((axpby_kernel<SO, SA, __half>), grid, smem, c->g, a); return MDWF_OK;
+        case 64: LAUNCH((axpby_kernel<SO, SA, double>), grid, blk, smem, c->g, a); return MDWF_OK;
+        case 32: LAUNCH((axpby_kernel<SO, SA, float>), grid, blk, smem, c->g, a); return MDWF_OK;
+        case 16: LAUNCH((axpby_kernel<SO, SA, __half>), grid, blk, smem, c->g, a); return MDWF_OK;
     }
     MDWF_FAIL(c, MDWF_EINVAL, "bad precision %d", pb);
 }
@@ -144,29 +146,29 @@ int launch_axpby(mdwf_ctx* c, int po, int pa, int pb, AxpbyArgs& a, cudaStream_t
 }
 
 int launch_cg_xr(mdwf_ctx* c, int prec_x, int prec, CgXrArgs& a, cudaStream_t st) {
-    const int grid = c->nblk * a.rl.nact;
-    const size_t smem = (size_t)c->block * sizeof(double);
-    if (prec == 64 && prec_x == 64) { LAUNCH((cg_update_xr_kernel<double, double>), grid, smem, c->g, a); return MDWF_OK; }
-    if (prec == 32 && prec_x == 32) { LAUNCH((cg_update_xr_kernel<float, float>), grid, smem, c->g, a); return MDWF_OK; }
-    if (prec == 16 && prec_x == 32) { LAUNCH((cg_update_xr_kernel<float, __half>), grid, smem, c->g, a); return MDWF_OK; }
-    if (prec == 16 && prec_x == 16) { LAUNCH((cg_update_xr_kernel<__half, __half>), grid, smem, c->g, a); return MDWF_OK; }
+    const int grid = c->nblk_cls[cls_of(prec)] * a.rl.nact, blk = c->blk_cls[cls_of(prec)];
+    const size_t smem = (size_t)blk * sizeof(double);
+    if (prec == 64 && prec_x == 64) { LAUNCH((cg_update_xr_kernel<double, double>), grid, blk, smem, c->g, a); return MDWF_OK; }
+    if (prec == 32 && prec_x == 32) { LAUNCH((cg_update_xr_kernel<float, float>), grid, blk, smem, c->g, a); return MDWF_OK; }
+    if (prec == 16 && prec_x == 32) { LAUNCH((cg_update_xr_kernel<float, __half>), grid, blk, smem, c->g, a); return MDWF_OK; }
+    if (prec == 16 && prec_x == 16) { LAUNCH((cg_update_xr_kernel<__half, __half>), grid, blk, smem, c->g, a); return MDWF_OK; }
     MDWF_FAIL(c, MDWF_EINVAL, "unsupported CG precision pair x=%d, r=%d", prec_x, prec);
 }
 
 int launch_cg_p(mdwf_ctx* c, int prec, CgPArgs& a, cudaStream_t st) {
-    const int grid = c->nblk * a.rl.nact;
+    const int grid = c->nblk_cls[cls_of(prec)] * a.rl.nact, blk = c->blk_cls[cls_of(prec)];
     switch (prec) {
-        case 64: return launch_big_smem(c, cg_update_p_kernel<double>, grid, g_smem<double>(c, a.op.kind != 0), st, a);
-        case 32: return launch_big_smem(c, cg_update_p_kernel<float>, grid, g_smem<float>(c, a.op.kind != 0), st, a);
-        case 16: return launch_big_smem(c, cg_update_p_kernel<__half>, grid, g_smem<__half>(c, a.op.kind != 0), st, a);
+        case 64: return launch_big_smem(c, cg_update_p_kernel<double>, grid, blk, g_smem<double>(c, a.op.kind != 0), st, a);
+        case 32: return launch_big_smem(c, cg_update_p_kernel<float>, grid, blk, g_smem<float>(c, a.op.kind != 0), st, a);
+        case 16: return launch_big_smem(c, cg_update_p_kernel<__half>, grid, blk, g_smem<__half>(c, a.op.kind != 0), st, a);
     }
     MDWF_FAIL(c, MDWF_EINVAL, "bad precision %d", prec);
 }
 
-int launch_finish(mdwf_ctx* c, const RhsList& rl, double* out, double* out2, cudaStream_t st) {
+int launch_finish(mdwf_ctx* c, int prec, const RhsList& rl, double* out, double* out2, cudaStream_t st) {
     FinishArgs f;
     f.partial = c->partial;
-    f.nblk = c->nblk;
+    f.nblk = c->nblk_cls[cls_of(prec)];
     f.out = out;
     f.out2 = out2;
     f.rl = rl;

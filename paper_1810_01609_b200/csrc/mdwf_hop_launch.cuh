@@ -24,31 +24,32 @@ static inline int launch_with_smem(mdwf_ctx* c, K kern, int grid, int block, siz
 template <typename S, int R>
 static int launch_hop_SR(mdwf_ctx* c, int dagger, int fused, HopArgs& a, cudaStream_t st) {
     typedef typename Store<S>::real T;
-    const int grid = c->nblk * a.nact;
-    const Geom& gh = c->ghop[sizeof(S) == 2 ? 0 : sizeof(S) == 4 ? 1 : 2];
+    const int cls = sizeof(S) == 2 ? 0 : sizeof(S) == 4 ? 1 : 2;
+    const Geom& gh = c->ghop[cls];
+    const int grid = c->nblk_cls[cls] * a.nact, blk = c->blk_cls[cls];
     size_t smem = 0;
     if (fused) {
-        smem = (size_t)c->block * sizeof(double);
-        if (a.op.kind) smem = std::max(smem, (size_t)smem_reals_G<T>(c->g.Ls, c->block) * sizeof(T));
+        smem = (size_t)blk * sizeof(double);
+        if (a.op.kind) smem = std::max(smem, (size_t)smem_reals_G<T>(c->g.Ls, blk) * sizeof(T));
     }
-    if (c->use_tiled && c->g.q4nsite > 0 && sizeof(T) == 4 && gh.zc % gh.q4L[2] == 0) {
+    if (c->use_tiled && c->g.q4nsite > 0 && sizeof(T) == 4 && gh.q4nsite == gh.nsite && gh.zc % gh.q4L[2] == 0) {
         // shared-memory staged 4D tiles; the epilogue reuses the spinor staging area
         const size_t st_bytes = smem_bytes_tile<S>(c->g.q4nsite, c->g.q4nslot, c->g.Ls);
         const size_t need = std::max(st_bytes, smem);
         if (fused) {
-            if (dagger) return launch_with_smem(c, hop_tile_kernel<S, R, true, true>, grid, c->block, need, st, gh, a);
-            return launch_with_smem(c, hop_tile_kernel<S, R, false, true>, grid, c->block, need, st, gh, a);
+            if (dagger) return launch_with_smem(c, hop_tile_kernel<S, R, true, true>, grid, blk, need, st, gh, a);
+            return launch_with_smem(c, hop_tile_kernel<S, R, false, true>, grid, blk, need, st, gh, a);
         }
-        if (dagger) return launch_with_smem(c, hop_tile_kernel<S, R, true, false>, grid, c->block, need, st, gh, a);
-        return launch_with_smem(c, hop_tile_kernel<S, R, false, false>, grid, c->block, need, st, gh, a);
+        if (dagger) return launch_with_smem(c, hop_tile_kernel<S, R, true, false>, grid, blk, need, st, gh, a);
+        return launch_with_smem(c, hop_tile_kernel<S, R, false, false>, grid, blk, need, st, gh, a);
     }
-    smem += smem_bytes_links<T>(c->block / c->g.Ls);
+    smem += smem_bytes_links<T>(blk / c->g.Ls);
     if (fused) {
-        if (dagger) return launch_with_smem(c, hop_kernel<S, R, true, true>, grid, c->block, smem, st, gh, a);
-        return launch_with_smem(c, hop_kernel<S, R, false, true>, grid, c->block, smem, st, gh, a);
+        if (dagger) return launch_with_smem(c, hop_kernel<S, R, true, true>, grid, blk, smem, st, gh, a);
+        return launch_with_smem(c, hop_kernel<S, R, false, true>, grid, blk, smem, st, gh, a);
     }
-    if (dagger) return launch_with_smem(c, hop_kernel<S, R, true, false>, grid, c->block, smem, st, gh, a);
-    return launch_with_smem(c, hop_kernel<S, R, false, false>, grid, c->block, smem, st, gh, a);
+    if (dagger) return launch_with_smem(c, hop_kernel<S, R, true, false>, grid, blk, smem, st, gh, a);
+    return launch_with_smem(c, hop_kernel<S, R, false, false>, grid, blk, smem, st, gh, a);
 }
 
 template <typename S>

@@ -32,8 +32,9 @@ struct mdwf_ctx {
     double M5, b5, c5, mf;
     mdwf::Geom g;
     mdwf::Geom ghop[3];        // the same with the hop traversal's z-slab depth for fp16 / fp32 / fp64 storage
-    int block;                 // threads per block: a multiple of Ls, <= 256
-    int nblk;                  // blocks per rhs = ceil(N5h / block)
+    int block;                 // threads per block (fp32 class): a multiple of Ls, <= 256
+    int nblk;                  // blocks per rhs = N5h / block (fp32 class)
+    int blk_cls[3], nblk_cls[3];   // the same per storage class (0 fp16, 1 fp32, 2 fp64): fp16 uses smaller blocks
     std::vector<GaugeSet> gauges;
     mdwf::LsOp lsop[MAT_COUNT];
     double* partial;           // [64][nblk] per-block partial sums
@@ -96,7 +97,8 @@ int launch_ls(mdwf_ctx* c, int prec, LsArgs& a, cudaStream_t st);
 int launch_axpby(mdwf_ctx* c, int prec_out, int prec_a, int prec_b, AxpbyArgs& a, cudaStream_t st);
 int launch_cg_xr(mdwf_ctx* c, int prec_x, int prec, CgXrArgs& a, cudaStream_t st);
 int launch_cg_p(mdwf_ctx* c, int prec, CgPArgs& a, cudaStream_t st);
-int launch_finish(mdwf_ctx* c, const RhsList& rl, double* out, double* out2, cudaStream_t st);
+int launch_finish(mdwf_ctx* c, int prec, const RhsList& rl, double* out, double* out2, cudaStream_t st);   // prec of the kernel that wrote the partials
+inline int cls_of(int prec) { return prec == 16 ? 0 : prec == 32 ? 1 : 2; }
 int launch_pack(mdwf_ctx* c, int prec, bool unpack, PackArgs& a, cudaStream_t st);
 int pack_gauge(mdwf_ctx* c, const void* U, int prec, int recon, GaugeSet* gs, cudaStream_t st);
 void free_gauge(GaugeSet* gs);

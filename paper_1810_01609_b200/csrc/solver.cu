@@ -51,7 +51,7 @@ struct Solver {
     int norm2(const OpCtx& o, const SpinorView& f, const RhsList& rl, int k) {
         int rc = op_ls(o, f, f, -1, nullptr, 0.0, 1.0, rl, c->partial, 0);
         if (rc) return rc;
-        return launch_finish(c, rl, dsc(k), hsc(k), st);
+        return launch_finish(c, o.prec, rl, dsc(k), hsc(k), st);
     }
     int sync() {
         MDWF_CUDA(c, cudaStreamSynchronize(st));
@@ -148,9 +148,9 @@ static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_o
         }
         if ((rc2 = launch_axpby(c, 64, 64, 64, d, st))) return rc2;                                   // rho -> t3
         if (sym && (rc2 = op_ls(S.hi, t3, t3, MAT_M5, nullptr, 0.0, 1.0, act, c->partial, 0))) return rc2;   // |M5 rho|^2
-        if ((rc2 = launch_finish(c, act, S.dsc(SC_TMP), S.hsc(SC_TMP), st))) return rc2;
+        if ((rc2 = launch_finish(c, 64, act, S.dsc(SC_TMP), S.hsc(SC_TMP), st))) return rc2;
         if ((rc2 = op_schur(S.hi, t4, t3, par, 1, sym, t4, t2, act, c->partial))) return rc2;         // r = S^dag rho
-        if ((rc2 = launch_finish(c, act, S.dsc(rrNew), S.hsc(rrNew), st))) return rc2;
+        if ((rc2 = launch_finish(c, 64, act, S.dsc(rrNew), S.hsc(rrNew), st))) return rc2;
         AxpbyArgs cv;
         cv.out = r; cv.a = t4; cv.b = none; cv.ca = 1.0; cv.cb = 0.0; cv.partial = nullptr; cv.rl = act;
         if ((rc2 = launch_axpby(c, S.prec, 64, 64, cv, st))) return rc2;
@@ -196,12 +196,12 @@ static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_o
         if (!open) { cudaEventRecord(e0, st); open = true; }
         // t = S p, pAp = |t|^2 ; Ap = S^dag t   (out may alias the first work field, see op_schur)
         if ((rc = op_schur(S.lo, t, p, par, 0, sym, t, wb, act, c->partial, 1))) break;   // t holds A p on entry
-        if ((rc = launch_finish(c, act, S.dsc(SC_PAP), S.hsc(SC_PAP), st))) break;
+        if ((rc = launch_finish(c, S.prec, act, S.dsc(SC_PAP), S.hsc(SC_PAP), st))) break;
         if ((rc = op_schur(S.lo, wa, t, par, 1, sym, wa, wb, act))) break;
         CgXrArgs u;
         u.x = xl; u.r = r; u.p = p; u.Ap = wa; u.rr = S.dsc(rrOld); u.pAp = S.dsc(SC_PAP); u.partial = c->partial; u.rl = act;
         if ((rc = launch_cg_xr(c, S.px, S.prec, u, st))) break;
-        if ((rc = launch_finish(c, act, S.dsc(rrNew), S.hsc(rrNew), st))) break;
+        if ((rc = launch_finish(c, S.prec, act, S.dsc(rrNew), S.hsc(rrNew), st))) break;
         for (int k = 0; k < act.nact; ++k) iters[act.rhs[k]]++;
         bool need_update = false;
         if (++since_check >= S.check_every) {
