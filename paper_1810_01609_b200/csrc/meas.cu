@@ -122,30 +122,34 @@ __device__ __forceinline__ double2 cfma(double2 a, double2 b, double2 c) {
     return make_double2(c.x + a.x * b.x - a.y * b.y, c.y + a.x * b.y + a.y * b.x);
 }
 
-#define MDWF_NUC_WARPS 4
+#define MDWF_NUC_WARPS 8      // warps per block
+#define MDWF_NUC_WPS 2        // warps per site (they meet at a named barrier)
 __constant__ int c_perm[6][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}, {0, 2, 1}, {2, 1, 0}, {1, 0, 2}};
 __constant__ double c_psign[6] = {1, 1, 1, -1, -1, -1};
 __global__ void __launch_bounds__(32 * MDWF_NUC_WARPS) nucleon_kernel(const NucArgs a) {
-    // One warp per site (only warp-level barriers); 144 work items per phase are spread over the 32 lanes.
+    // MDWF_NUC_WPS warps per site (named barriers only); 144 work items per phase are spread over their lanes.
     // prop element (sink spin al, sink colour ca, source spin be, source colour cb) at S[(3*be+cb)*12 + 3*al+ca]
     extern __shared__ __align__(16) unsigned char nuc_smem[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    double2* base = reinterpret_cast<double2*>(nuc_smem) + warp * (5 * 144 + 16);
+    constexpr int GT = 32 * MDWF_NUC_WPS;                     // threads per site group
+    const int grp = threadIdx.x / GT, lane = threadIdx.x % GT;
+    double2* base = reinterpret_cast<double2*>(nuc_smem) + grp * (5 * 144 + 16);
+#define NUC_SYNC() asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "r"(GT) : "memory")
     double2 *s1 = base, *sd = base + 144, *s2 = base + 288, *Q = base + 432, *W = base + 576, *trP = base + 720;
     const int t = blockIdx.y;
     double accr = 0.0, acci = 0.0;
-    const int wid = blockIdx.x * MDWF_NUC_WARPS + warp, nw = a.nblk_t * MDWF_NUC_WARPS;
-    for (long long xs = wid; xs < a.V3; xs += nw) {
+    constexpr int GPB = MDWF_NUC_WARPS / MDWF_NUC_WPS;         // site groups per block
+    const int gid = blockIdx.x * GPB + grp, ng = a.nblk_t * GPB;
+    for (long long xs = gid; xs < a.V3; xs += ng) {
         const long long x = (long long)t * a.V3 + xs;
-        for (int i = lane; i < 144; i += 32) {
+        for (int i = lane; i < 144; i += GT) {
             const int col = i / 12, k = i - col * 12;
             const long long off = ((long long)col * a.V4 + x) * 12 + k;
             s1[i] = __ldg(a.Su1 + off);
             sd[i] = __ldg(a.Sd + off);
             s2[i] = __ldg(a.Su2 + off);
         }
-        __syncwarp();
-        for (int e = lane; e < 144; e += 32) {
+        NUC_SYNC();
+        for (int e = lane; e < 144; e += GT) {
             // e -> (b, b', al, al'):  Q^{bb'}_{al al'} = sum_{be,be'} G[al][be] Sd^{bb'}_{be be'} Gt[be'][al']
             const int b = e / 48, bp = (e / 16) % 3, al = (e / 4) % 4, alp = e % 4;
             double2 q = make_double2(0.0, 0.0);
@@ -180,8 +184,8 @@ __global__ void __launch_bounds__(32 * MDWF_NUC_WARPS) nucleon_kernel(const NucA
                               s2[(3 * gap + cp) * 12 + 3 * ga + c], tr);
             trP[lane] = tr;
         }
-        __syncwarp();
-        for (int wi = lane; wi < 144; wi += 32) {
+        NUC_SYNC();
+        for (int wi = lane; wi < 144; wi += GT) {
             const int e = wi / 4, alp = wi % 4, e1 = e / 6, e2 = e % 6;
             const int ca = c_perm[e1][0], cb = c_perm[e1][1], cc = c_perm[e1][2];
             const int cap = c_perm[e2][0], cbp = c_perm[e2][1], ccp = c_perm[e2][2];
@@ -205,7 +209,7 @@ __global__ void __launch_bounds__(32 * MDWF_NUC_WARPS) nucleon_kernel(const NucA
             accr += sg * (d.x - ex.x);
             acci += sg * (d.y - ex.y);
         }
-        __syncwarp();
+        NUC_SYNC();
     }
     // fixed-order warp sum, one partial per warp
 #pragma unroll
@@ -213,10 +217,12 @@ __global__ void __launch_bounds__(32 * MDWF_NUC_WARPS) nucleon_kernel(const NucA
         accr += __shfl_down_sync(0xffffffffu, accr, o);
         acci += __shfl_down_sync(0xffffffffu, acci, o);
     }
-    if (lane == 0) {
+    if ((threadIdx.x & 31) == 0) {
+        const int wid = blockIdx.x * MDWF_NUC_WARPS + (threadIdx.x >> 5), nw = a.nblk_t * MDWF_NUC_WARPS;
         a.partial[((long long)t * nw + wid) * 2] = accr;
         a.partial[((long long)t * nw + wid) * 2 + 1] = acci;
     }
+#undef NUC_SYNC
 }
 
 __global__ void nucleon_finish_kernel(double* corr, const double* partial, int nblk_t, int T, int t0) {
@@ -310,7 +316,8 @@ int mdwf_nucleon_2pt(mdwf_ctx* c, double* corr, const void* S_u1, const void* S_
     a.Su1 = (const double2*)S_u1; a.Sd = (const double2*)S_d; a.Su2 = (const double2*)S_u2;
     a.V4 = 2ll * c->g.Vh; a.V3 = a.V4 / c->g.T;
     const int T = c->g.T;
-    a.nblk_t = (int)std::min<long long>((a.V3 + MDWF_NUC_WARPS - 1) / MDWF_NUC_WARPS, std::max(1, (c->sm_count * 16) / T));
+    const int gpb = MDWF_NUC_WARPS / MDWF_NUC_WPS;
+    a.nblk_t = (int)std::min<long long>((a.V3 + gpb - 1) / gpb, std::max(1, (c->sm_count * 16) / T));
     // C = gamma_y gamma_t, G = C gamma5, Gt = gamma_t G^dag gamma_t in the DeGrand-Rossi basis (SURVEY 8 Notation)
     const double gy[32] = {0,0, 0,0, 0,0, -1,0,   0,0, 0,0, 1,0, 0,0,   0,0, 1,0, 0,0, 0,0,   -1,0, 0,0, 0,0, 0,0};
     const double gt[32] = {0,0, 0,0, 1,0, 0,0,   0,0, 0,0, 0,0, 1,0,   1,0, 0,0, 0,0, 0,0,   0,0, 1,0, 0,0, 0,0};
@@ -330,7 +337,7 @@ int mdwf_nucleon_2pt(mdwf_ctx* c, double* corr, const void* S_u1, const void* S_
     MDWF_CUDA(c, cudaMallocAsync(&partial, sizeof(double) * 2 * T * npart, st));
     a.partial = partial;
     dim3 grid(a.nblk_t, T);
-    const size_t nsm = (size_t)MDWF_NUC_WARPS * (5 * 144 + 16) * sizeof(double2);
+    const size_t nsm = (size_t)gpb * (5 * 144 + 16) * sizeof(double2);
     static bool raised = false;
     if (!raised) { MDWF_CUDA(c, cudaFuncSetAttribute(nucleon_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nsm)); raised = true; }
     nucleon_kernel<<<grid, 32 * MDWF_NUC_WARPS, nsm, st>>>(a);
