@@ -168,6 +168,10 @@ int mdwf_profile_read(mdwf_ctx* ctx, int cls, double* ms, double* bytes, double*
 /* set the z-slab depth of the hop kernel's site traversal (L2 tiling); 0 = automatic */
 int mdwf_set_tiling(mdwf_ctx* ctx, int zc);
 
+/* Measured plain-FP32 FMA throughput of the device [TFLOP/s] (dependent-chain-free FFMA loop on every SM, CUDA-event
+ * timed): the ALU ceiling that co-bounds the 16-bit-storage stencil.  Returns MDWF_OK. */
+int mdwf_probe_fp32_fma(mdwf_ctx* ctx, double* tflops, void* stream);
+
 /* Host-only self-test (needs no GPU): the run-time-constant division used for site decoding (exhaustive over
  * the index ranges in use), the closed-form M5^-1 blocks against M5 (M5 * M5^-1 = 1) and dagger = transpose,
  * for Ls = 1..32 at the given parameters.  Returns 0 on success, else the number of the failed check. */

@@ -24,7 +24,7 @@ EXPORTS = [
     "mdwf_create", "mdwf_destroy", "mdwf_last_error", "mdwf_load_gauge", "mdwf_dslash", "mdwf_field_create",
     "mdwf_field_destroy", "mdwf_field_pack", "mdwf_field_unpack", "mdwf_dslash_packed", "mdwf_dslash_cost",
     "mdwf_solve", "mdwf_solve_host", "mdwf_seq_source", "mdwf_nucleon_2pt", "mdwf_wall_inject",
-    "mdwf_wall_project", "mdwf_launch_count", "mdwf_set_tiling", "mdwf_profile", "mdwf_profile_read", "mdwf_selftest_host",
+    "mdwf_wall_project", "mdwf_launch_count", "mdwf_set_tiling", "mdwf_profile", "mdwf_profile_read", "mdwf_selftest_host", "mdwf_probe_fp32_fma",
 ]
 
 
@@ -90,6 +90,7 @@ def lib():
         L.mdwf_profile_read.argtypes = [vp, ci, ctypes.POINTER(cd), ctypes.POINTER(cd), ctypes.POINTER(cd),
                                         ctypes.POINTER(ctypes.c_int64)]
         L.mdwf_selftest_host.argtypes = [cd, cd, cd, cd]
+        L.mdwf_probe_fp32_fma.argtypes = [vp, ctypes.POINTER(cd), vp]
         _lib = L
     return _lib
 
@@ -302,3 +303,9 @@ class Context:
         self._chk(lib().mdwf_profile_read(self._h, cls, ctypes.byref(ms), ctypes.byref(by), ctypes.byref(fl),
                                           ctypes.byref(n)))
         return ms.value, by.value, fl.value, n.value
+
+    def mdwf_probe_fp32_fma(self):
+        """measured plain-FP32 FMA throughput of the device, TFLOP/s"""
+        t = ctypes.c_double()
+        self._chk(lib().mdwf_probe_fp32_fma(self._h, ctypes.byref(t), _stream()))
+        return t.value
