@@ -179,20 +179,37 @@ static int pick_zc(const mdwf_ctx* c, const Geom& g, int want, double site_bytes
         if (g.Z % z == 0 && z % lz == 0 && (best == 0 || (double)g.XH * g.Y * z * g.Ls * site_bytes <= 9.0e6)) best = z;
     return best;
 }
+static void fill_zc(mdwf_ctx* c, Geom& g, int zc) {
+    g.zc = zc;
+    g.dZc = make_fastdiv(zc);
+    g.dSlab = make_fastdiv((uint32_t)(g.XH * g.Y * zc));
+    g.dTslab = make_fastdiv((uint32_t)(g.XH * g.Y * zc) * (uint32_t)g.T);
+    g.dnTzs = make_fastdiv((uint32_t)(zc / g.tz));
+    g.q4dTzs = make_fastdiv((uint32_t)std::max(1, zc / (g.q4nsite > 0 ? g.q4L[2] : 1)));
+    g.ntc = (g.XH / g.txh) * (g.Y / g.ty) * (zc / g.tz);
+    g.dntc = make_fastdiv((uint32_t)g.ntc);
+    (void)c;
+}
+static const double kSiteBytes[3] = {52.0, 96.0, 192.0};
 static void set_zc(mdwf_ctx* c, int want) {
-    const double site_bytes[3] = {52.0, 96.0, 192.0};
-    for (int cls = 0; cls < 3; ++cls) {
-        Geom& g = c->ghop[cls];
-        const int zc = pick_zc(c, g, want, site_bytes[cls]);
-        g.zc = zc;
-        g.dZc = make_fastdiv(zc);
-        g.dSlab = make_fastdiv((uint32_t)(g.XH * g.Y * zc));
-        g.dTslab = make_fastdiv((uint32_t)(g.XH * g.Y * zc) * (uint32_t)g.T);
-        g.dnTzs = make_fastdiv((uint32_t)(zc / g.tz));
-        g.q4dTzs = make_fastdiv((uint32_t)std::max(1, zc / (g.q4nsite > 0 ? g.q4L[2] : 1)));
-    }
+    c->zc_forced = want > 0 ? want : 0;
+    c->ghop_multi.clear();
+    for (int cls = 0; cls < 3; ++cls) fill_zc(c, c->ghop[cls], pick_zc(c, c->ghop[cls], want, kSiteBytes[cls]));
     c->g = c->ghop[1];
 }
+namespace mdwf {
+// Geometry of a hop launch: with nact rhs in flight the slab working set is nact times larger, so the slab depth is
+// chosen for nact * (bytes per site)
+const Geom& hop_geom(mdwf_ctx* c, int cls, int nact) {
+    if (nact <= 1 || c->zc_forced > 0) return c->ghop[cls];
+    const int key = cls * 100 + nact;
+    auto it = c->ghop_multi.find(key);
+    if (it != c->ghop_multi.end()) return it->second;
+    Geom g = c->ghop[cls];
+    fill_zc(c, g, pick_zc(c, g, 0, kSiteBytes[cls] * nact));
+    return c->ghop_multi.emplace(key, g).first->second;
+}
+}  // namespace mdwf
 // Sites of a block: a box txh*ty*tz*tt (x fastest) that divides the lattice, filled greedily along x, then y, z, t
 // up to `cap` sites, i.e. (nearly) whole x-rows in storage order.  Compact 4D boxes (e.g. 4x4x2x2) were measured
 // SLOWER on B200 (profiles/README.md, "tile shape").  cap: min(256/Ls, 32) sites for fp32/fp64 storage, min(128/Ls, 32)
@@ -239,7 +256,7 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     mdwf_ctx* c = new mdwf_ctx;
     c->geo = *geo;
     c->M5 = M5; c->b5 = b5; c->c5 = c5; c->mf = mf;
-    c->partial = nullptr; c->dscal = nullptr; c->hscal = nullptr; c->launches = 0; c->prof_on = 0; c->use_tiled = 0;
+    c->partial = nullptr; c->dscal = nullptr; c->hscal = nullptr; c->launches = 0; c->prof_on = 0; c->use_tiled = 0; c->zc_forced = 0;
     for (int i = 0; i < 6; ++i) c->q4dev[i] = nullptr;
     for (int i = 0; i < 3; ++i) { c->prof_ms[i] = c->prof_bytes[i] = c->prof_flops[i] = 0.0; c->prof_n[i] = 0; }
     *out = c;   // returned even on failure so that mdwf_last_error can be read; caller destroys it

@@ -57,6 +57,8 @@ struct Geom {
     // 4D tiles of the hop kernel: a block owns txh*ty*tz*tt sites (x fastest); tiles are ordered x, y, z within a
     // z-slab of depth zc, then t, then slab, so that t-neighbours are re-used from L2 and in-tile neighbours from L1
     int txh, ty, tz, tt, nsite;
+    int ntc;                            // tiles per (z-slab, timeslice-of-tiles) chunk: blocks run chunk-major, then rhs, then tile
+    FastDiv dntc;
     FastDiv dtxh, dty, dtz;             // in-tile decode
     FastDiv dnTx, dnTy, dnTzs, dnTt;    // tile-index decode: tiles per row, per column, per slab depth, per T
     // compact 4D tiles with shared-memory staged neighbours (mdwf_hop_tile.cuh); q4nsite == 0 -> not available.

@@ -398,8 +398,12 @@ __global__ void __launch_bounds__(256, (sizeof(S) == 8 ? MDWF_HOP_MINB64 : sizeo
     T* links = reinterpret_cast<T*>(smem_raw);
     int* tab = reinterpret_cast<int*>(smem_raw + (size_t)nsite * MDWF_LSITE * sizeof(T));
     unsigned char* smem_epi = smem_raw + smem_bytes_links<T>(nsite);
-    const int slot = blockIdx.x % a.nact;
-    const int tile = blockIdx.x / a.nact;
+    // block order: chunk (z-slab x tile-timeslice) slowest, then rhs, then the tiles of the chunk -- all rhs of a
+    // chunk run back to back (their links stay in L2) while each rhs streams through its own slab working set
+    uint32_t bq, tin;
+    g.dntc.divmod(blockIdx.x, bq, tin);
+    const int slot = bq % a.nact;
+    const int tile = (bq / a.nact) * g.ntc + tin;
     const int rhs = a.rhs_list[slot];
     // ---- stage the block's links and neighbour table --------------------------------------------------
     if (Store<S>::HALF && a.g.prep[a.par] != nullptr) {

@@ -25,7 +25,7 @@ template <typename S, int R>
 static int launch_hop_SR(mdwf_ctx* c, int dagger, int fused, HopArgs& a, cudaStream_t st) {
     typedef typename Store<S>::real T;
     const int cls = sizeof(S) == 2 ? 0 : sizeof(S) == 4 ? 1 : 2;
-    const Geom& gh = c->ghop[cls];
+    const Geom& gh = hop_geom(c, cls, a.nact);
     const int grid = c->nblk_cls[cls] * a.nact, blk = c->blk_cls[cls];
     size_t smem = 0;
     if (fused) {

@@ -31,7 +31,9 @@ struct mdwf_ctx {
     mdwf_geometry geo;
     double M5, b5, c5, mf;
     mdwf::Geom g;
-    mdwf::Geom ghop[3];        // the same with the hop traversal's z-slab depth for fp16 / fp32 / fp64 storage
+    mdwf::Geom ghop[3];
+    std::map<int, mdwf::Geom> ghop_multi;   // the same for launches with several rhs (key cls*100 + nact): shallower slabs
+    int zc_forced;             // > 0: mdwf_set_tiling fixed the slab depth        // the same with the hop traversal's z-slab depth for fp16 / fp32 / fp64 storage
     int block;                 // threads per block (fp32 class): a multiple of Ls, <= 256
     int nblk;                  // blocks per rhs = N5h / block (fp32 class)
     int blk_cls[3], nblk_cls[3];   // the same per storage class (0 fp16, 1 fp32, 2 fp64): fp16 uses smaller blocks
@@ -100,6 +102,7 @@ int launch_cg_p(mdwf_ctx* c, int prec, CgPArgs& a, cudaStream_t st);
 int launch_finish(mdwf_ctx* c, int prec, const RhsList& rl, double* out, double* out2, cudaStream_t st);   // prec of the kernel that wrote the partials
 inline int cls_of(int prec) { return prec == 16 ? 0 : prec == 32 ? 1 : 2; }
 int launch_pack(mdwf_ctx* c, int prec, bool unpack, PackArgs& a, cudaStream_t st);
+const mdwf::Geom& hop_geom(mdwf_ctx* c, int cls, int nact);
 int pack_gauge(mdwf_ctx* c, const void* U, int prec, int recon, GaugeSet* gs, cudaStream_t st);
 void free_gauge(GaugeSet* gs);
 
