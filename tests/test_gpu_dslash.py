@@ -129,3 +129,21 @@ def test_tiled_shared_memory_hop_variant_matches_oracle():
                        capture_output=True, text=True, timeout=900)
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
     assert "passed" in r.stdout
+
+
+def test_traversal_order_does_not_change_results():
+    """the z-slab depth (mdwf_set_tiling) only reorders blocks: results are bit-identical for every legal depth"""
+    dims, Ls = (8, 8, 8, 4), 8          # blocks are whole (x, y) planes here, so every divisor of Z is a legal depth
+    mdwf, p, U, ctx = setup(dims, Ls, 0.1)
+    ctx.mdwf_load_gauge(U.cuda(), 32, 12)
+    Vh = int(np.prod(dims)) // 2
+    inp = synth.gaussian_spinor(dims, Ls, 3, 1010)[:, :, :Vh].contiguous().cuda()
+    ref = None
+    for zc in (0, 1, 2, 4, 8):
+        ctx.mdwf_set_tiling(zc)
+        out = ctx.mdwf_dslash(mdwf.OP_DHAT_SYM, inp, parity=1, prec=32, recon=12)
+        if ref is None:
+            ref = out
+        assert torch.equal(torch.view_as_real(out), torch.view_as_real(ref)), zc
+    with pytest.raises(mdwf.MdwfError):
+        ctx.mdwf_set_tiling(3)
