@@ -10,10 +10,10 @@
 // traffic", turns Mhat into two of these launches).  gamma matrices: DeGrand-Rossi chiral
 // basis written out below from SURVEY 8 Notation (gamma5 = diag(1,1,-1,-1): P+ = spins 0,1).
 //
-// One thread per 5D site (s fastest), one rhs per block; blocks are ordered rhs-fastest so the blocks
-// that share a tile's links run together and hit L2; sites are traversed in z-slabs so t-neighbours
-// are reused from L2.  Links are loaded through L1 (all Ls threads of a site read the
-// same vectors: one broadcast sector per warp).
+// One thread per 5D site (s fastest), one rhs per block; blocks run chunk-major (z-slab x timeslice of tiles), then
+// rhs, then tile, so the rhs sharing a chunk's links run back to back; sites are traversed in z-slabs so that
+// t-neighbours are re-read from L2, not HBM.  The block's links are reconstructed once into shared
+// memory and read from there by all Ls threads of a site.
 #pragma once
 #include "mdwf_device.cuh"
 
