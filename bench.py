@@ -309,10 +309,13 @@ def main():
         return
     line = {"metric": METRIC, "value": aggregate(st["sec_per_rhs"], world), "unit": "s/RHS", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": st["ms_step"], "higher_is_better": False,
-            "scaling": "weak", "vs_baseline": None, "dtype": {16: "f16 storage / f32 compute / f64 outer", 32: "f32 / f64 outer", 64: "f64"}[args.inner],
+            "scaling": "weak", "vs_baseline": None, "dtype": {16: "f32", 32: "f32", 64: "f64"}[args.inner],
             "data": "synthetic",
             "config": {"workload": cfg.name, "lattice": list(cfg.dims), "Ls": cfg.Ls, "nrhs_per_gpu": nrhs, "tol": cfg.tol,
-                       "mf": cfg.mf, "inner_prec": args.inner, "recon": args.recon, "links": "reunit(exp(i*%.3f*H))" % cfg.eps,
+                       "mf": cfg.mf, "inner_prec": args.inner, "recon": args.recon,
+                       "arithmetic": {16: "inner CG: fp16 storage (+fp32 scale per site), fp32 arithmetic, fp64 reductions; outer: fp64 reliable updates",
+                                      32: "inner CG: fp32 storage and arithmetic, fp64 reductions; outer: fp64 reliable updates",
+                                      64: "fp64 throughout"}[args.inner], "links": "reunit(exp(i*%.3f*H))" % cfg.eps,
                        "rhs": "Gaussian complex 5D, device-drawn, seeded", "parallelism": "replicas only",
                        "l2": "inputs larger than L2 (half-lattice 16-bit spinor %.0f MB per rhs)" % (cfg.V4 / 2 * cfg.Ls * 52 / 1e6)},
             "cg": {"seconds_per_rhs_per_replica": st["sec_per_rhs"], "iters": res.iters, "reliable_updates": res.reliable_updates,
