@@ -159,7 +159,7 @@ def run_ours(args):
     torch.cuda.empty_cache()
     b = synth.gaussian_spinor_device(cfg.dims, cfg.Ls, nrhs, synth.seed_for(cfg.index, 2) + 7 * rank, device=dev)
     x = torch.empty_like(b)
-    kw = dict(tol=cfg.tol, inner_prec=inner, recon=recon, symmetric=True, batch=args.batch, check_every=args.check_every, delta=args.delta)
+    kw = dict(tol=cfg.tol, inner_prec=inner, recon=recon, symmetric=not args.asym, batch=args.batch, check_every=args.check_every, delta=args.delta)
 
     def step():
         _, res = ctx.mdwf_solve(b, out=x, **kw)
@@ -293,6 +293,7 @@ def main():
     ap.add_argument("--recon", type=int, default=12)
     ap.add_argument("--batch", type=int, default=0)
     ap.add_argument("--check-every", type=int, default=1)
+    ap.add_argument("--asym", action="store_true", help="solve with Dhat instead of Mhat = M5^-1 Dhat")
     ap.add_argument("--delta", type=float, default=0.0, help="reliable-update threshold (0 = library default)")
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--e2e-warmup", type=int, default=1)
