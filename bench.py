@@ -214,10 +214,12 @@ def run_ours(args):
                             "peak_measured_ffma_loop": fp32_measured,
                             "note": "convention flops (1320 per 5D site) / FP32 FMA peak; ncu: issue slots 68-70 % busy"}
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic_r1.json")) as f:
-            tr = json.load(f).get("%s|inner%d|recon%d" % (cfg.name, inner, recon))
-        if tr and nrhs >= 1:
-            roof["traffic"] = tr["dram_bytes_per_launch"]
+        import csv
+        with open(os.path.join(ROOT, "profiles", "traffic_r1.csv")) as f:
+            rows = {r["key"]: r for r in csv.DictReader(f)}
+        tr = rows.get("%s|inner%d|recon%d" % (cfg.name, inner, recon))
+        if tr:
+            roof["traffic"] = float(tr["dram_bytes_per_launch"])
             roof["traffic_source"] = tr["source"]
             roof["algorithmic_bytes_per_launch"] = pby / pn if pn else None
     except Exception:
