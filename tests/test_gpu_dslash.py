@@ -147,3 +147,23 @@ def test_traversal_order_does_not_change_results():
         assert torch.equal(torch.view_as_real(out), torch.view_as_real(ref)), zc
     with pytest.raises(mdwf.MdwfError):
         ctx.mdwf_set_tiling(3)
+
+
+def test_maximum_ls_and_empty_batch():
+    """Ls = 32 (the maximum the library accepts: 8 resp. 4 sites per block) through the fused Schur operator in all
+    three storage precisions; Ls = 33 and an empty batch are refused."""
+    dims, Ls = (4, 4, 2, 4), 32
+    mdwf, p, U, ctx = setup(dims, Ls, 0.05)
+    psi = synth.gaussian_spinor(dims, Ls, 2, 1020).numpy()
+    same = oracle.mask(p, psi, 0)
+    inp = torch.from_numpy(oracle.to_half(same, dims, 0)).cuda()
+    for prec, recon in [(64, 18), (32, 12), (16, 8)]:
+        ctx.mdwf_load_gauge(U.cuda(), prec, recon)
+        for dagger in (False, True):
+            exp = oracle.to_half(oracle.schur(p, U.numpy(), same, 0, dagger, True), dims, 0)
+            got = ctx.mdwf_dslash(mdwf.OP_DHAT_SYM, inp, parity=0, dagger=dagger, prec=prec, recon=recon)
+            assert rel(got.cpu().numpy(), exp) <= TOL[prec] * (4 if prec == 16 else 1), (prec, dagger)
+    with pytest.raises(mdwf.MdwfError):
+        mdwf.Context(dims, 33, 1.3, 1.5, 0.5, 0.1)
+    with pytest.raises(mdwf.MdwfError):
+        ctx.mdwf_dslash(mdwf.OP_HOP, inp[:0].contiguous(), prec=64, recon=18)
