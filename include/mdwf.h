@@ -22,6 +22,8 @@
  *      gauge      U[mu][x4][row 3][col 3][re,im]               U_mu(x) = link from x to x+mu
  *      4D field   eta[col][x4][spin][colour][re,im]            col = 3*spin_src + colour_src
  *  - there is no CPU fallback: every entry point needs a CUDA device.
+ *  - a context (and the fields created from it) must not be used from two host threads at the same time; separate
+ *    contexts are independent.
  */
 #ifndef MDWF_H
 #define MDWF_H
