@@ -207,11 +207,9 @@ def run_ours(args):
     # the 16-bit kernel is co-bound by FP32 issue: report it against the plain-FP32 FMA peak
     # 148 SMs x 128 lanes x 2 flop x max SM clock, with the 1320 flop/site convention
     fp32_peak = 148 * 128 * 2 * (clocks.get("sm_max_mhz") or 1965) * 1e-6
-    fp32_measured = ctx.mdwf_probe_fp32_fma()
     if roof["gflops"]:
         roof["co_bound"] = {"bound": "alu", "achieved": roof["gflops"] * 1e-3, "peak": fp32_peak, "unit": "TFLOP/s",
                             "frac": roof["gflops"] * 1e-3 / fp32_peak,
-                            "peak_measured_ffma_loop": fp32_measured,
                             "note": "convention flops (1320 per 5D site) / FP32 FMA peak; ncu: issue slots 68-70 % busy"}
     try:
         import csv

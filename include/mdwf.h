@@ -124,6 +124,7 @@ typedef struct {
     double seconds;                    /* device time of the whole call (CUDA events)                 */
     double seconds_inner;              /* device time spent in inner (low precision) iterations       */
     int64_t kernel_launches;           /* kernels launched by this call                               */
+    int32_t batch;                     /* rhs that were in flight together (the launches' n_active)    */
 } mdwf_solve_info;
 
 /* Solve D psi = b for nrhs (<= MDWF_MAX_RHS) right-hand sides by even-odd preconditioning +
@@ -137,6 +138,20 @@ int mdwf_solve(mdwf_ctx* ctx, void* x, const void* b, int nrhs, const mdwf_solve
  * and copies the result back; all copies are inside the call. */
 int mdwf_solve_host(mdwf_ctx* ctx, void* x_host, const void* b_host, int nrhs, const mdwf_solve_opts* opts,
                     mdwf_solve_info* info, void* stream);
+
+/* The same solve on PACKED fp64 half-lattice fields, in place: psi_even / psi_odd (mdwf_field_create(ctx, 64, nrhs),
+ * filled with mdwf_field_pack) hold b on entry and the solution on exit.  No canonical copies are involved, so a
+ * whole batch of large-volume rhs fits on the device at once (config 5: 4 rhs in flight, SURVEY 8(a) A20
+ * "batched multi-RHS").  5D sources / solutions only. */
+int mdwf_solve_packed(mdwf_ctx* ctx, mdwf_field* psi_even, mdwf_field* psi_odd, const mdwf_solve_opts* opts,
+                      mdwf_solve_info* info, void* stream);
+/* Solver workspace: by default the library allocates it on first use and keeps it until destroy (it grows
+ * when a larger batch asks for more).  mdwf_workspace_bytes: bytes a batch of `nrhs` rhs needs with the fp64 temporaries
+ * of the reliable updates shared one rhs at a time (packed != 0: for mdwf_solve_packed, whose sources live in the
+ * caller's fields).  mdwf_set_workspace hands the library a caller-owned device buffer (e.g. from PyTorch's allocator)
+ * to use instead -- it must stay valid until replaced or destroy; mem = NULL returns to library-owned memory. */
+int mdwf_workspace_bytes(mdwf_ctx* ctx, int nrhs, int inner_prec, int packed, int64_t* bytes);
+int mdwf_set_workspace(mdwf_ctx* ctx, void* mem, int64_t bytes);
 
 /* Feynman-Hellmann sequential source:
  * out4d[col](x) = Gamma . prop4d[col](x) on timeslices t_min <= t <= t_max (all t = "sum over t"),
@@ -163,16 +178,17 @@ int64_t mdwf_launch_count(const mdwf_ctx* ctx);
  * mdwf_profile(ctx, 1) clears the counters and starts recording, mdwf_profile(ctx, 0) stops.
  * mdwf_profile_read synchronises the recorded events and returns, for class cls (0: fp16 storage, 1: fp32,
  * 2: fp64), the summed device time [ms], algorithmic bytes and flops (DESIGN.md cost convention: per 5D
- * site 24*w (+4) bytes per spinor pass, 2 passes (+1 with an xpay input), links once per launch; 1320 flop)
+ * site 24*w bytes per spinor pass, 2 passes (+1 with an xpay input), links once per launch; 1320 flop)
  * and the launch count. */
 int mdwf_profile(mdwf_ctx* ctx, int enable);
 int mdwf_profile_read(mdwf_ctx* ctx, int cls, double* ms, double* bytes, double* flops, int64_t* launches);
 /* set the z-slab depth of the hop kernel's site traversal (L2 tiling); 0 = automatic */
 int mdwf_set_tiling(mdwf_ctx* ctx, int zc);
 
-/* Measured plain-FP32 FMA throughput of the device [TFLOP/s] (dependent-chain-free FFMA loop on every SM, CUDA-event
- * timed): the ALU ceiling that co-bounds the 16-bit-storage stencil.  Returns MDWF_OK. */
-int mdwf_probe_fp32_fma(mdwf_ctx* ctx, double* tflops, void* stream);
+/* Tuning control of the fp16 tensor-core stencil (mdwf_hop16.cuh): the 4D box of output sites one block owns
+ * (lx even; each extent divides the lattice) and the warps per block (0 = default).  lx = 0 returns to the automatic
+ * choice.  Results do not depend on it beyond fp32 summation order.  EINVAL if the box does not fit in shared memory. */
+int mdwf_set_hop16_tile(mdwf_ctx* ctx, int lx, int ly, int lz, int lt, int warps);
 
 /* Host-only self-test (needs no GPU): the run-time-constant division used for site decoding (exhaustive over
  * the index ranges in use), the closed-form M5^-1 blocks against M5 (M5 * M5^-1 = 1) and dagger = transpose,

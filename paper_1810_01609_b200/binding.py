@@ -24,7 +24,8 @@ EXPORTS = [
     "mdwf_create", "mdwf_destroy", "mdwf_last_error", "mdwf_load_gauge", "mdwf_dslash", "mdwf_field_create",
     "mdwf_field_destroy", "mdwf_field_pack", "mdwf_field_unpack", "mdwf_dslash_packed", "mdwf_dslash_cost",
     "mdwf_solve", "mdwf_solve_host", "mdwf_seq_source", "mdwf_nucleon_2pt", "mdwf_wall_inject",
-    "mdwf_wall_project", "mdwf_launch_count", "mdwf_set_tiling", "mdwf_profile", "mdwf_profile_read", "mdwf_selftest_host", "mdwf_probe_fp32_fma",
+    "mdwf_wall_project", "mdwf_launch_count", "mdwf_set_tiling", "mdwf_profile", "mdwf_profile_read", "mdwf_selftest_host", "mdwf_solve_packed",
+    "mdwf_workspace_bytes", "mdwf_set_workspace", "mdwf_set_hop16_tile",
 ]
 
 
@@ -50,7 +51,7 @@ class SolveInfo(ctypes.Structure):
     _fields_ = [("iters", ctypes.c_int32 * MAX_RHS), ("reliable_updates", ctypes.c_int32 * MAX_RHS),
                 ("status", ctypes.c_int32 * MAX_RHS), ("true_resid", ctypes.c_double * MAX_RHS),
                 ("seconds", ctypes.c_double), ("seconds_inner", ctypes.c_double),
-                ("kernel_launches", ctypes.c_int64)]
+                ("kernel_launches", ctypes.c_int64), ("batch", ctypes.c_int32)]
 
 
 _lib = None
@@ -90,7 +91,10 @@ def lib():
         L.mdwf_profile_read.argtypes = [vp, ci, ctypes.POINTER(cd), ctypes.POINTER(cd), ctypes.POINTER(cd),
                                         ctypes.POINTER(ctypes.c_int64)]
         L.mdwf_selftest_host.argtypes = [cd, cd, cd, cd]
-        L.mdwf_probe_fp32_fma.argtypes = [vp, ctypes.POINTER(cd), vp]
+        L.mdwf_solve_packed.argtypes = [vp, vp, vp, ctypes.POINTER(SolveOpts), ctypes.POINTER(SolveInfo), vp]
+        L.mdwf_workspace_bytes.argtypes = [vp, ci, ci, ci, ctypes.POINTER(ctypes.c_int64)]
+        L.mdwf_set_workspace.argtypes = [vp, vp, ctypes.c_int64]
+        L.mdwf_set_hop16_tile.argtypes = [vp, ci, ci, ci, ci, ci]
         _lib = L
     return _lib
 
@@ -125,6 +129,7 @@ class SolveResult:
     seconds: float
     seconds_inner: float
     kernel_launches: int
+    batch: int = 0
 
 
 def mdwf_selftest_host(M5=1.3, b5=1.5, c5=0.5, mf=0.05):
@@ -231,7 +236,8 @@ class Context:
     @staticmethod
     def _result(rc, info, nrhs):
         return SolveResult(rc, list(info.iters[:nrhs]), list(info.reliable_updates[:nrhs]), list(info.status[:nrhs]),
-                           list(info.true_resid[:nrhs]), info.seconds, info.seconds_inner, info.kernel_launches)
+                           list(info.true_resid[:nrhs]), info.seconds, info.seconds_inner, info.kernel_launches,
+                           info.batch)
 
     def mdwf_solve(self, b: torch.Tensor, tol=1e-8, max_iter=20000, inner_prec=16, recon=12, parity=0, symmetric=True,
                    delta=0.1, src_kind=0, out_kind=0, batch=0, check_every=1, out=None):
@@ -258,6 +264,33 @@ class Context:
                                              ctypes.c_void_p(b_host.data_ptr()), nrhs, ctypes.byref(o),
                                              ctypes.byref(info), _stream()), soft_ok=True)
         return x_host, self._result(rc, info, nrhs)
+
+    def mdwf_solve_packed(self, psi_even: Field, psi_odd: Field, **kw):
+        """In-place solve on packed fp64 half-lattice fields (b on entry, solution on exit)."""
+        nrhs = psi_even.nrhs
+        o = self._opts(kw.get("tol", 1e-8), kw.get("max_iter", 20000), kw.get("inner_prec", 16), kw.get("recon", 12),
+                       kw.get("parity", 0), kw.get("symmetric", True), kw.get("delta", 0.1), 0, 0, 0,
+                       kw.get("check_every", 1))
+        info = SolveInfo()
+        rc = self._chk(lib().mdwf_solve_packed(self._h, psi_even._h, psi_odd._h, ctypes.byref(o), ctypes.byref(info),
+                                               _stream()), soft_ok=True)
+        return self._result(rc, info, nrhs)
+
+    def mdwf_workspace_bytes(self, nrhs, inner_prec=16, packed=False):
+        n = ctypes.c_int64()
+        self._chk(lib().mdwf_workspace_bytes(self._h, nrhs, inner_prec, int(bool(packed)), ctypes.byref(n)))
+        return n.value
+
+    def mdwf_set_workspace(self, buf):
+        """buf: a CUDA uint8 tensor the library uses as its solver workspace (kept alive here), or None."""
+        self._ws = buf
+        if buf is None:
+            self._chk(lib().mdwf_set_workspace(self._h, None, 0))
+        else:
+            self._chk(lib().mdwf_set_workspace(self._h, ctypes.c_void_p(buf.data_ptr()), buf.numel() * buf.element_size()))
+
+    def mdwf_set_hop16_tile(self, lx, ly, lz, lt, warps=0):
+        self._chk(lib().mdwf_set_hop16_tile(self._h, lx, ly, lz, lt, warps))
 
     def mdwf_seq_source(self, prop4d: torch.Tensor, Gamma, t_min=0, t_max=None, out=None):
         ncol = prop4d.shape[0]
@@ -303,9 +336,3 @@ class Context:
         self._chk(lib().mdwf_profile_read(self._h, cls, ctypes.byref(ms), ctypes.byref(by), ctypes.byref(fl),
                                           ctypes.byref(n)))
         return ms.value, by.value, fl.value, n.value
-
-    def mdwf_probe_fp32_fma(self):
-        """measured plain-FP32 FMA throughput of the device, TFLOP/s"""
-        t = ctypes.c_double()
-        self._chk(lib().mdwf_probe_fp32_fma(self._h, ctypes.byref(t), _stream()))
-        return t.value

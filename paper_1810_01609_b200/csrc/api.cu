@@ -1,6 +1,7 @@
 // csrc/api.cu -- the C-ABI entry points declared in include/mdwf.h (context, gauge load, Dslash family,
 // packed fields) and the composite even-odd operators built from the fused kernels.
 #include "mdwf_host.h"
+#include "mdwf_hop16.cuh"
 #include <cmath>
 #include <cstring>
 #include <algorithm>
@@ -62,70 +63,6 @@ static void build_matrices(int Ls, double M5, double b5, double c5, double mf, s
     }
 }
 
-// Compact 4D tiles for mdwf_hop_tile.cuh: choose a box Lx x Ly x Lz x Lt (Lx even) that divides the lattice, holds
-// exactly g.nsite output sites (so every kernel keeps the same thread <-> site blocking) and needs the fewest input
-// slots (box interior of the other parity + one-site halo); tabulate, for both parities of the box origin, the
-// local coordinates of outputs and slots and the slot of each leg.
-static int setup_tile4(mdwf_ctx* c) {
-    Geom& g = c->g;
-    g.q4nsite = 0; g.q4nslot = 0;
-    for (int i = 0; i < 4; ++i) g.q4L[i] = 1;
-    for (int p = 0; p < 2; ++p) { g.q4out[p] = nullptr; g.q4slot[p] = nullptr; g.q4nbr[p] = nullptr; }
-    const int dims[4] = {g.X, g.Y, g.Z, g.T};
-    int best[4] = {0, 0, 0, 0}, bestslots = 1 << 30;
-    for (int lx = 2; lx <= 8; lx += 2) for (int ly = 1; ly <= 6; ++ly) for (int lz = 1; lz <= 6; ++lz) for (int lt = 1; lt <= 6; ++lt) {
-        if (dims[0] % lx || dims[1] % ly || dims[2] % lz || dims[3] % lt) continue;
-        if (lx * ly * lz * lt != 2 * g.nsite) continue;
-        if ((ly * lz * lt) % 2 || (lx * lz * lt) % 2 || (lx * ly * lt) % 2 || (lx * ly * lz) % 2) continue;   // faces split evenly by parity
-        const int slots = g.nsite + ly * lz * lt + lx * lz * lt + lx * ly * lt + lx * ly * lz;
-        if (slots < bestslots && slots <= 255) { bestslots = slots; best[0] = lx; best[1] = ly; best[2] = lz; best[3] = lt; }
-    }
-    if (!best[0]) return MDWF_OK;      // no suitable box: the row-tile kernel is used
-    const int* L = best;
-    for (int pat = 0; pat < 2; ++pat) {
-        std::vector<int> outp, slotp;
-        std::vector<unsigned char> nbr;
-        std::map<int, int> slot_of;
-        auto pack = [](int x, int y, int z, int t) { return x | (y << 8) | (z << 16) | (t << 24); };
-        // interior input sites, then the halo, in (t, z, y, x) order over the extended box [-1, L]
-        for (int pass = 0; pass < 2; ++pass)
-            for (int t = -1; t <= L[3]; ++t) for (int z = -1; z <= L[2]; ++z) for (int y = -1; y <= L[1]; ++y) for (int x = -1; x <= L[0]; ++x) {
-                const int outside = (x < 0 || x >= L[0]) + (y < 0 || y >= L[1]) + (z < 0 || z >= L[2]) + (t < 0 || t >= L[3]);
-                if (outside != pass) continue;                       // pass 0: interior, pass 1: faces (exactly one coordinate out)
-                if (((x + y + z + t + pat) & 1) == 0) continue;      // inputs have the other parity (x+..+pat odd; -1 is odd too)
-                const int key = pack(x + 1, y + 1, z + 1, t + 1);
-                slot_of[key] = (int)slotp.size();
-                slotp.push_back(key);
-            }
-        for (int t = 0; t < L[3]; ++t) for (int z = 0; z < L[2]; ++z) for (int y = 0; y < L[1]; ++y) for (int x = 0; x < L[0]; ++x) {
-            if ((x + y + z + t + pat) & 1) continue;
-            outp.push_back(pack(x, y, z, t));
-            for (int mu = 0; mu < 4; ++mu)
-                for (int dir = 0; dir < 2; ++dir) {
-                    int cc[4] = {x, y, z, t};
-                    cc[mu] += dir == 0 ? 1 : -1;
-                    const auto it = slot_of.find(pack(cc[0] + 1, cc[1] + 1, cc[2] + 1, cc[3] + 1));
-                    if (it == slot_of.end()) MDWF_FAIL(c, MDWF_EINVAL, "internal: 4D tile table is inconsistent");
-                    nbr.push_back((unsigned char)it->second);
-                }
-        }
-        if ((int)outp.size() != g.nsite || (int)slotp.size() != bestslots) MDWF_FAIL(c, MDWF_EINVAL, "internal: 4D tile counts (%zu, %zu)", outp.size(), slotp.size());
-        void *d0, *d1, *d2;
-        MDWF_CUDA(c, cudaMalloc(&d0, outp.size() * 4));
-        MDWF_CUDA(c, cudaMalloc(&d1, slotp.size() * 4));
-        MDWF_CUDA(c, cudaMalloc(&d2, nbr.size()));
-        MDWF_CUDA(c, cudaMemcpy(d0, outp.data(), outp.size() * 4, cudaMemcpyHostToDevice));
-        MDWF_CUDA(c, cudaMemcpy(d1, slotp.data(), slotp.size() * 4, cudaMemcpyHostToDevice));
-        MDWF_CUDA(c, cudaMemcpy(d2, nbr.data(), nbr.size(), cudaMemcpyHostToDevice));
-        c->q4dev[3 * pat] = d0; c->q4dev[3 * pat + 1] = d1; c->q4dev[3 * pat + 2] = d2;
-        g.q4out[pat] = (const int*)d0; g.q4slot[pat] = (const int*)d1; g.q4nbr[pat] = (const unsigned char*)d2;
-    }
-    for (int i = 0; i < 4; ++i) g.q4L[i] = L[i];
-    g.q4nsite = g.nsite; g.q4nslot = bestslots;
-    g.q4dTx = make_fastdiv(g.X / L[0]); g.q4dTy = make_fastdiv(g.Y / L[1]); g.q4dTt = make_fastdiv(g.T / L[3]);
-    return MDWF_OK;
-}
-
 // The structured form of the same operators that the kernels apply (LsOp, mdwf_hop.cuh).
 static void build_lsops(int Ls, double M5, double b5, double c5, double mf, LsOp ops[MAT_COUNT]) {
     const double a = b5 * (4.0 - M5) + 1.0, d = c5 * (4.0 - M5) - 1.0, kappa = -d / a;
@@ -143,6 +80,17 @@ static void build_lsops(int Ls, double M5, double b5, double c5, double mf, LsOp
         else { o.kind = 1; o.c0 = b5 / a; o.c1 = c5 / a; }
         ops[MAT_AM5INV + 4 * dag] = o;
     }
+}
+// 2-norm bounds of the same operators (used only to choose fp16 scales, mdwf_device.cuh ScaleRule): |L| <= max(1, mf);
+// |M5^-1| <= sqrt(|.|_1 |.|_inf) = max(1, mf) sum_k |kappa|^k / |a (1 + mf kappa^Ls)| from the closed form.
+static void build_lsop_norms(int Ls, double M5, double b5, double c5, double mf, const LsOp ops[MAT_COUNT], double nrm[MAT_COUNT]) {
+    const double a = b5 * (4.0 - M5) + 1.0, d = c5 * (4.0 - M5) - 1.0, kappa = -d / a;
+    const double lmax = std::max(1.0, std::fabs(mf));
+    double geo = 0.0;
+    for (int k = 0; k < Ls; ++k) geo += std::pow(std::fabs(kappa), k);
+    const double minv = lmax * geo / std::fabs(a * (1.0 + mf * std::pow(kappa, Ls)));
+    for (int i = 0; i < MAT_COUNT; ++i)
+        nrm[i] = std::fabs(ops[i].c0) + std::fabs(ops[i].c1) * (ops[i].kind == 2 ? minv : lmax);
 }
 // host emulation of apply_ls on one chirality column (for the self-test): out = op(v), v[s], chi 0 = P+
 static void lsop_host(const LsOp& op, int Ls, int chi, const std::vector<double>& v, std::vector<double>& out) {
@@ -172,11 +120,11 @@ static void lsop_host(const LsOp& op, int Ls, int chi, const std::vector<double>
 // the streamed output) live in L2 (measured on B200, 48^3x64 Ls=10: fp32 fastest at zc = 8,
 // fp64 at zc = 4, fp16 flat between 2 and 16)
 static int pick_zc(const mdwf_ctx* c, const Geom& g, int want, double site_bytes) {
-    const int lz = (c->use_tiled && g.q4nsite > 0) ? g.q4L[2] : 1;   // only the opt-in tile kernel constrains zc
-    if (want > 0 && g.Z % want == 0 && want % g.tz == 0 && want % lz == 0) return want;
+    (void)c;
+    if (want > 0 && g.Z % want == 0 && want % g.tz == 0) return want;
     int best = 0;
     for (int z = g.tz; z <= g.Z; z += g.tz)
-        if (g.Z % z == 0 && z % lz == 0 && (best == 0 || (double)g.XH * g.Y * z * g.Ls * site_bytes <= 9.0e6)) best = z;
+        if (g.Z % z == 0 && (best == 0 || (double)g.XH * g.Y * z * g.Ls * site_bytes <= 9.0e6)) best = z;
     return best;
 }
 static void fill_zc(mdwf_ctx* c, Geom& g, int zc) {
@@ -185,12 +133,11 @@ static void fill_zc(mdwf_ctx* c, Geom& g, int zc) {
     g.dSlab = make_fastdiv((uint32_t)(g.XH * g.Y * zc));
     g.dTslab = make_fastdiv((uint32_t)(g.XH * g.Y * zc) * (uint32_t)g.T);
     g.dnTzs = make_fastdiv((uint32_t)(zc / g.tz));
-    g.q4dTzs = make_fastdiv((uint32_t)std::max(1, zc / (g.q4nsite > 0 ? g.q4L[2] : 1)));
     g.ntc = (g.XH / g.txh) * (g.Y / g.ty) * (zc / g.tz);
     g.dntc = make_fastdiv((uint32_t)g.ntc);
     (void)c;
 }
-static const double kSiteBytes[3] = {52.0, 96.0, 192.0};
+static const double kSiteBytes[3] = {48.0, 96.0, 192.0};
 static void set_zc(mdwf_ctx* c, int want) {
     c->zc_forced = want > 0 ? want : 0;
     c->ghop_multi.clear();
@@ -216,7 +163,6 @@ const Geom& hop_geom(mdwf_ctx* c, int cls, int nact) {
 // for fp16 -- the issue-bound fp16 kernels stall less at their block barriers with ~128-thread blocks (measured
 // -5..7 % on the fused kernels), while fp32 prefers the larger ones.
 static void pick_tile(Geom& g, int cap) {
-    if (getenv("MDWF_MAX_SITES")) cap = std::min(cap, atoi(getenv("MDWF_MAX_SITES")));   // experiments
     cap = std::max(1, cap);
     int best[4] = {1, 1, 1, 1};
     const int ext[4] = {g.XH, g.Y, g.Z, g.T};
@@ -256,8 +202,10 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     mdwf_ctx* c = new mdwf_ctx;
     c->geo = *geo;
     c->M5 = M5; c->b5 = b5; c->c5 = c5; c->mf = mf;
-    c->partial = nullptr; c->dscal = nullptr; c->hscal = nullptr; c->launches = 0; c->prof_on = 0; c->use_tiled = 0; c->zc_forced = 0;
-    for (int i = 0; i < 6; ++i) c->q4dev[i] = nullptr;
+    c->partial = nullptr; c->dscal = nullptr; c->hscal = nullptr; c->launches = 0; c->prof_on = 0; c->zc_forced = 0;
+    c->tile16 = nullptr; c->tile16_nw = 0; c->partial_nblk = 0; c->partial_cap = 0;
+    c->ws = nullptr; c->ws_bytes = 0; c->ws_external = false;
+    for (int i = 0; i < 4; ++i) c->tile16_forced[i] = 0;
     for (int i = 0; i < 3; ++i) { c->prof_ms[i] = c->prof_bytes[i] = c->prof_flops[i] = 0.0; c->prof_n[i] = 0; }
     *out = c;   // returned even on failure so that mdwf_last_error can be read; caller destroys it
     long long v4 = 1;
@@ -288,11 +236,6 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     for (int m = 0; m < 4; ++m) g.bc[m] = geo->bc[m];
     g.dLs = make_fastdiv(g.Ls); g.dXH = make_fastdiv(g.XH); g.dY = make_fastdiv(g.Y); g.dZ = make_fastdiv(g.Z);
     pick_tile(g, std::min(256 / g.Ls, 32));
-    {
-        const int rc4 = setup_tile4(c);      // the (opt-in) 4D tiles follow the fp32 blocking
-        if (rc4) return rc4;
-    }
-    c->use_tiled = getenv("MDWF_HOP_TILED") ? atoi(getenv("MDWF_HOP_TILED")) : 0;
     int max_nblk = 0;
     for (int cls = 0; cls < 3; ++cls) {
         c->ghop[cls] = g;
@@ -304,11 +247,14 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     c->block = c->blk_cls[1];
     c->nblk = c->nblk_cls[1];
     set_zc(c, 0);
-    MDWF_CUDA(c, cudaMalloc(&c->partial, sizeof(double) * 64 * (size_t)max_nblk));
-    MDWF_CUDA(c, cudaMalloc(&c->dscal, sizeof(double) * 8 * 64));
-    MDWF_CUDA(c, cudaMemset(c->dscal, 0, sizeof(double) * 8 * 64));
-    MDWF_CUDA(c, cudaHostAlloc(&c->hscal, sizeof(double) * 8 * 64, cudaHostAllocDefault));
+    c->partial_cap = std::max<size_t>((size_t)max_nblk, (size_t)(g.N5h + 255) / 256 + 1);
+    c->partial_cap = std::max<size_t>(c->partial_cap, (size_t)c->sm_count * 4);
+    MDWF_CUDA(c, cudaMalloc(&c->partial, sizeof(double) * 64 * c->partial_cap));
+    MDWF_CUDA(c, cudaMalloc(&c->dscal, sizeof(double) * 16 * 64));
+    MDWF_CUDA(c, cudaMemset(c->dscal, 0, sizeof(double) * 16 * 64));
+    MDWF_CUDA(c, cudaHostAlloc(&c->hscal, sizeof(double) * 16 * 64, cudaHostAllocDefault));
     build_lsops(g.Ls, M5, b5, c5, mf, c->lsop);
+    build_lsop_norms(g.Ls, M5, b5, c5, mf, c->lsop, c->lsop_norm);
     return MDWF_OK;
 }
 
@@ -316,7 +262,8 @@ int mdwf_destroy(mdwf_ctx* c) {
     if (!c) return MDWF_OK;
     for (size_t i = 0; i < c->gauges.size(); ++i) free_gauge(&c->gauges[i]);
     for (auto& kv : c->temps) for (mdwf_field* f : kv.second) free_field(f);
-    for (int i = 0; i < 6; ++i) if (c->q4dev[i]) cudaFree(c->q4dev[i]);
+    if (c->tile16) { free_tile16(c->tile16); delete c->tile16; c->tile16 = nullptr; }
+    if (c->ws && !c->ws_external) cudaFree(c->ws);
     prof_drain(c);
     for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
     if (c->partial) cudaFree(c->partial);
@@ -390,9 +337,8 @@ int mdwf_selftest_host(double M5, double b5, double c5, double mf) {
 
 int mdwf_set_tiling(mdwf_ctx* c, int zc) {
     if (!c) return MDWF_EINVAL;
-    if (zc < 0 || (zc > 0 && (c->g.Z % zc != 0 || zc % c->ghop[0].tz != 0 || zc % c->ghop[1].tz != 0)))
+    if (zc < 0 || (zc > 0 && (c->g.Z % zc != 0 || zc % c->ghop[1].tz != 0 || zc % c->ghop[2].tz != 0)))
         MDWF_FAIL(c, MDWF_EINVAL, "zc = %d must divide Z = %d and be a multiple of the tile depth %d", zc, c->g.Z, c->g.tz);
-    if (zc > 0 && c->use_tiled && c->g.q4nsite > 0 && zc % c->g.q4L[2] != 0) MDWF_FAIL(c, MDWF_EINVAL, "zc = %d must be a multiple of the 4D tile depth %d", zc, c->g.q4L[2]);
     set_zc(c, zc);
     return MDWF_OK;
 }
@@ -418,28 +364,40 @@ int mdwf_load_gauge(mdwf_ctx* c, const void* U, int store_prec, int recon, void*
 // ---------------------------------------------------------------------------------------------
 namespace mdwf {
 
-int op_ls(const OpCtx& o, const SpinorView& out, const SpinorView& in, int mat, const SpinorView* xin, double cx,
-          double ch, const RhsList& rl, double* partial, int write) {
-    LsArgs a;
-    a.out = out; a.in = in;
-    if (xin) a.xin = *xin; else { a.xin.v = nullptr; a.xin.n = nullptr; a.xin.rs = a.xin.rn = 0; }
-    if (mat >= 0) a.op = o.c->lsop[mat]; else a.op.kind = 0;
-    a.cx = cx; a.ch = ch; a.partial = partial; a.write = write; a.rl = rl;
-    return launch_ls(o.c, o.prec, a, o.st);
+static SpinorView no_view() {
+    SpinorView v;
+    v.v = nullptr; v.m = nullptr; v.rs = 0;
+    return v;
 }
 
-int op_hop(const OpCtx& o, const SpinorView& out, const SpinorView& in, int out_par, int dagger, int mat,
-           const SpinorView* xin, double cx, double ch, const RhsList& rl, double* partial) {
-    HopArgs a;
-    a.out = out; a.in = in;
-    if (xin) a.xin = *xin; else { a.xin.v = nullptr; a.xin.n = nullptr; a.xin.rs = a.xin.rn = 0; }
-    a.g.v[0] = o.gs->v[0]; a.g.v[1] = o.gs->v[1];
-    for (int p = 0; p < 2; ++p) { a.g.prep[p] = reinterpret_cast<const float4*>(o.gs->prep[p]); a.g.nbr[p] = o.gs->nbr[p]; }
+int op_ls(const OpCtx& o, mdwf_field* out, const mdwf_field* in, int mat, const mdwf_field* xin, double cx,
+          double ch, const RhsList& rl, double* partial, int write) {
+    LsArgs a;
+    a.out = out->view(); a.in = in->view();
+    a.xin = xin ? xin->view() : no_view();
     if (mat >= 0) a.op = o.c->lsop[mat]; else a.op.kind = 0;
+    a.cx = cx; a.ch = ch; a.partial = partial; a.write = write; a.rl = rl;
+    a.sr = write ? rule_lin(out, in, std::fabs(ch) * (mat >= 0 ? o.c->lsop_norm[mat] : 1.0), xin, std::fabs(cx)) : rule_lin(nullptr, nullptr, 0.0);
+    const int rc = launch_ls(o.c, o.prec, a, o.st);
+    if (write) out->flip();
+    return rc;
+}
+
+int op_hop(const OpCtx& o, mdwf_field* out, const mdwf_field* in, int out_par, int dagger, int mat,
+           const mdwf_field* xin, double cx, double ch, const RhsList& rl, double* partial) {
+    HopArgs a;
+    a.out = out->view(); a.in = in->view();
+    a.xin = xin ? xin->view() : no_view();
+    a.g.v[0] = o.gs->v[0]; a.g.v[1] = o.gs->v[1];
+    if (mat >= 0) a.op = o.c->lsop[mat]; else { a.op = o.c->lsop[0]; a.op.kind = 0; }
     a.cx = cx; a.ch = ch; a.partial = partial; a.par = out_par; a.nact = rl.nact;
     for (int i = 0; i < 64; ++i) a.rhs_list[i] = rl.rhs[i];
+    // |H_{p<-pbar}| <= 8: each of the 8 legs is (1 -+ gamma_mu) x unitary = 2 x (projector x unitary)
+    a.sr = rule_lin(out, in, 8.0 * std::fabs(ch) * (mat >= 0 ? o.c->lsop_norm[mat] : 1.0), xin, std::fabs(cx));
     const int fused = (mat >= 0 || xin || partial || ch != 1.0) ? 1 : 0;
-    return launch_hop(o.c, o.prec, o.recon, dagger, fused, a, o.st);
+    const int rc = launch_hop(o.c, o.prec, o.recon, dagger, fused, a, o.st);
+    out->flip();
+    return rc;
 }
 
 // Dhat = M5 - 1/4 H A M5^-1 H A,  Mhat = M5^-1 Dhat,  and their adjoints (SURVEY 8 "Even-odd form"):
@@ -447,24 +405,24 @@ int op_hop(const OpCtx& o, const SpinorView& out, const SpinorView& in, int out_
 //   Dhat v     : t1 = A v ; t2 = (A M5^-1) H t1 ; t1 = M5 v ; out = t1 - 1/4 H t2
 //   Mhat^dag v : t1 = M5^-dag v ; t2 = (A M5^-1)^dag H^dag t1 ; out = v - 1/4 A^dag H^dag t2
 //   Dhat^dag v : t2 = (A M5^-1)^dag H^dag v ; t1 = M5^dag v ; out = t1 - 1/4 A^dag H^dag t2
-int op_schur(const OpCtx& o, const SpinorView& out, const SpinorView& in, int par, int dagger, int symmetric,
-             const SpinorView& t1, const SpinorView& t2, const RhsList& rl, double* partial, int first_factor_done) {
+int op_schur(const OpCtx& o, mdwf_field* out, const mdwf_field* in, int par, int dagger, int symmetric,
+             mdwf_field* t1, mdwf_field* t2, const RhsList& rl, double* partial, int first_factor_done) {
     int rc;
     if (!dagger) {
         if (!first_factor_done && (rc = op_ls(o, t1, in, MAT_A, nullptr, 0.0, 1.0, rl))) return rc;
         if ((rc = op_hop(o, t2, t1, 1 - par, 0, MAT_AM5INV, nullptr, 0.0, 1.0, rl))) return rc;
-        if (symmetric) return op_hop(o, out, t2, par, 0, MAT_M5INV, &in, 1.0, -0.25, rl, partial);
+        if (symmetric) return op_hop(o, out, t2, par, 0, MAT_M5INV, in, 1.0, -0.25, rl, partial);
         if ((rc = op_ls(o, t1, in, MAT_M5, nullptr, 0.0, 1.0, rl))) return rc;
-        return op_hop(o, out, t2, par, 0, -1, &t1, 1.0, -0.25, rl, partial);
+        return op_hop(o, out, t2, par, 0, -1, t1, 1.0, -0.25, rl, partial);
     }
     if (symmetric) {
         if ((rc = op_ls(o, t1, in, MAT_M5INV_D, nullptr, 0.0, 1.0, rl))) return rc;
         if ((rc = op_hop(o, t2, t1, 1 - par, 1, MAT_AM5INV_D, nullptr, 0.0, 1.0, rl))) return rc;
-        return op_hop(o, out, t2, par, 1, MAT_A_D, &in, 1.0, -0.25, rl, partial);
+        return op_hop(o, out, t2, par, 1, MAT_A_D, in, 1.0, -0.25, rl, partial);
     }
     if ((rc = op_hop(o, t2, in, 1 - par, 1, MAT_AM5INV_D, nullptr, 0.0, 1.0, rl))) return rc;
     if ((rc = op_ls(o, t1, in, MAT_M5_D, nullptr, 0.0, 1.0, rl))) return rc;
-    return op_hop(o, out, t2, par, 1, MAT_A_D, &t1, 1.0, -0.25, rl, partial);
+    return op_hop(o, out, t2, par, 1, MAT_A_D, t1, 1.0, -0.25, rl, partial);
 }
 
 static int make_opctx(mdwf_ctx* c, int prec, int recon, cudaStream_t st, OpCtx* o) {
@@ -487,18 +445,17 @@ static int dslash_packed_impl(mdwf_ctx* c, int op, int parity, int dagger, int r
     const bool needs_gauge = !(op == MDWF_OP_M4PRE || op == MDWF_OP_M5 || op == MDWF_OP_M5INV);
     int rc;
     if (needs_gauge && (rc = make_opctx(c, prec, recon, st, &o))) return rc;
-    const SpinorView vi = in->view(), vo = out->view();
     const int dg = dagger ? 4 : 0;
     switch (op) {
-        case MDWF_OP_HOP: return op_hop(o, vo, vi, parity, dagger, -1, nullptr, 0.0, 1.0, rl);
-        case MDWF_OP_M4PRE: return op_ls(o, vo, vi, MAT_A + dg, nullptr, 0.0, 1.0, rl);
-        case MDWF_OP_M5: return op_ls(o, vo, vi, MAT_M5 + dg, nullptr, 0.0, 1.0, rl);
-        case MDWF_OP_M5INV: return op_ls(o, vo, vi, MAT_M5INV + dg, nullptr, 0.0, 1.0, rl);
+        case MDWF_OP_HOP: return op_hop(o, out, in, parity, dagger, -1, nullptr, 0.0, 1.0, rl);
+        case MDWF_OP_M4PRE: return op_ls(o, out, in, MAT_A + dg, nullptr, 0.0, 1.0, rl);
+        case MDWF_OP_M5: return op_ls(o, out, in, MAT_M5 + dg, nullptr, 0.0, 1.0, rl);
+        case MDWF_OP_M5INV: return op_ls(o, out, in, MAT_M5INV + dg, nullptr, 0.0, 1.0, rl);
         case MDWF_OP_DHAT_ASYM:
         case MDWF_OP_DHAT_SYM: {
             mdwf_field *t1, *t2;
             if ((rc = temp_field(c, prec, nrhs, 2, &t1)) || (rc = temp_field(c, prec, nrhs, 3, &t2))) return rc;
-            return op_schur(o, vo, vi, parity, dagger, op == MDWF_OP_DHAT_SYM, t1->view(), t2->view(), rl);
+            return op_schur(o, out, in, parity, dagger, op == MDWF_OP_DHAT_SYM, t1, t2, rl);
         }
         case MDWF_OP_NORMAL_ASYM:
         case MDWF_OP_NORMAL_SYM: {
@@ -506,8 +463,8 @@ static int dslash_packed_impl(mdwf_ctx* c, int op, int parity, int dagger, int r
             if ((rc = temp_field(c, prec, nrhs, 2, &t1)) || (rc = temp_field(c, prec, nrhs, 3, &t2)) ||
                 (rc = temp_field(c, prec, nrhs, 4, &t3))) return rc;
             const int sym = op == MDWF_OP_NORMAL_SYM;
-            if ((rc = op_schur(o, t3->view(), vi, parity, 0, sym, t1->view(), t2->view(), rl))) return rc;
-            return op_schur(o, vo, t3->view(), parity, 1, sym, t1->view(), t2->view(), rl);
+            if ((rc = op_schur(o, t3, in, parity, 0, sym, t1, t2, rl))) return rc;
+            return op_schur(o, out, t3, parity, 1, sym, t1, t2, rl);
         }
     }
     MDWF_FAIL(c, MDWF_EINVAL, "unknown or non-packed op %d", op);
@@ -515,7 +472,37 @@ static int dslash_packed_impl(mdwf_ctx* c, int op, int parity, int dagger, int r
 
 }  // namespace mdwf
 
+namespace mdwf {
+// canonical fp64 <-> packed field (half lattice: full = 0; one parity of a full-lattice field: full = 1)
+int pack_field(mdwf_field* f, const double* canon, int full, int par, cudaStream_t st) {
+    PackArgs a;
+    memset(&a, 0, sizeof(a));
+    a.f = f->view(); a.canon = const_cast<double*>(canon); a.Vc = (full ? 2ll : 1ll) * f->ctx->g.Vh; a.full = full; a.par = par;
+    a.nrhs = f->nrhs; a.rhs0 = 0;
+    a.sr.out = f->wmeta();
+    const int rc = launch_pack(f->ctx, f->prec, false, a, st);
+    f->flip();
+    return rc;
+}
+int unpack_field(const mdwf_field* f, double* canon, int full, int par, cudaStream_t st) {
+    PackArgs a;
+    memset(&a, 0, sizeof(a));
+    a.f = f->view(); a.canon = canon; a.Vc = (full ? 2ll : 1ll) * f->ctx->g.Vh; a.full = full; a.par = par; a.nrhs = f->nrhs; a.rhs0 = 0;
+    return launch_pack(f->ctx, f->prec, true, a, st);
+}
+}  // namespace mdwf
+
 extern "C" {
+
+int mdwf_set_hop16_tile(mdwf_ctx* c, int lx, int ly, int lz, int lt, int warps) {
+    if (!c) return MDWF_EINVAL;
+    if (warps < 0 || warps > MDWF_H16_MAXW) MDWF_FAIL(c, MDWF_EINVAL, "warps must be in 0..%d", MDWF_H16_MAXW);
+    if (c->tile16) { free_tile16(c->tile16); delete c->tile16; c->tile16 = nullptr; }
+    c->tile16_forced[0] = lx; c->tile16_forced[1] = ly; c->tile16_forced[2] = lz; c->tile16_forced[3] = lt;
+    c->tile16_nw = warps;
+    Tile16Host* th;
+    return get_tile16(c, &th);
+}
 
 int mdwf_field_create(mdwf_ctx* c, int prec, int nrhs, mdwf_field** out) {
     if (!c || !out) return MDWF_EINVAL;
@@ -527,15 +514,11 @@ int mdwf_field_destroy(mdwf_field* f) {
 }
 int mdwf_field_pack(mdwf_field* f, const void* canonical, void* stream) {
     if (!f || !canonical) return MDWF_EINVAL;
-    PackArgs a;
-    a.f = f->view(); a.canon = (double*)canonical; a.Vc = f->ctx->g.Vh; a.full = 0; a.par = 0; a.nrhs = f->nrhs; a.rhs0 = 0;
-    return launch_pack(f->ctx, f->prec, false, a, (cudaStream_t)stream);
+    return pack_field(f, (const double*)canonical, 0, 0, (cudaStream_t)stream);
 }
 int mdwf_field_unpack(const mdwf_field* f, void* canonical, void* stream) {
     if (!f || !canonical) return MDWF_EINVAL;
-    PackArgs a;
-    a.f = f->view(); a.canon = (double*)canonical; a.Vc = f->ctx->g.Vh; a.full = 0; a.par = 0; a.nrhs = f->nrhs; a.rhs0 = 0;
-    return launch_pack(f->ctx, f->prec, true, a, (cudaStream_t)stream);
+    return unpack_field(f, (double*)canonical, 0, 0, (cudaStream_t)stream);
 }
 
 int mdwf_dslash_packed(mdwf_ctx* c, int op, int parity, int dagger, int recon, mdwf_field* out,
@@ -566,35 +549,30 @@ int mdwf_dslash(mdwf_ctx* c, int op, int parity, int dagger, int prec, int recon
         (rc = temp_field(c, prec, nrhs, 1, &fo)) || (rc = temp_field(c, prec, nrhs, 2, &t1)) ||
         (rc = temp_field(c, prec, nrhs, 3, &t2))) return rc;
     const RhsList rl = all_rhs(nrhs);
+    for (int p = 0; p < 2; ++p)
+        if ((rc = pack_field(f[p], (const double*)in, 1, p, st))) return rc;
     for (int p = 0; p < 2; ++p) {
-        PackArgs a;
-        a.f = f[p]->view(); a.canon = (double*)in; a.Vc = 2ll * c->g.Vh; a.full = 1; a.par = p; a.nrhs = nrhs; a.rhs0 = 0;
-        if ((rc = launch_pack(c, prec, false, a, st))) return rc;
-    }
-    for (int p = 0; p < 2; ++p) {
-        const SpinorView same = f[p]->view(), other = f[1 - p]->view(), v1 = t1->view(), v2 = t2->view();
+        mdwf_field *same = f[p], *other = f[1 - p];
         if (!dagger) {
-            if ((rc = op_ls(o, v1, other, MAT_A, nullptr, 0.0, 1.0, rl))) return rc;
-            if ((rc = op_ls(o, v2, same, MAT_M5, nullptr, 0.0, 1.0, rl))) return rc;
-            if ((rc = op_hop(o, fo->view(), v1, p, 0, -1, &v2, 1.0, -0.5, rl))) return rc;
+            if ((rc = op_ls(o, t1, other, MAT_A, nullptr, 0.0, 1.0, rl))) return rc;
+            if ((rc = op_ls(o, t2, same, MAT_M5, nullptr, 0.0, 1.0, rl))) return rc;
+            if ((rc = op_hop(o, fo, t1, p, 0, -1, t2, 1.0, -0.5, rl))) return rc;
         } else {
-            if ((rc = op_ls(o, v2, same, MAT_M5_D, nullptr, 0.0, 1.0, rl))) return rc;
-            if ((rc = op_hop(o, fo->view(), other, p, 1, MAT_A_D, &v2, 1.0, -0.5, rl))) return rc;
+            if ((rc = op_ls(o, t2, same, MAT_M5_D, nullptr, 0.0, 1.0, rl))) return rc;
+            if ((rc = op_hop(o, fo, other, p, 1, MAT_A_D, t2, 1.0, -0.5, rl))) return rc;
         }
-        PackArgs a;
-        a.f = fo->view(); a.canon = (double*)out; a.Vc = 2ll * c->g.Vh; a.full = 1; a.par = p; a.nrhs = nrhs; a.rhs0 = 0;
-        if ((rc = launch_pack(c, prec, true, a, st))) return rc;
+        if ((rc = unpack_field(fo, (double*)out, 1, p, st))) return rc;
     }
     return MDWF_OK;
 }
 
 // per 5D site and rhs, w = bytes per real,
-//   hop: 1320 flop, 2*24*w (+8 for fp16 norms) + 8*R*w/(Ls*nrhs) bytes;  A, M5: 72 flop;  M5^-1: 48*Ls flop;
-//   site-local ops: 2*24*w (+8) bytes;  Dhat/Mhat: 2832 + 96*Ls flop, fused floor 5 spinor passes + 2 link passes.
+//   hop: 1320 flop, 2*24*w + 8*R*w/(Ls*nrhs) bytes;  A, M5: 72 flop;  M5^-1: 48*Ls flop;
+//   site-local ops: 2*24*w bytes;  Dhat/Mhat: 2832 + 96*Ls flop, fused floor 5 spinor passes + 2 link passes.
 int mdwf_dslash_cost(const mdwf_ctx* c, int op, int prec, int recon, int nrhs, double* bytes, double* flops) {
     if (!c || !bytes || !flops) return MDWF_EINVAL;
     const double w = prec / 8.0, n5 = (double)c->g.N5h * nrhs, Ls = c->g.Ls;
-    const double pass = 24.0 * w + (prec == 16 ? 4.0 : 0.0);
+    const double pass = 24.0 * w;
     const double links = 8.0 * recon * w * c->g.Vh;
     switch (op) {
         case MDWF_OP_HOP: *bytes = 2 * pass * n5 + links; *flops = 1320.0 * n5; return MDWF_OK;

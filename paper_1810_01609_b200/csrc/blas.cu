@@ -1,40 +1,59 @@
 // csrc/blas.cu -- launchers of the 4D-site-local kernels in mdwf_blas.cuh and the packed-field allocator.
 #include "mdwf_hop_launch.cuh"
+#include <cstring>
 
 namespace mdwf {
 
 static size_t rhs_bytes(const Geom& g, int prec) {
+    if (prec == 16) return ((size_t)g.N5h * 48 + 255) / 256 * 256;       // site-major, 48 bytes per 5D site
     const size_t nb = ((size_t)g.N5h + 31) / 32;
-    return nb * (size_t)((24 * (prec / 8) / 16) * 512 + (prec == 16 ? 128 : 0));
+    return nb * (size_t)((24 * (prec / 8) / 16) * 512);
 }
-size_t field_bytes(const Geom& g, int prec, int nrhs, size_t* norm_off) {
-    if (norm_off) *norm_off = 0;
-    return rhs_bytes(g, prec) * nrhs;
-}
+size_t field_bytes(const Geom& g, int prec, int nrhs) { return rhs_bytes(g, prec) * nrhs; }
 
-int alloc_field(mdwf_ctx* c, int prec, int nrhs, mdwf_field** out) {
+static int make_field(mdwf_ctx* c, int prec, int nrhs, void* mem, void* meta_mem, mdwf_field** out) {
     if (prec != 64 && prec != 32 && prec != 16) MDWF_FAIL(c, MDWF_EINVAL, "prec must be 64, 32 or 16 (got %d)", prec);
     if (nrhs < 1 || nrhs > MDWF_MAX_RHS) MDWF_FAIL(c, MDWF_EINVAL, "nrhs must be in 1..%d (got %d)", MDWF_MAX_RHS, nrhs);
     mdwf_field* f = new mdwf_field;
     f->ctx = c;
     f->prec = prec;
     f->nrhs = nrhs;
-    size_t noff = 0;
-    f->bytes = field_bytes(c->g, prec, nrhs, &noff);
-    f->v = nullptr;
-    cudaError_t e = cudaMalloc(&f->v, f->bytes);
-    if (e != cudaSuccess) {
-        delete f;
-        cudaGetLastError();
-        MDWF_FAIL(c, MDWF_ENOMEM, "cudaMalloc of %zu bytes for a packed field failed: %s", f->bytes, cudaGetErrorString(e));
+    f->bytes = field_bytes(c->g, prec, nrhs);
+    f->v = mem;
+    f->meta = nullptr;
+    f->cur = 0;
+    f->rhs0 = 0;
+    f->owns = mem == nullptr;
+    f->owns_meta = false;
+    if (!mem) {
+        cudaError_t e = cudaMalloc(&f->v, f->bytes);
+        if (e != cudaSuccess) {
+            delete f;
+            cudaGetLastError();
+            MDWF_FAIL(c, MDWF_ENOMEM, "cudaMalloc of %zu bytes for a packed field failed: %s", f->bytes, cudaGetErrorString(e));
+        }
     }
-    f->n = nullptr;
+    if (prec == 16 && meta_mem) f->meta = reinterpret_cast<FieldMeta*>(meta_mem);
+    else if (prec == 16) {
+        f->owns_meta = true;
+        cudaError_t e = cudaMalloc(&f->meta, 2 * sizeof(FieldMeta));
+        if (e == cudaSuccess) e = cudaMemset(f->meta, 0, 2 * sizeof(FieldMeta));
+        if (e != cudaSuccess) {
+            if (f->owns) cudaFree(f->v);
+            delete f;
+            cudaGetLastError();
+            MDWF_FAIL(c, MDWF_ENOMEM, "cudaMalloc of field scales failed: %s", cudaGetErrorString(e));
+        }
+    }
     *out = f;
     return MDWF_OK;
 }
+int alloc_field(mdwf_ctx* c, int prec, int nrhs, mdwf_field** out) { return make_field(c, prec, nrhs, nullptr, nullptr, out); }
+int wrap_field(mdwf_ctx* c, int prec, int nrhs, void* mem, void* meta_mem, mdwf_field** out) { return make_field(c, prec, nrhs, mem, meta_mem, out); }
 void free_field(mdwf_field* f) {
     if (!f) return;
-    if (f->v) cudaFree(f->v);
+    if (f->v && f->owns) cudaFree(f->v);
+    if (f->meta && f->owns_meta) cudaFree(f->meta);
     delete f;
 }
 int temp_field(mdwf_ctx* c, int prec, int nrhs, int slot, mdwf_field** out) {
@@ -48,6 +67,16 @@ int temp_field(mdwf_ctx* c, int prec, int nrhs, int slot, mdwf_field** out) {
     return MDWF_OK;
 }
 
+ScaleRule rule_lin(const mdwf_field* out, const mdwf_field* a, double ca, const mdwf_field* b, double cb) {
+    ScaleRule r;
+    memset(&r, 0, sizeof(r));
+    if (!out || !out->meta) return r;
+    r.out = out->wmeta();
+    if (a && a->meta) { r.t[r.n].nb = a->nb(); r.t[r.n].coef = ca; ++r.n; }
+    if (b && b->meta) { r.t[r.n].nb = b->nb(); r.t[r.n].coef = cb; ++r.n; }
+    return r;
+}
+
 #define LAUNCH(kern, grid, blk, smem, ...)                              \
     do {                                                                \
         kern<<<(grid), (blk), (smem), st>>>(__VA_ARGS__);               \
@@ -57,10 +86,9 @@ int temp_field(mdwf_ctx* c, int prec, int nrhs, int slot, mdwf_field** out) {
 
 template <typename K, typename A>
 static int launch_big_smem(mdwf_ctx* c, K kern, int grid, int blk, size_t smem, cudaStream_t st, const A& a) {
-    static std::set<const void*> raised;
-    if (smem > 48 * 1024 && !raised.count((const void*)kern)) {
+    if (smem > 48 * 1024 && !c->attr_raised.count((const void*)kern)) {
         MDWF_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        raised.insert((const void*)kern);
+        c->attr_raised.insert((const void*)kern);
     }
     kern<<<grid, blk, smem, st>>>(c->g, a);
     MDWF_CUDA(c, cudaGetLastError());
@@ -78,6 +106,7 @@ template <typename S> static size_t g_smem(mdwf_ctx* c, bool useG) {
 
 int launch_ls(mdwf_ctx* c, int prec, LsArgs& a, cudaStream_t st) {
     const int grid = c->nblk_cls[cls_of(prec)] * a.rl.nact, blk = c->blk_cls[cls_of(prec)];
+    if (a.partial) c->partial_nblk = c->nblk_cls[cls_of(prec)];
     switch (prec) {
         case 64: return launch_big_smem(c, ls_kernel<double>, grid, blk, g_smem<double>(c, a.op.kind != 0), st, a);
         case 32: return launch_big_smem(c, ls_kernel<float>, grid, blk, g_smem<float>(c, a.op.kind != 0), st, a);
@@ -104,7 +133,7 @@ int launch_hop(mdwf_ctx* c, int prec, int recon, int dagger, int fused, HopArgs&
         (k ? r.e1 : r.e0) = e;
     }
     const double w = prec / 8.0, n5 = (double)c->g.N5h * a.nact;
-    const double pass = 24.0 * w + (prec == 16 ? 4.0 : 0.0);
+    const double pass = 24.0 * w;
     r.cls = prec == 16 ? 0 : prec == 32 ? 1 : 2;
     r.bytes = (2.0 + (a.xin.v ? 1.0 : 0.0)) * pass * n5 + 8.0 * recon * w * c->g.Vh;
     r.flops = 1320.0 * n5;
@@ -120,6 +149,7 @@ static int axpby_b(mdwf_ctx* c, int pb, AxpbyArgs& a, cudaStream_t st) {
     const int cls = sizeof(SO) == 2 ? 0 : sizeof(SO) == 4 ? 1 : 2;      // blocked like the output's storage class
     const int grid = c->nblk_cls[cls] * a.rl.nact, blk = c->blk_cls[cls];
     const size_t smem = (size_t)blk * sizeof(double);
+    if (a.partial) c->partial_nblk = c->nblk_cls[cls];
     switch (pb) {
         case 64: LAUNCH((axpby_kernel<SO, SA, double>), grid, blk, smem, c->g, a); return MDWF_OK;
         case 32: LAUNCH((axpby_kernel<SO, SA, float>), grid, blk, smem, c->g, a); return MDWF_OK;
@@ -148,15 +178,16 @@ int launch_axpby(mdwf_ctx* c, int po, int pa, int pb, AxpbyArgs& a, cudaStream_t
 int launch_cg_xr(mdwf_ctx* c, int prec_x, int prec, CgXrArgs& a, cudaStream_t st) {
     const int grid = c->nblk_cls[cls_of(prec)] * a.rl.nact, blk = c->blk_cls[cls_of(prec)];
     const size_t smem = (size_t)blk * sizeof(double);
+    c->partial_nblk = c->nblk_cls[cls_of(prec)];
     if (prec == 64 && prec_x == 64) { LAUNCH((cg_update_xr_kernel<double, double>), grid, blk, smem, c->g, a); return MDWF_OK; }
     if (prec == 32 && prec_x == 32) { LAUNCH((cg_update_xr_kernel<float, float>), grid, blk, smem, c->g, a); return MDWF_OK; }
     if (prec == 16 && prec_x == 32) { LAUNCH((cg_update_xr_kernel<float, __half>), grid, blk, smem, c->g, a); return MDWF_OK; }
-    if (prec == 16 && prec_x == 16) { LAUNCH((cg_update_xr_kernel<__half, __half>), grid, blk, smem, c->g, a); return MDWF_OK; }
     MDWF_FAIL(c, MDWF_EINVAL, "unsupported CG precision pair x=%d, r=%d", prec_x, prec);
 }
 
 int launch_cg_p(mdwf_ctx* c, int prec, CgPArgs& a, cudaStream_t st) {
     const int grid = c->nblk_cls[cls_of(prec)] * a.rl.nact, blk = c->blk_cls[cls_of(prec)];
+    if (a.partial) c->partial_nblk = c->nblk_cls[cls_of(prec)];
     switch (prec) {
         case 64: return launch_big_smem(c, cg_update_p_kernel<double>, grid, blk, g_smem<double>(c, a.op.kind != 0), st, a);
         case 32: return launch_big_smem(c, cg_update_p_kernel<float>, grid, blk, g_smem<float>(c, a.op.kind != 0), st, a);
@@ -165,12 +196,13 @@ int launch_cg_p(mdwf_ctx* c, int prec, CgPArgs& a, cudaStream_t st) {
     MDWF_FAIL(c, MDWF_EINVAL, "bad precision %d", prec);
 }
 
-int launch_finish(mdwf_ctx* c, int prec, const RhsList& rl, double* out, double* out2, cudaStream_t st) {
+int launch_finish(mdwf_ctx* c, const RhsList& rl, double* out, double* out2, cudaStream_t st, double* nb) {
     FinishArgs f;
     f.partial = c->partial;
-    f.nblk = c->nblk_cls[cls_of(prec)];
+    f.nblk = c->partial_nblk;
     f.out = out;
     f.out2 = out2;
+    f.nb = nb;
     f.rl = rl;
     finish_sum_kernel<<<rl.nact, 256, 0, st>>>(f);
     MDWF_CUDA(c, cudaGetLastError());
@@ -180,6 +212,23 @@ int launch_finish(mdwf_ctx* c, int prec, const RhsList& rl, double* out, double*
 
 int launch_pack(mdwf_ctx* c, int prec, bool unpack, PackArgs& a, cudaStream_t st) {
     dim3 grid((c->g.N5h + 255) / 256, a.nrhs);
+    if (prec == 16 && !unpack) {
+        // the scale of an fp16 field follows from its 2-norm: measure it first (R11).  a.sr.out is set by the caller.
+        if ((size_t)grid.x > c->partial_cap) MDWF_FAIL(c, MDWF_EINVAL, "internal: partial buffer too small for the pack norm");
+        PackArgs n = a;
+        n.partial = c->partial;
+        pack_norm_kernel<<<grid, 256, 256 * sizeof(double), st>>>(c->g, n);
+        MDWF_CUDA(c, cudaGetLastError());
+        c->launches++;
+        c->partial_nblk = grid.x;
+        RhsList rl = all_rhs(a.nrhs);
+        double* dn = c->dscal + 64 * 7;
+        if (a.rhs0 != 0) MDWF_FAIL(c, MDWF_EINVAL, "internal: fp16 pack with a rhs offset");
+        int rc = launch_finish(c, rl, dn, nullptr, st);
+        if (rc) return rc;
+        a.sr.n = 1;
+        a.sr.t[0].nb = dn; a.sr.t[0].num = nullptr; a.sr.t[0].den = nullptr; a.sr.t[0].coef = 1.0009765625; a.sr.t[0].sq = 1;
+    }
 #define PK(S, U) pack_kernel<S, U><<<grid, 256, 0, st>>>(c->g, a)
     if (prec == 64) { if (unpack) PK(double, true); else PK(double, false); }
     else if (prec == 32) { if (unpack) PK(float, true); else PK(float, false); }
@@ -195,9 +244,8 @@ int launch_pack(mdwf_ctx* c, int prec, bool unpack, PackArgs& a, cudaStream_t st
 
 mdwf::SpinorView mdwf_field::view() const {
     mdwf::SpinorView s;
-    s.v = v;
-    s.n = nullptr;
     s.rs = (long long)(bytes / nrhs);
-    s.rn = 0;
+    s.v = reinterpret_cast<char*>(v) - (long long)rhs0 * s.rs;
+    s.m = rmeta();
     return s;
 }

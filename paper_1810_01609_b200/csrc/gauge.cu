@@ -3,7 +3,6 @@
 // per (parity of the base site, mu): vec[c][xh] in {fp64,fp32,fp16} x {18,12,8 reals} (formats: SURVEY A12).
 // The boundary sign is never stored (the 8/12-real formats need an SU(3) matrix); hop_kernel applies it.
 #include "mdwf_host.h"
-#include <cstdlib>
 
 namespace mdwf {
 
@@ -56,37 +55,10 @@ __global__ void __launch_bounds__(256) gauge_pack_kernel(const Geom g, const Gau
     }
 }
 
-// "Prepared" stencil links for fp16 storage (hop kernel): for every output site of parity `par` and leg
-// l the link exactly as hop_kernel's staging would produce it from the packed fp16 format (so results are
-// bit-identical with and without this table), as 20 fp32, plus the neighbour half-index.  Trades 640 B of link
-// traffic per 4D site and launch for ~240 fewer instructions per thread.  Experimental, off by default (see
-// pack_gauge).
-template <int R>
-__global__ void __launch_bounds__(256) gauge_prepare_kernel(const Geom g, GaugeView gv, float* prep, int* nbr, int par) {
-    const int task = blockIdx.x * blockDim.x + threadIdx.x;
-    if (task >= g.Vh * 8) return;
-    const int xh = task >> 3, l = task & 7;
-    SiteCoord c;
-    uint32_t row, xx, r2, y, t, z;
-    g.dXH.divmod((uint32_t)xh, row, xx);
-    g.dY.divmod(row, r2, y);
-    g.dZ.divmod(r2, t, z);
-    c.xh = xh; c.xx = xx; c.y = y; c.z = z; c.t = t;
-    c.o = (par + y + z + t) & 1;
-    float V[MDWF_LROW];
-    const int n = stage_link<__half, R>(g, gv, par, c, l, V);
-    float4* dst = reinterpret_cast<float4*>(prep) + (long long)task * 5;
-#pragma unroll
-    for (int q = 0; q < 5; ++q) dst[q] = make_float4(V[4 * q], V[4 * q + 1], V[4 * q + 2], V[4 * q + 3]);
-    nbr[task] = n;
-}
-
 void free_gauge(GaugeSet* gs) {
     for (int p = 0; p < 2; ++p) {
         if (gs->v[p]) cudaFree(gs->v[p]);
-        if (gs->prep[p]) cudaFree(gs->prep[p]);
-        if (gs->nbr[p]) cudaFree(gs->nbr[p]);
-        gs->v[p] = nullptr; gs->prep[p] = nullptr; gs->nbr[p] = nullptr;
+        gs->v[p] = nullptr;
     }
 }
 
@@ -115,8 +87,6 @@ int pack_gauge(mdwf_ctx* c, const void* U, int prec, int recon, GaugeSet* gs, cu
     gs->recon = recon;
     gs->bytes_per_parity = (size_t)4 * ngv * c->g.Vh * vbytes;
     gs->v[0] = gs->v[1] = nullptr;
-    gs->prep[0] = gs->prep[1] = nullptr;
-    gs->nbr[0] = gs->nbr[1] = nullptr;
     int* bad = nullptr;
     for (int p = 0; p < 2; ++p) {
         cudaError_t e = cudaMalloc(&gs->v[p], gs->bytes_per_parity);
@@ -148,29 +118,6 @@ int pack_gauge(mdwf_ctx* c, const void* U, int prec, int recon, GaugeSet* gs, cu
         snprintf(b, sizeof(b), "8-real link format cannot represent %d links with |U01|^2+|U02|^2 -> 0 (SURVEY A12); use recon 12 or 18", nbad);
         c->err = b;
         rc = MDWF_EINVAL;
-    }
-    // opt-in only: measured SLOWER on B200 (48^3x64x10 fp16 hop 2.58 ms vs 2.26 ms, profiles/README.md): the kernel is
-    // latency/L2-bound rather than purely issue-bound, so 640 B/site of extra link traffic costs more than the ~240
-    // instructions per thread it saves.
-    if (rc == MDWF_OK && prec == 16 && getenv("MDWF_PREPARED_LINKS")) {
-        GaugeView gv;
-        gv.v[0] = gs->v[0]; gv.v[1] = gs->v[1];
-        gv.prep[0] = gv.prep[1] = nullptr; gv.nbr[0] = gv.nbr[1] = nullptr;
-        const int ntask = c->g.Vh * 8;
-        for (int p = 0; p < 2 && rc == MDWF_OK; ++p) {
-            if (cudaMalloc(&gs->prep[p], (size_t)ntask * 80) != cudaSuccess || cudaMalloc(&gs->nbr[p], (size_t)ntask * 4) != cudaSuccess) {
-                cudaGetLastError();
-                c->err = "cudaMalloc of prepared links failed";
-                rc = MDWF_ENOMEM;
-                break;
-            }
-            const int grid = (ntask + 255) / 256;
-            if (recon == 18) gauge_prepare_kernel<18><<<grid, 256, 0, st>>>(c->g, gv, gs->prep[p], gs->nbr[p], p);
-            else if (recon == 12) gauge_prepare_kernel<12><<<grid, 256, 0, st>>>(c->g, gv, gs->prep[p], gs->nbr[p], p);
-            else gauge_prepare_kernel<8><<<grid, 256, 0, st>>>(c->g, gv, gs->prep[p], gs->nbr[p], p);
-            if (cudaGetLastError() != cudaSuccess) { c->err = "gauge_prepare_kernel launch failed"; rc = MDWF_ECUDA; }
-            c->launches++;
-        }
     }
     if (rc != MDWF_OK) free_gauge(gs);
     return rc;

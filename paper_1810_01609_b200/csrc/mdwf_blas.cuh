@@ -21,6 +21,7 @@ struct LsArgs {
     double* partial;
     int write;
     RhsList rl;
+    ScaleRule sr;       // fp16 output only
 };
 template <typename S>
 __global__ void __launch_bounds__(256) ls_kernel(const Geom g, const LsArgs a) {
@@ -46,7 +47,10 @@ __global__ void __launch_bounds__(256) ls_kernel(const Geom g, const LsArgs a) {
 #pragma unroll
         for (int i = 0; i < 24; ++i) acc[i] *= ch;
     }
-    if (live && a.write) store_spinor<S>(a.out, rhs, idx, g.N5h, acc);
+    if (a.write) {
+        const T oinv = block_out_scale<S>(a.sr, rhs, tile == 0);
+        if (live) store_spinor<S>(a.out, rhs, idx, g.N5h, acc, oinv);
+    }
     if (a.partial != nullptr) {
         double s2 = 0.0;
         if (live) {
@@ -64,6 +68,7 @@ struct AxpbyArgs {
     double ca, cb;
     double* partial;
     RhsList rl;
+    ScaleRule sr;       // fp16 output only
 };
 template <typename SO, typename SA, typename SB>
 __global__ void __launch_bounds__(256) axpby_kernel(const Geom g, const AxpbyArgs p) {
@@ -73,6 +78,7 @@ __global__ void __launch_bounds__(256) axpby_kernel(const Geom g, const AxpbyArg
     const int idx = tile * blockDim.x + threadIdx.x;
     const bool live = idx < g.N5h;
     double s2 = 0.0;
+    const TO oinv = block_out_scale<SO>(p.sr, rhs, tile == 0);
     if (live) {
         double o[24];
 #pragma unroll
@@ -95,7 +101,7 @@ __global__ void __launch_bounds__(256) axpby_kernel(const Geom g, const AxpbyArg
             w[i] = (TO)o[i];
             s2 += o[i] * o[i];
         }
-        store_spinor<SO>(p.out, rhs, idx, g.N5h, w);
+        store_spinor<SO>(p.out, rhs, idx, g.N5h, w, oinv);
     }
     if (p.partial != nullptr)
         block_sum_store(s2, smem_raw, p.partial + (long long)slot * (gridDim.x / p.rl.nact) + tile);
@@ -108,6 +114,7 @@ struct CgXrArgs {
     const double* pAp;    // [64]
     double* partial;
     RhsList rl;
+    ScaleRule sr;         // fp16 r only: scale of the updated r
 };
 template <typename SX, typename S>
 __global__ void __launch_bounds__(256) cg_update_xr_kernel(const Geom g, const CgXrArgs a) {
@@ -118,6 +125,7 @@ __global__ void __launch_bounds__(256) cg_update_xr_kernel(const Geom g, const C
     const int idx = tile * blockDim.x + threadIdx.x;
     const bool live = idx < g.N5h;
     double s2 = 0.0;
+    const T oinv = block_out_scale<S>(a.sr, rhs, tile == 0);
     if (live) {
         const double alpha_d = a.rr[rhs] / a.pAp[rhs];
         T pv[24], rv[24], av[24];
@@ -135,7 +143,7 @@ __global__ void __launch_bounds__(256) cg_update_xr_kernel(const Geom g, const C
             s2 += (double)rv[i] * (double)rv[i];
         }
         store_spinor<SX>(a.x, rhs, idx, g.N5h, xv);
-        store_spinor<S>(a.r, rhs, idx, g.N5h, rv);
+        store_spinor<S>(a.r, rhs, idx, g.N5h, rv, oinv);
     }
     block_sum_store(s2, smem_raw, a.partial + (long long)slot * (gridDim.x / a.rl.nact) + tile);
 }
@@ -147,7 +155,9 @@ struct CgPArgs {
     LsOp op;
     const double* rr_new;
     const double* rr_old;
+    double* partial;      // optional |p_new|^2 partials (fp16: refreshes p's norm bound)
     RhsList rl;
+    ScaleRule sr_p, sr_q; // fp16 only: scales of the updated p and of q
 };
 template <typename S>
 __global__ void __launch_bounds__(256) cg_update_p_kernel(const Geom g, const CgPArgs a) {
@@ -159,6 +169,7 @@ __global__ void __launch_bounds__(256) cg_update_p_kernel(const Geom g, const Cg
     T pv[24];
 #pragma unroll
     for (int i = 0; i < 24; ++i) pv[i] = 0;
+    const T oinv_p = block_out_scale<S>(a.sr_p, rhs, tile == 0);
     if (live) {
         const T beta = (T)(a.rr_new[rhs] / a.rr_old[rhs]);
         T rv[24];
@@ -166,11 +177,19 @@ __global__ void __launch_bounds__(256) cg_update_p_kernel(const Geom g, const Cg
         load_spinor<S>(a.r, rhs, idx, g.N5h, rv);
 #pragma unroll
         for (int i = 0; i < 24; ++i) pv[i] = rv[i] + beta * pv[i];
-        store_spinor<S>(a.p, rhs, idx, g.N5h, pv);
+        store_spinor<S>(a.p, rhs, idx, g.N5h, pv, oinv_p);
+    }
+    if (a.partial != nullptr) {
+        double s2 = 0.0;
+#pragma unroll
+        for (int i = 0; i < 24; ++i) s2 += (double)pv[i] * (double)pv[i];
+        block_sum_store(s2, smem_raw, a.partial + (long long)slot * (gridDim.x / a.rl.nact) + tile);
+        __syncthreads();
     }
     if (a.op.kind != 0) {
         apply_ls<T>(pv, a.op, g.Ls, smem_raw);
-        if (live) store_spinor<S>(a.q, rhs, idx, g.N5h, pv);
+        const T oinv_q = block_out_scale<S>(a.sr_q, rhs, tile == 0);
+        if (live) store_spinor<S>(a.q, rhs, idx, g.N5h, pv, oinv_q);
     }
 }
 
@@ -180,6 +199,7 @@ struct FinishArgs {
     int nblk;
     double* out;        // [64] by rhs id
     double* out2;       // optional second destination (e.g. host-mapped), may be nullptr
+    double* nb;         // optional: norm bound of the fp16 field that was just measured, nb[rhs] = sqrt(sum) (1 + 2^-9)
     RhsList rl;
 };
 static __global__ void __launch_bounds__(256) finish_sum_kernel(const FinishArgs a) {
@@ -197,6 +217,7 @@ static __global__ void __launch_bounds__(256) finish_sum_kernel(const FinishArgs
     if (threadIdx.x == 0) {
         a.out[rhs] = red[0];
         if (a.out2) a.out2[rhs] = red[0];
+        if (a.nb) a.nb[rhs] = sqrt(red[0]) * 1.001953125;
     }
 }
 
@@ -207,6 +228,8 @@ struct PackArgs {
     long long Vc;           // Vh or V4
     int full, par, nrhs;
     int rhs0;               // packed rhs index = rhs0 + r for canonical rhs r
+    double* partial;        // NORM pass only: [nrhs][gridDim.x] sums of squares of the canonical data
+    ScaleRule sr;           // fp16 pack only
 };
 __device__ __forceinline__ long long canon_site(const Geom& g, int full, int par, int xh) {
     if (!full) return xh;
@@ -217,11 +240,32 @@ __device__ __forceinline__ long long canon_site(const Geom& g, int full, int par
     const int o = (par + y + z + t) & 1;
     return 2ll * xh + o;
 }
+// fp16 packing needs |field|_2 before it can choose the scale: first pass over the canonical data
+static __global__ void __launch_bounds__(256) pack_norm_kernel(const Geom g, const PackArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int rhs = blockIdx.y;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    double s2 = 0.0;
+    if (idx < g.N5h) {
+        uint32_t xh, s;
+        g.dLs.divmod((uint32_t)idx, xh, s);
+        const long long xs = canon_site(g, a.full, a.par, (int)xh);
+        const double* c = a.canon + (((long long)rhs * g.Ls + s) * a.Vc + xs) * 24;
+#pragma unroll
+        for (int i = 0; i < 12; ++i) {
+            const double2 t = reinterpret_cast<const double2*>(c)[i];
+            s2 += t.x * t.x + t.y * t.y;
+        }
+    }
+    block_sum_store(s2, smem_raw, a.partial + (long long)rhs * gridDim.x + blockIdx.x);
+}
 template <typename S, bool UNPACK>
 __global__ void __launch_bounds__(256) pack_kernel(const Geom g, const PackArgs a) {
     typedef typename Store<S>::real T;
     const int rhs = blockIdx.y;
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    T oinv = 1;
+    if (!UNPACK) oinv = block_out_scale<S>(a.sr, a.rhs0 + rhs, blockIdx.x == 0);
     if (idx >= g.N5h) return;
     uint32_t xh, s;
     g.dLs.divmod((uint32_t)idx, xh, s);
@@ -239,7 +283,7 @@ __global__ void __launch_bounds__(256) pack_kernel(const Geom g, const PackArgs 
             v[2 * i] = (T)t.x;
             v[2 * i + 1] = (T)t.y;
         }
-        store_spinor<S>(a.f, a.rhs0 + rhs, idx, g.N5h, v);
+        store_spinor<S>(a.f, a.rhs0 + rhs, idx, g.N5h, v, oinv);
     }
 }
 

@@ -2,12 +2,17 @@
 // product path (sm_100a).  Private to csrc/.  Shares nothing with oracle/.
 //
 // Packed layouts:
-//   spinor, one parity, one rhs:  blocks of 32 consecutive 5D sites, each block = vec[c][lane] c = 0..NV-1,
-//        16-byte vectors (+ 32 fp32 scales for fp16); 5D site idx = xh*Ls + s (s fastest)
-//        fp64: NV = 12 x double2     fp32: NV = 6 x float4     fp16: NV = 3 x (8 x half) + float norm[xh][s]
+//   spinor fp64/fp32, one parity, one rhs:  blocks of 32 consecutive 5D sites, each block = vec[c][lane]
+//        c = 0..NV-1, 16-byte vectors; 5D site idx = xh*Ls + s (s fastest)
+//        fp64: NV = 12 x double2     fp32: NV = 6 x float4
 //        reals inside a site are in canonical order r = ((spin*3 + colour)*2 + reim), vector c holds
 //        r = c*RPV .. c*RPV+RPV-1.  A thread owns one 5D site idx = xh*Ls + s (s fastest), so a warp
-//        reads 512 contiguous bytes per vector index.  rhs are separate fields (stride in vectors).
+//        reads 512 contiguous bytes per vector index.  rhs are separate fields (stride in bytes).
+//   spinor fp16 ("16-bit storage, single-precision computation"; reading R11):
+//        site-major, 48 bytes per 5D site: half[colour 3][spin 4][re,im] -- one 16-byte chunk per colour, so
+//        that (a) the Ls slices of a 4D site are Ls*48 contiguous bytes (one bulk copy into shared memory) and
+//        (b) an ldmatrix row (16 bytes) is a K-slice of the tensor-core stencil whose lane <-> spin mapping is
+//        regular (mdwf_hop16.cuh).  One power-of-two fp32 scale per (field, rhs): value = e * half.
 //   gauge, per (site parity, mu): vec[c][xh]   fp64: double2 x ceil(R/2), fp32: float4 x ceil(R/4),
 //        fp16: 4 x half (8 bytes) x ceil(R/4);  R = 18 | 12 | 8 reals.
 #pragma once
@@ -61,30 +66,60 @@ struct Geom {
     FastDiv dntc;
     FastDiv dtxh, dty, dtz;             // in-tile decode
     FastDiv dnTx, dnTy, dnTzs, dnTt;    // tile-index decode: tiles per row, per column, per slab depth, per T
-    // compact 4D tiles with shared-memory staged neighbours (mdwf_hop_tile.cuh); q4nsite == 0 -> not available.
-    // q4L: box extents in lattice sites; tables per parity pattern of the box origin: packed local coordinates of
-    // the output sites, of the input slots (+1, so the halo fits), and the slot of each of the 8 legs.
-    int q4L[4], q4nsite, q4nslot;
-    const int* q4out[2];
-    const int* q4slot[2];
-    const unsigned char* q4nbr[2];
-    FastDiv q4dTx, q4dTy, q4dTzs, q4dTt;
 };
+
+// fp16 fields carry, per rhs, a power-of-two scale e (value = e * stored half) and a bound nb >= |field|_2 from which
+// the scale of whatever is computed from the field is derived ON THE DEVICE (no host round trip): a kernel that writes
+// an fp16 field evaluates a ScaleRule  nb_out = sum_i coef_i |num_i/den_i| (sq_i ? sqrt(nb_i) : nb_i)  -- operator-norm
+// bounds times the inputs' bounds, refreshed by measured norms wherever a reduction exists -- and stores with
+// e_out = 2^ceil(log2(nb_out / 2^15)), so |stored| <= |field|_2 / e_out <= 2^15 can never overflow a half.
+struct FieldMeta {
+    float e[64];
+    double nb[64];
+};
+struct ScaleTerm {
+    const double* nb;      // [64] by rhs id: a norm bound, or (sq != 0) a squared norm
+    const double* num;     // optional device scalars [64]: the term is multiplied by |num/den|
+    const double* den;
+    double coef;
+    int sq;
+};
+struct ScaleRule {
+    ScaleTerm t[3];
+    int n;                 // 0: the output is not an fp16 field
+    FieldMeta* out;        // meta slot of the output field (written by one thread per rhs)
+};
+__device__ __forceinline__ float eval_scale(const ScaleRule& r, int rhs, bool write) {
+    double nb = 0.0;
+    for (int i = 0; i < r.n; ++i) {
+        const ScaleTerm& t = r.t[i];
+        double v = t.nb[rhs];
+        if (t.sq) v = sqrt(fmax(v, 0.0));
+        double s = t.coef;
+        if (t.num) s *= fabs(t.num[rhs]);
+        if (t.den) s /= fabs(t.den[rhs]);
+        nb += fabs(s) * v;
+    }
+    float e = 1.0f;
+    if (nb > 1e-300 && nb < 1e300) {
+        int k;
+        frexp(nb * (1.0 / 32768.0), &k);     // nb/2^15 = m 2^k, m in [0.5, 1)  ->  2^k >= nb/2^15
+        k = k < -120 ? -120 : k > 120 ? 120 : k;
+        e = (float)ldexp(1.0, k);
+    }
+    if (write && r.out) { r.out->e[rhs] = e; r.out->nb[rhs] = nb; }
+    return e;
+}
 
 // one packed spinor field set (nrhs fields of one parity)
 struct SpinorView {
     void* v;          // vectors
-    float* n;         // fp16 only: per 5D-site scale
-    long long rs;     // rhs stride in BYTES (= ceil(N5h/32) * block bytes)
-    long long rn;     // rhs stride in norms (= N5h)
+    FieldMeta* m;     // fp16 only: scales / norm bounds of the CURRENT content (read side)
+    long long rs;     // rhs stride in BYTES
 };
 
 struct GaugeView {
     const void* v[2];   // per parity of the link's base site; [mu][c][xh] vectors
-    // optional "prepared" stencil links (fp16 storage only): per OUTPUT parity, per site the 8 legs as 20 fp32 each
-    // (reconstructed, daggered for backward legs, bc sign folded) and the 8 neighbour half-indices
-    const float4* prep[2];
-    const int* nbr[2];
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -124,9 +159,10 @@ __device__ __forceinline__ uint32_t f2h(float a, float b) {
 
 // Blocked layout: 32 consecutive 5D sites form one block of NV rows of 32 x 16 bytes (+ 32 fp32 scales for
 // fp16), so all vectors of a site sit within BLK bytes (one DRAM page, constant offsets between rows).
-template <typename S> struct Blk { static constexpr int BYTES = Store<S>::NV * 512 + (Store<S>::HALF ? 128 : 0); };
+template <typename S> struct Blk { static constexpr int BYTES = Store<S>::NV * 512; };
 template <typename S>
 __device__ __forceinline__ const char* site_ptr(const SpinorView& f, int r, int idx) {
+    if (Store<S>::HALF) return reinterpret_cast<const char*>(f.v) + (long long)r * f.rs + (long long)idx * 48;
     return reinterpret_cast<const char*>(f.v) + (long long)r * f.rs + (long long)(idx >> 5) * Blk<S>::BYTES + (idx & 31) * 16;
 }
 
@@ -166,13 +202,15 @@ template <>
 __device__ __forceinline__ void load_raw<__half>(const SpinorView& f, int r, int idx, int N5h, float v[24],
                                                  float& scale) {
     const char* p = site_ptr<__half>(f, r, idx);
-    scale = __ldg(reinterpret_cast<const float*>(p - (idx & 31) * 12 + 3 * 512));
+    scale = f.m->e[r];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        uint4 t = ldg(reinterpret_cast<const uint4*>(p + c * 512));
+    for (int c = 0; c < 3; ++c) {        // chunk c = colour c: spins 0..3 (re, im)
+        uint4 t = ldg(reinterpret_cast<const uint4*>(p + c * 16));
         float2 a = h2f(t.x), b = h2f(t.y), cc = h2f(t.z), d = h2f(t.w);
-        v[8 * c] = a.x; v[8 * c + 1] = a.y; v[8 * c + 2] = b.x; v[8 * c + 3] = b.y;
-        v[8 * c + 4] = cc.x; v[8 * c + 5] = cc.y; v[8 * c + 6] = d.x; v[8 * c + 7] = d.y;
+        v[(0 * 3 + c) * 2] = a.x; v[(0 * 3 + c) * 2 + 1] = a.y;
+        v[(1 * 3 + c) * 2] = b.x; v[(1 * 3 + c) * 2 + 1] = b.y;
+        v[(2 * 3 + c) * 2] = cc.x; v[(2 * 3 + c) * 2 + 1] = cc.y;
+        v[(3 * 3 + c) * 2] = d.x; v[(3 * 3 + c) * 2 + 1] = d.y;
     }
 }
 
@@ -193,51 +231,50 @@ __device__ __forceinline__ void load_spinor(const SpinorView& f, int r, int idx,
 template <bool CS, typename V> __device__ __forceinline__ void st_(V* p, V v) {
     if (CS) __stcs(p, v); else *p = v;
 }
+// two floats -> packed half2, round to nearest, saturating to +-65504 (an overflow becomes a rounding error that the
+// next reliable update removes, never an Inf)
+__device__ __forceinline__ uint32_t f2h_sat(float a, float b) {
+    uint32_t r;
+    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(b), "f"(a));
+    return r;
+}
+// store the 24 reals of 5D site `idx`.  fp16 ("16-bit storage, single-precision computation"; DESIGN.md
+// R11): stored half = v * oinv with oinv = 1 / (scale of the output field, see ScaleRule); other types ignore oinv.
 template <typename S, bool CS = false>
 __device__ __forceinline__ void store_spinor(const SpinorView& f, int r, int idx, int N5h,
-                                             const typename Store<S>::real v[24]);
-template <bool CS>
-__device__ __forceinline__ void store_spinor_d(const SpinorView& f, int r, int idx, const double v[24]) {
-    char* p = const_cast<char*>(site_ptr<double>(f, r, idx));
+                                             const typename Store<S>::real v[24], typename Store<S>::real oinv = 1) {
+    char* p = const_cast<char*>(site_ptr<S>(f, r, idx));
+    if constexpr (sizeof(S) == 8) {
 #pragma unroll
-    for (int c = 0; c < 12; ++c) st_<CS>(reinterpret_cast<double2*>(p + c * 512), make_double2(v[2 * c], v[2 * c + 1]));
-}
-template <> __device__ __forceinline__ void store_spinor<double, false>(const SpinorView& f, int r, int idx, int N5h, const double v[24]) { store_spinor_d<false>(f, r, idx, v); }
-template <> __device__ __forceinline__ void store_spinor<double, true>(const SpinorView& f, int r, int idx, int N5h, const double v[24]) { store_spinor_d<true>(f, r, idx, v); }
-template <bool CS>
-__device__ __forceinline__ void store_spinor_f(const SpinorView& f, int r, int idx, const float v[24]) {
-    char* p = const_cast<char*>(site_ptr<float>(f, r, idx));
+        for (int c = 0; c < 12; ++c) st_<CS>(reinterpret_cast<double2*>(p + c * 512), make_double2(v[2 * c], v[2 * c + 1]));
+    } else if constexpr (sizeof(S) == 4) {
 #pragma unroll
-    for (int c = 0; c < 6; ++c)
-        st_<CS>(reinterpret_cast<float4*>(p + c * 512), make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]));
-}
-template <> __device__ __forceinline__ void store_spinor<float, false>(const SpinorView& f, int r, int idx, int N5h, const float v[24]) { store_spinor_f<false>(f, r, idx, v); }
-template <> __device__ __forceinline__ void store_spinor<float, true>(const SpinorView& f, int r, int idx, int N5h, const float v[24]) { store_spinor_f<true>(f, r, idx, v); }
-// fp16: per-site max-norm scale (fp32) + IEEE half mantissas in [-1,1] ("16-bit storage, single-precision
-// computation"; format choice: SURVEY A11 / DESIGN.md reading R11)
-template <bool CS>
-__device__ __forceinline__ void store_spinor_h(const SpinorView& f, int r, int idx, const float v[24]) {
-    float m = 0.f;
+        for (int c = 0; c < 6; ++c)
+            st_<CS>(reinterpret_cast<float4*>(p + c * 512), make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]));
+    } else {
 #pragma unroll
-    for (int i = 0; i < 24; ++i) m = fmaxf(m, fabsf(v[i]));
-    // sites whose largest component is below 1e-30 (far outside the support of a point source after a few
-    // iterations: denormal range, 1/m would overflow) are stored as exact zeros
-    const bool nz = m > 1e-30f;
-    const float inv = nz ? __fdividef(1.0f, m) : 0.f;
-    char* p = const_cast<char*>(site_ptr<__half>(f, r, idx));
-    st_<CS>(reinterpret_cast<float*>(p - (idx & 31) * 12 + 3 * 512), nz ? m : 0.f);
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        uint4 t;
-        t.x = f2h(v[8 * c] * inv, v[8 * c + 1] * inv);
-        t.y = f2h(v[8 * c + 2] * inv, v[8 * c + 3] * inv);
-        t.z = f2h(v[8 * c + 4] * inv, v[8 * c + 5] * inv);
-        t.w = f2h(v[8 * c + 6] * inv, v[8 * c + 7] * inv);
-        st_<CS>(reinterpret_cast<uint4*>(p + c * 512), t);
+        for (int c = 0; c < 3; ++c) {      // chunk c = colour c: spins 0..3 (re, im)
+            uint4 t;
+            t.x = f2h_sat(v[(0 * 3 + c) * 2] * oinv, v[(0 * 3 + c) * 2 + 1] * oinv);
+            t.y = f2h_sat(v[(1 * 3 + c) * 2] * oinv, v[(1 * 3 + c) * 2 + 1] * oinv);
+            t.z = f2h_sat(v[(2 * 3 + c) * 2] * oinv, v[(2 * 3 + c) * 2 + 1] * oinv);
+            t.w = f2h_sat(v[(3 * 3 + c) * 2] * oinv, v[(3 * 3 + c) * 2 + 1] * oinv);
+            st_<CS>(reinterpret_cast<uint4*>(p + c * 16), t);
+        }
     }
 }
-template <> __device__ __forceinline__ void store_spinor<__half, false>(const SpinorView& f, int r, int idx, int N5h, const float v[24]) { store_spinor_h<false>(f, r, idx, v); }
-template <> __device__ __forceinline__ void store_spinor<__half, true>(const SpinorView& f, int r, int idx, int N5h, const float v[24]) { store_spinor_h<true>(f, r, idx, v); }
+// Scale of an fp16 output: thread 0 evaluates the rule, everybody gets 1/e through shared memory (one barrier).
+// `writer` blocks (one per rhs) also store the new meta.  No-op (returns 1) for fp32/fp64 outputs.
+template <typename S>
+__device__ __forceinline__ typename Store<S>::real block_out_scale(const ScaleRule& sr, int rhs, bool writer) {
+    if constexpr (!Store<S>::HALF) return 1;
+    else {
+        __shared__ float s_oinv;
+        if (threadIdx.x == 0) s_oinv = 1.0f / eval_scale(sr, rhs, writer);
+        __syncthreads();
+        return s_oinv;
+    }
+}
 
 // ---------------------------------------------------------------------------------------------
 // Links.  NGV = vectors per link; U[18] = [row][col][re,im] after reconstruction.

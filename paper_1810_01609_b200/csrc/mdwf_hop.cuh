@@ -226,12 +226,6 @@ __device__ __forceinline__ void block_sum_store(double v, unsigned char* smem_ra
 #ifndef MDWF_HOP_MINB64
 #define MDWF_HOP_MINB64 2    // fp64: 128 registers, 2 blocks/SM (measured: 6.6 -> 5.8 ms on 48^3x64x10)
 #endif
-#ifndef MDWF_TILE_MINB32
-#define MDWF_TILE_MINB32 2
-#endif
-#ifndef MDWF_TILE_MINB16
-#define MDWF_TILE_MINB16 3
-#endif
 #define MDWF_LROW 20
 #define MDWF_LSITE (8 * MDWF_LROW + 4)
 template <typename T> __host__ __device__ inline size_t smem_bytes_links(int nsite) {
@@ -297,6 +291,7 @@ struct HopArgs {
     int par;                   // parity of the output sites
     int nact;                  // active rhs count; blockIdx.x = tile*nact + slot
     int rhs_list[64];
+    ScaleRule sr;              // fp16 output only (mdwf_hop16.cuh)
 };
 
 // (tile, site-in-tile) -> coordinates; see Geom for the traversal order
@@ -317,9 +312,8 @@ __device__ __forceinline__ SiteCoord decode_site(const Geom& g, int par, uint32_
     return c;
 }
 
-// Fused epilogue shared by hop_kernel and hop_tile_kernel:  out = cx * xin + ch * op(acc), streaming store, optional
-// fixed-order |out|^2 partial.  ch is folded into the s-direction coefficients and, for fp16 storage, the per-site
-// scale of xin into cx, so the xpay costs 24 FMAs.
+// Fused epilogue of hop_kernel:  out = cx * xin + ch * op(acc), streaming store, optional fixed-order |out|^2
+// partial.  ch is folded into the s-direction coefficients, so the xpay costs 24 FMAs.
 template <typename S>
 __device__ __forceinline__ void fused_epilogue(const Geom& g, const HopArgs& a, typename Store<S>::real acc[24], bool live,
                                                int rhs, int idx, int slot, int tile, unsigned char* smem_epi) {
@@ -406,19 +400,7 @@ __global__ void __launch_bounds__(256, (sizeof(S) == 8 ? MDWF_HOP_MINB64 : sizeo
     const int tile = (bq / a.nact) * g.ntc + tin;
     const int rhs = a.rhs_list[slot];
     // ---- stage the block's links and neighbour table --------------------------------------------------
-    if (Store<S>::HALF && a.g.prep[a.par] != nullptr) {
-        // prepared links: a block's sites are a consecutive xh range, so this is a coalesced copy of
-        // nsite*640 bytes (+ 32 bytes of neighbour indices per site); see stage_link()
-        const int xh0 = decode_site(g, a.par, (uint32_t)tile, 0u).xh;
-        const float4* src = a.g.prep[a.par] + (long long)xh0 * 40;
-        float4* dst = reinterpret_cast<float4*>(links);
-        for (int v = threadIdx.x; v < nsite * 40; v += blockDim.x) dst[v + v / 40] = __ldg(src + v);
-        const int* ns = a.g.nbr[a.par] + (long long)xh0 * 8;
-        for (int w = threadIdx.x; w < nsite * 8; w += blockDim.x) {
-            tab[(w >> 3) * 12 + (w & 7)] = __ldg(ns + w);
-            if ((w & 7) == 0) tab[(w >> 3) * 12 + 8] = xh0 + (w >> 3);
-        }
-    } else {
+    {
         for (int task = threadIdx.x; task < nsite * 8; task += blockDim.x) {
             const int i = task >> 3, l = task & 7;
             const SiteCoord c = decode_site(g, a.par, (uint32_t)tile, (uint32_t)i);

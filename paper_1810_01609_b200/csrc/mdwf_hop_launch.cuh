@@ -1,19 +1,16 @@
-// csrc/mdwf_hop_launch.cuh -- launcher template for hop_kernel; instantiated per storage precision in
-// hop_f64.cu / hop_f32.cu / hop_f16.cu so the three compile in parallel.
+// csrc/mdwf_hop_launch.cuh -- launcher template for hop_kernel (fp32/fp64 storage); instantiated per storage precision
+// in hop_f64.cu / hop_f32.cu so they compile in parallel.  The fp16 stencil has its own unit (hop16.cu).
 #pragma once
 #include "mdwf_host.h"
-#include "mdwf_hop_tile.cuh"
-#include <set>
 
 namespace mdwf {
 
 template <typename K>
 static inline int launch_with_smem(mdwf_ctx* c, K kern, int grid, int block, size_t smem, cudaStream_t st,
                                    const Geom& g, const HopArgs& a) {
-    static std::set<const void*> raised;
-    if (smem > 48 * 1024 && !raised.count((const void*)kern)) {
+    if (smem > 48 * 1024 && !c->attr_raised.count((const void*)kern)) {
         MDWF_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        raised.insert((const void*)kern);
+        c->attr_raised.insert((const void*)kern);
     }
     kern<<<grid, block, smem, st>>>(g, a);
     MDWF_CUDA(c, cudaGetLastError());
@@ -24,7 +21,7 @@ static inline int launch_with_smem(mdwf_ctx* c, K kern, int grid, int block, siz
 template <typename S, int R>
 static int launch_hop_SR(mdwf_ctx* c, int dagger, int fused, HopArgs& a, cudaStream_t st) {
     typedef typename Store<S>::real T;
-    const int cls = sizeof(S) == 2 ? 0 : sizeof(S) == 4 ? 1 : 2;
+    const int cls = sizeof(S) == 4 ? 1 : 2;
     const Geom& gh = hop_geom(c, cls, a.nact);
     const int grid = c->nblk_cls[cls] * a.nact, blk = c->blk_cls[cls];
     size_t smem = 0;
@@ -32,17 +29,7 @@ static int launch_hop_SR(mdwf_ctx* c, int dagger, int fused, HopArgs& a, cudaStr
         smem = (size_t)blk * sizeof(double);
         if (a.op.kind) smem = std::max(smem, (size_t)smem_reals_G<T>(c->g.Ls, blk) * sizeof(T));
     }
-    if (c->use_tiled && c->g.q4nsite > 0 && sizeof(T) == 4 && gh.q4nsite == gh.nsite && gh.zc % gh.q4L[2] == 0) {
-        // shared-memory staged 4D tiles; the epilogue reuses the spinor staging area
-        const size_t st_bytes = smem_bytes_tile<S>(c->g.q4nsite, c->g.q4nslot, c->g.Ls);
-        const size_t need = std::max(st_bytes, smem);
-        if (fused) {
-            if (dagger) return launch_with_smem(c, hop_tile_kernel<S, R, true, true>, grid, blk, need, st, gh, a);
-            return launch_with_smem(c, hop_tile_kernel<S, R, false, true>, grid, blk, need, st, gh, a);
-        }
-        if (dagger) return launch_with_smem(c, hop_tile_kernel<S, R, true, false>, grid, blk, need, st, gh, a);
-        return launch_with_smem(c, hop_tile_kernel<S, R, false, false>, grid, blk, need, st, gh, a);
-    }
+    if (a.partial) c->partial_nblk = c->nblk_cls[cls];
     smem += smem_bytes_links<T>(blk / c->g.Ls);
     if (fused) {
         if (dagger) return launch_with_smem(c, hop_kernel<S, R, true, true>, grid, blk, smem, st, gh, a);

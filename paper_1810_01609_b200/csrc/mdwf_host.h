@@ -3,7 +3,9 @@
 #include <string>
 #include <vector>
 #include <map>
+#include <set>
 #include <cstdio>
+#include <cstddef>
 #include "../../include/mdwf.h"
 #include "mdwf_blas.cuh"
 
@@ -14,18 +16,29 @@ struct GaugeSet {
     int prec, recon;
     void* v[2];
     size_t bytes_per_parity;
-    float* prep[2];     // prepared stencil links (prec 16 only), else nullptr
-    int* nbr[2];
 };
 
+// A packed field set.  fp16 fields own two FieldMeta slots (scales / norm bounds, mdwf_device.cuh): readers use slot
+// `cur`, the kernel that rewrites the field fills the other one (so in-place updates never race) and the host then
+// calls flip().
 struct mdwf_field {
     mdwf_ctx* ctx;
     int prec, nrhs;
     void* v;
-    float* n;
+    mdwf::FieldMeta* meta;     // device, [2]; nullptr unless prec == 16
+    int cur;
+    int rhs0;                  // rhs id of slot 0 (temporaries that serve a window of a larger batch), normally 0
     size_t bytes;
+    bool owns, owns_meta;      // v / meta were cudaMalloc'ed by alloc_field (else they live in a workspace)
     mdwf::SpinorView view() const;
+    mdwf::FieldMeta* rmeta() const { return meta ? meta + cur : nullptr; }
+    mdwf::FieldMeta* wmeta() const { return meta ? meta + (cur ^ 1) : nullptr; }
+    void flip() { if (meta) cur ^= 1; }
+    const double* nb() const { return meta ? reinterpret_cast<const double*>(reinterpret_cast<const char*>(meta + cur) + offsetof(mdwf::FieldMeta, nb)) : nullptr; }
+    double* nb_w() const { return meta ? reinterpret_cast<double*>(reinterpret_cast<char*>(meta + cur) + offsetof(mdwf::FieldMeta, nb)) : nullptr; }
 };
+
+namespace mdwf { struct Tile16Host; }
 
 struct mdwf_ctx {
     mdwf_geometry geo;
@@ -54,8 +67,15 @@ struct mdwf_ctx {
     double prof_ms[3], prof_bytes[3], prof_flops[3];
     long long prof_n[3];
     int sm_count;
-    int use_tiled;             // hop through mdwf_hop_tile.cuh (fp32/fp16 storage) when the geometry allows
-    void* q4dev[6];            // device tables of the 4D tiles (freed at destroy)
+    double lsop_norm[MAT_COUNT];   // 2-norm bounds of the s-direction operators (fp16 scale rules)
+    mdwf::Tile16Host* tile16;      // tile tables of the fp16 tensor-core stencil (built on first use)
+    int tile16_forced[4], tile16_nw;
+    std::set<const void*> attr_raised;   // kernels whose dynamic shared-memory limit was raised on THIS device
+    int partial_nblk;              // partial sums per rhs written by the last kernel that filled `partial`
+    size_t partial_cap;            // doubles per rhs in `partial`
+    void* ws;                      // solver workspace: library-owned (kept between calls) or caller-supplied
+    size_t ws_bytes;
+    bool ws_external;
     const GaugeSet* find_gauge(int prec, int recon) const {
         for (size_t i = 0; i < gauges.size(); ++i)
             if (gauges[i].prec == prec && gauges[i].recon == recon) return &gauges[i];
@@ -86,8 +106,10 @@ inline RhsList all_rhs(int n) {
     return r;
 }
 
-size_t field_bytes(const Geom& g, int prec, int nrhs, size_t* norm_off);
+size_t field_bytes(const Geom& g, int prec, int nrhs);
 int alloc_field(mdwf_ctx* c, int prec, int nrhs, mdwf_field** out);
+// a field whose vectors live at `mem` (field_bytes() bytes, 256-byte aligned) instead of their own allocation
+int wrap_field(mdwf_ctx* c, int prec, int nrhs, void* mem, void* meta_mem, mdwf_field** out);
 void free_field(mdwf_field* f);
 // cached temporaries: slot-th work field of (prec, nrhs)
 int temp_field(mdwf_ctx* c, int prec, int nrhs, int slot, mdwf_field** out);
@@ -99,9 +121,13 @@ int launch_ls(mdwf_ctx* c, int prec, LsArgs& a, cudaStream_t st);
 int launch_axpby(mdwf_ctx* c, int prec_out, int prec_a, int prec_b, AxpbyArgs& a, cudaStream_t st);
 int launch_cg_xr(mdwf_ctx* c, int prec_x, int prec, CgXrArgs& a, cudaStream_t st);
 int launch_cg_p(mdwf_ctx* c, int prec, CgPArgs& a, cudaStream_t st);
-int launch_finish(mdwf_ctx* c, int prec, const RhsList& rl, double* out, double* out2, cudaStream_t st);   // prec of the kernel that wrote the partials
+// sums the partials of the LAST kernel that wrote them (c->partial_nblk per rhs); nb: optional norm-bound slot of the
+// fp16 field that was just measured
+int launch_finish(mdwf_ctx* c, const RhsList& rl, double* out, double* out2, cudaStream_t st, double* nb = nullptr);
 inline int cls_of(int prec) { return prec == 16 ? 0 : prec == 32 ? 1 : 2; }
 int launch_pack(mdwf_ctx* c, int prec, bool unpack, PackArgs& a, cudaStream_t st);
+int pack_field(mdwf_field* f, const double* canon, int full, int par, cudaStream_t st);
+int unpack_field(const mdwf_field* f, double* canon, int full, int par, cudaStream_t st);
 const mdwf::Geom& hop_geom(mdwf_ctx* c, int cls, int nact);
 int pack_gauge(mdwf_ctx* c, const void* U, int prec, int recon, GaugeSet* gs, cudaStream_t st);
 void free_gauge(GaugeSet* gs);
@@ -113,17 +139,25 @@ struct OpCtx {
     const GaugeSet* gs;
     cudaStream_t st;
 };
-// simple helpers: out = cx*xin + ch*G*in ; out = cx*xin + ch*G*H(in)
-int op_ls(const OpCtx& o, const SpinorView& out, const SpinorView& in, int mat, const SpinorView* xin, double cx,
+// simple helpers: out = cx*xin + ch*G*in ; out = cx*xin + ch*G*H(in).  All fields of one call have precision o.prec;
+// for fp16 the scale rule of the output is built here (operator-norm bounds x the inputs' norm bounds) and the
+// output's meta slot is flipped after the launch.
+int op_ls(const OpCtx& o, mdwf_field* out, const mdwf_field* in, int mat, const mdwf_field* xin, double cx,
           double ch, const RhsList& rl, double* partial = nullptr, int write = 1);
-int op_hop(const OpCtx& o, const SpinorView& out, const SpinorView& in, int out_par, int dagger, int mat,
-           const SpinorView* xin, double cx, double ch, const RhsList& rl, double* partial = nullptr);
+int op_hop(const OpCtx& o, mdwf_field* out, const mdwf_field* in, int out_par, int dagger, int mat,
+           const mdwf_field* xin, double cx, double ch, const RhsList& rl, double* partial = nullptr);
 // Schur operator: out = Dhat/Mhat (dagger) in, parity p; t1, t2 are work fields; if partial != nullptr the
 // per-block |out|^2 sums are written there (to be finished with launch_finish)
-int op_schur(const OpCtx& o, const SpinorView& out, const SpinorView& in, int par, int dagger, int symmetric,
-             const SpinorView& t1, const SpinorView& t2, const RhsList& rl, double* partial = nullptr,
+int op_schur(const OpCtx& o, mdwf_field* out, const mdwf_field* in, int par, int dagger, int symmetric,
+             mdwf_field* t1, mdwf_field* t2, const RhsList& rl, double* partial = nullptr,
              int first_factor_done = 0);   // non-dagger only: t1 already holds A*in (fused into the CG p-update)
+// fp16 scale rule  nb_out = ca nb(a) + cb nb(b)  (b optional); n = 0 when out is not fp16
+ScaleRule rule_lin(const mdwf_field* out, const mdwf_field* a, double ca, const mdwf_field* b = nullptr, double cb = 0.0);
+int get_tile16(mdwf_ctx* c, Tile16Host** out);
+void free_tile16(Tile16Host* th);
 
 int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_opts* opts, mdwf_solve_info* info,
                cudaStream_t st, bool host_buffers);
+int solve_packed_impl(mdwf_ctx* c, mdwf_field* even, mdwf_field* odd, const mdwf_solve_opts* opts, mdwf_solve_info* info,
+                      cudaStream_t st);
 }  // namespace mdwf

@@ -253,51 +253,9 @@ static void mat4mul(const double* A, const double* B, double* C) {   // complex 
 
 }  // namespace mdwf
 
-namespace mdwf {
-// 16 independent FMA chains per thread, 4096 FMAs each: pure FFMA issue, no memory traffic
-__global__ void __launch_bounds__(256) fma_probe_kernel(float* out, float a, float b) {
-    float v[16];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) v[i] = (float)(threadIdx.x + i) * 1e-3f;
-    for (int it = 0; it < 4096; ++it) {
-#pragma unroll
-        for (int i = 0; i < 16; ++i) v[i] = __fmaf_rn(v[i], a, b);
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int i = 0; i < 16; ++i) s += v[i];
-    if (s == 123.456f) out[0] = s;      // never true: keeps the loop alive
-}
-}  // namespace mdwf
-
 using namespace mdwf;
 
 extern "C" {
-
-int mdwf_probe_fp32_fma(mdwf_ctx* c, double* tflops, void* stream) {
-    if (!c || !tflops) return MDWF_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
-    float* d = nullptr;
-    MDWF_CUDA(c, cudaMalloc(&d, 4));
-    const int grid = c->sm_count * 8;
-    cudaEvent_t e0, e1;
-    MDWF_CUDA(c, cudaEventCreate(&e0));
-    MDWF_CUDA(c, cudaEventCreate(&e1));
-    fma_probe_kernel<<<grid, 256, 0, st>>>(d, 0.999f, 1e-4f);
-    MDWF_CUDA(c, cudaEventRecord(e0, st));
-    for (int r = 0; r < 5; ++r) fma_probe_kernel<<<grid, 256, 0, st>>>(d, 0.999f, 1e-4f);
-    MDWF_CUDA(c, cudaEventRecord(e1, st));
-    MDWF_CUDA(c, cudaEventSynchronize(e1));
-    float ms = 0.f;
-    MDWF_CUDA(c, cudaEventElapsedTime(&ms, e0, e1));
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(d);
-    c->launches += 6;
-    *tflops = 5.0 * (double)grid * 256.0 * 16.0 * 4096.0 * 2.0 / (ms * 1e-3) * 1e-12;
-    return MDWF_OK;
-}
-
 
 int mdwf_wall_inject(mdwf_ctx* c, void* b5, const void* eta4, int ncol, int recon, void* stream) {
     if (!c) return MDWF_EINVAL;
@@ -315,11 +273,8 @@ int mdwf_wall_inject(mdwf_ctx* c, void* b5, const void* eta4, int ncol, int reco
     const double d = c->c5 * (4.0 - c->M5) - 1.0;
     const RhsList rl = all_rhs(ncol);
     for (int p = 0; p < 2; ++p) {
-        const SpinorView same = w[p]->view();
-        if ((rc = op_hop(o, fo->view(), w[1 - p]->view(), p, 0, -1, &same, -d, 0.5 * c->c5, rl))) return rc;
-        PackArgs a;
-        a.f = fo->view(); a.canon = (double*)b5; a.Vc = 2ll * c->g.Vh; a.full = 1; a.par = p; a.nrhs = ncol; a.rhs0 = 0;
-        if ((rc = launch_pack(c, 64, true, a, st))) return rc;
+        if ((rc = op_hop(o, fo, w[1 - p], p, 0, -1, w[p], -d, 0.5 * c->c5, rl))) return rc;
+        if ((rc = unpack_field(fo, (double*)b5, 1, p, st))) return rc;
     }
     return MDWF_OK;
 }
@@ -380,8 +335,10 @@ int mdwf_nucleon_2pt(mdwf_ctx* c, double* corr, const void* S_u1, const void* S_
     a.partial = partial;
     dim3 grid(a.nblk_t, T);
     const size_t nsm = (size_t)gpb * (5 * 144 + 16) * sizeof(double2);
-    static bool raised = false;
-    if (!raised) { MDWF_CUDA(c, cudaFuncSetAttribute(nucleon_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nsm)); raised = true; }
+    if (!c->attr_raised.count((const void*)nucleon_kernel)) {
+        MDWF_CUDA(c, cudaFuncSetAttribute(nucleon_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nsm));
+        c->attr_raised.insert((const void*)nucleon_kernel);
+    }
     nucleon_kernel<<<grid, 32 * MDWF_NUC_WARPS, nsm, st>>>(a);
     MDWF_CUDA(c, cudaGetLastError());
     nucleon_finish_kernel<<<(T + 63) / 64, 64, 0, st>>>(corr, partial, npart, T, t0);

@@ -11,6 +11,13 @@
 //   beta = rr'/rr ; p = r + beta p.
 // Reliable update (fp64): x_hi += x_lo ; x_lo = 0 ; rho = rhs - S x_hi ; r = S^dag rho ; the acceptance test is
 // on the true residual |bhat - Dhat x_hi| / |b| ( = |M5 rho| / |b| in the symmetric form), SURVEY A9.
+//
+// Memory plan.  Per rhs of a batch: three fp64 half-lattice fields (rhs, x_hi and the other
+// parity's source, which becomes the other parity's solution), five inner-precision fields (r, p, t, Ap, work) and
+// x_lo (fp32 for 16-bit inner vectors); the three fp64 temporaries of the reliable updates are shared by `nhi` <= batch
+// rhs at a time.  Everything lives in one workspace (library-owned and kept between calls, or supplied by the caller
+// through mdwf_set_workspace).  The inner loop never waits for the host: the decision to leave it is taken on the
+// device (finish_rr_kernel) and the kernels of iterations already queued behind that point turn into no-ops.
 #include "mdwf_host.h"
 #include <cmath>
 #include <algorithm>
@@ -24,23 +31,31 @@ int launch_wall_unpack(mdwf_ctx* c, double* q4, const SpinorView& in, int par, i
 
 namespace {
 
-struct Fields {
-    std::vector<mdwf_field*> all;
-    ~Fields() { for (size_t i = 0; i < all.size(); ++i) free_field(all[i]); }
-    int make(mdwf_ctx* c, int prec, int nrhs, mdwf_field** f) {
-        int rc = alloc_field(c, prec, nrhs, f);
-        if (rc == MDWF_OK) all.push_back(*f);
-        return rc;
+enum { SC_RR_A = 0, SC_RR_B = 1, SC_PAP = 2, SC_TMP = 3, SC_TMP2 = 4, SC_PP = 5, SC_STOPNR = 8, SC_MAXR = 9 };
+
+struct Arena {
+    char* base;
+    size_t cap, off;
+    void* take(size_t n) {
+        off = (off + 255) / 256 * 256;
+        void* p = base ? base + off : nullptr;
+        off += n;
+        return p;
     }
 };
 
-enum { SC_RR_A = 0, SC_RR_B = 1, SC_PAP = 2, SC_TMP = 3, SC_TMP2 = 4 };
+struct Work {
+    std::vector<mdwf_field*> all;
+    mdwf_field *rhs, *xh, *opar, *t2, *t3, *t4, *r, *p, *t, *wa, *wb, *xl;
+    bool rhs_external;      // rhs / opar are the caller's packed fields (mdwf_solve_packed)
+    ~Work() { for (size_t i = 0; i < all.size(); ++i) free_field(all[i]); }
+};
 
 struct Solver {
     mdwf_ctx* c;
     cudaStream_t st;
     OpCtx hi, lo;
-    int nb, par, sym, prec, px;
+    int nb, nhi, par, sym, prec, px;
     double tol, delta;
     int max_iter, check_every;
 
@@ -48,10 +63,10 @@ struct Solver {
     double* hsc(int k) { return c->hscal + 64 * k; }
 
     // out[rhs] (device + pinned host mirror) = sum |f|^2
-    int norm2(const OpCtx& o, const SpinorView& f, const RhsList& rl, int k) {
+    int norm2(const OpCtx& o, mdwf_field* f, const RhsList& rl, int k) {
         int rc = op_ls(o, f, f, -1, nullptr, 0.0, 1.0, rl, c->partial, 0);
         if (rc) return rc;
-        return launch_finish(c, o.prec, rl, dsc(k), hsc(k), st);
+        return launch_finish(c, rl, dsc(k), hsc(k), st);
     }
     int sync() {
         MDWF_CUDA(c, cudaStreamSynchronize(st));
@@ -59,60 +74,112 @@ struct Solver {
     }
 };
 
-size_t per_rhs_bytes(const Geom& g, int prec, int px) {
-    const size_t f64 = (size_t)g.N5h * 24 * 8;
-    const size_t flo = (size_t)g.N5h * (24 * (prec / 8) + (prec == 16 ? 4 : 0));
-    const size_t fx = (size_t)g.N5h * 24 * (px / 8);
-    return 5 * f64 + 5 * flo + fx;
+// bytes of the workspace of one batch (nb rhs in flight, nhi rhs of fp64 temporaries); own_src: rhs/opar inside
+size_t work_bytes(const Geom& g, int prec, int px, int nb, int nhi, bool own_src) {
+    auto al = [](size_t n) { return (n + 255) / 256 * 256; };
+    size_t n = 0;
+    n += (own_src ? 3 : 1) * al(field_bytes(g, 64, nb));
+    n += 3 * al(field_bytes(g, 64, nhi));
+    n += 5 * al(field_bytes(g, prec, nb));
+    n += al(field_bytes(g, px, nb));
+    n += 16 * al(2 * sizeof(FieldMeta));
+    return n + 4096;
+}
+
+int ensure_workspace(mdwf_ctx* c, size_t need) {
+    if (c->ws_bytes >= need) return MDWF_OK;
+    if (c->ws_external) MDWF_FAIL(c, MDWF_ENOMEM, "caller-supplied workspace of %zu bytes is too small (%zu needed)", c->ws_bytes, need);
+    if (c->ws) { cudaFree(c->ws); c->ws = nullptr; c->ws_bytes = 0; }
+    cudaError_t e = cudaMalloc(&c->ws, need);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        c->ws = nullptr;
+        MDWF_FAIL(c, MDWF_ENOMEM, "cudaMalloc of the %zu-byte solver workspace failed: %s", need, cudaGetErrorString(e));
+    }
+    c->ws_bytes = need;
+    return MDWF_OK;
+}
+
+int make_work(Solver& S, Work& W, mdwf_field* ext_rhs, mdwf_field* ext_opar) {
+    mdwf_ctx* c = S.c;
+    const Geom& g = c->g;
+    W.rhs_external = ext_rhs != nullptr;
+    const size_t need = work_bytes(g, S.prec, S.px, S.nb, S.nhi, !W.rhs_external);
+    int rc = ensure_workspace(c, need);
+    if (rc) return rc;
+    Arena A;
+    A.base = (char*)c->ws; A.cap = c->ws_bytes; A.off = 0;
+    auto mk = [&](int prec, int n, mdwf_field** f) -> int {
+        void* mem = A.take(field_bytes(g, prec, n));
+        void* meta = prec == 16 ? A.take(2 * sizeof(FieldMeta)) : nullptr;
+        int r2 = wrap_field(c, prec, n, mem, meta, f);
+        if (r2 == MDWF_OK) {
+            W.all.push_back(*f);
+            if (meta) MDWF_CUDA(c, cudaMemsetAsync(meta, 0, 2 * sizeof(FieldMeta), S.st));
+        }
+        return r2;
+    };
+    if (W.rhs_external) { W.rhs = ext_rhs; W.opar = ext_opar; }
+    else if ((rc = mk(64, S.nb, &W.rhs)) || (rc = mk(64, S.nb, &W.opar))) return rc;
+    if ((rc = mk(64, S.nb, &W.xh)) || (rc = mk(64, S.nhi, &W.t2)) || (rc = mk(64, S.nhi, &W.t3)) || (rc = mk(64, S.nhi, &W.t4)) ||
+        (rc = mk(S.prec, S.nb, &W.r)) || (rc = mk(S.prec, S.nb, &W.p)) || (rc = mk(S.prec, S.nb, &W.t)) ||
+        (rc = mk(S.prec, S.nb, &W.wa)) || (rc = mk(S.prec, S.nb, &W.wb)) || (rc = mk(S.px, S.nb, &W.xl)))
+        return rc;
+    if (A.off > A.cap) MDWF_FAIL(c, MDWF_ENOMEM, "internal: workspace plan exceeds its size");
+    return MDWF_OK;
+}
+
+// the rhs ids of `act` that fall into [c0, c0 + n)
+RhsList chunk_of(const RhsList& act, int c0, int n) {
+    RhsList r;
+    r.nact = 0;
+    for (int k = 0; k < 64; ++k) r.rhs[k] = 0;
+    for (int k = 0; k < act.nact; ++k)
+        if (act.rhs[k] >= c0 && act.rhs[k] < c0 + n) r.rhs[r.nact++] = act.rhs[k];
+    return r;
+}
+
+SpinorView no_view() {
+    SpinorView v;
+    v.v = nullptr; v.m = nullptr; v.rs = 0;
+    return v;
 }
 
 }  // namespace
 
-// build the packed fp64 source halves of one batch: src_kind 0: pack the canonical 5D field;
+// build the packed fp64 source halves of one batch from canonical data: src_kind 0: pack the canonical 5D field;
 // src_kind 1: wall-inject the 4D source, b5 = -D_- w = -d w + (c5/2) H w  (D_- = c5 D_W - 1)
-static int make_source(Solver& S, const double* b, int src_kind, int which_par, const SpinorView& out,
-                       const SpinorView& tmp_same, const SpinorView& tmp_other) {
+static int make_source(Solver& S, Work& W, const double* b, int src_kind, int which_par, mdwf_field* out) {
     mdwf_ctx* c = S.c;
-    const RhsList rl = all_rhs(S.nb);
-    if (src_kind == 0) {
-        PackArgs a;
-        a.f = out; a.canon = const_cast<double*>(b); a.Vc = 2ll * c->g.Vh; a.full = 1; a.par = which_par; a.nrhs = S.nb; a.rhs0 = 0;
-        return launch_pack(c, 64, false, a, S.st);
-    }
+    if (src_kind == 0) return pack_field(out, b, 1, which_par, S.st);
     int rc;
-    if ((rc = launch_wall_pack(c, tmp_same, b, which_par, S.nb, S.st))) return rc;
-    if ((rc = launch_wall_pack(c, tmp_other, b, 1 - which_par, S.nb, S.st))) return rc;
     const double d = c->c5 * (4.0 - c->M5) - 1.0;
-    return op_hop(S.hi, out, tmp_other, which_par, 0, -1, &tmp_same, -d, 0.5 * c->c5, rl);
+    const size_t x4d = (size_t)2 * c->g.Vh * 24;
+    for (int c0 = 0; c0 < S.nb; c0 += S.nhi) {          // temporaries hold nhi columns at a time
+        const int n = std::min(S.nhi, S.nb - c0);
+        W.t2->rhs0 = W.t4->rhs0 = 0;
+        if ((rc = launch_wall_pack(c, W.t2->view(), b + c0 * x4d, which_par, n, S.st))) return rc;
+        if ((rc = launch_wall_pack(c, W.t4->view(), b + c0 * x4d, 1 - which_par, n, S.st))) return rc;
+        W.t2->rhs0 = W.t4->rhs0 = c0;
+        RhsList rl = chunk_of(all_rhs(S.nb), c0, n);
+        if ((rc = op_hop(S.hi, out, W.t4, which_par, 0, -1, W.t2, -d, 0.5 * c->c5, rl))) return rc;
+    }
+    return MDWF_OK;
 }
 
-static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_opts* opts, mdwf_solve_info* info,
-                       int r0, double* t_inner_ms) {
+// The solve proper on packed fp64 halves: on entry W.rhs = b_p, W.opar = b_pbar; on exit W.xh = psi_p, W.opar = psi_pbar.
+static int solve_core(Solver& S, Work& W, mdwf_solve_info* info, int r0, double* t_inner_ms) {
     mdwf_ctx* c = S.c;
-    const Geom& g = c->g;
     const int nb = S.nb, par = S.par, sym = S.sym;
     cudaStream_t st = S.st;
     int rc;
-    Fields F;
-    mdwf_field *f_rhs, *f_x, *f_t2, *f_t3, *f_t4, *f_r, *f_p, *f_t, *f_a, *f_b, *f_xl;
-    if ((rc = F.make(c, 64, nb, &f_rhs)) || (rc = F.make(c, 64, nb, &f_x)) || (rc = F.make(c, 64, nb, &f_t2)) ||
-        (rc = F.make(c, 64, nb, &f_t3)) || (rc = F.make(c, 64, nb, &f_t4)) || (rc = F.make(c, S.prec, nb, &f_r)) ||
-        (rc = F.make(c, S.prec, nb, &f_p)) || (rc = F.make(c, S.prec, nb, &f_t)) || (rc = F.make(c, S.prec, nb, &f_a)) ||
-        (rc = F.make(c, S.prec, nb, &f_b)) || (rc = F.make(c, S.px, nb, &f_xl)))
-        return rc;
-    const SpinorView rhs = f_rhs->view(), xh = f_x->view(), t2 = f_t2->view(), t3 = f_t3->view(), t4 = f_t4->view(),
-                     r = f_r->view(), p = f_p->view(), t = f_t->view(), wa = f_a->view(), wb = f_b->view(),
-                     xl = f_xl->view();
     const RhsList all = all_rhs(nb);
-    const size_t x4d = (size_t)2 * g.Vh * 24, x5d = x4d * g.Ls;
-    const double* bsrc = b + (size_t)r0 * (opts->src_kind ? x4d : x5d);
-    SpinorView none;
-    none.v = nullptr; none.n = nullptr; none.rs = none.rn = 0;
+    mdwf_field *rhs = W.rhs, *xh = W.xh, *opar = W.opar, *t2 = W.t2, *t3 = W.t3, *t4 = W.t4, *r = W.r, *p = W.p, *t = W.t,
+               *wa = W.wa, *wb = W.wb, *xl = W.xl;
+    auto set_chunk = [&](int c0) { t2->rhs0 = t3->rhs0 = t4->rhs0 = c0; };
 
-    // ---- source: b_p -> rhs, b_pbar -> t3 ; |b|^2 ; bhat ; (sym) M5^-1 bhat ------------------------
-    if ((rc = make_source(S, bsrc, opts->src_kind, par, rhs, t2, t4))) return rc;
-    if ((rc = make_source(S, bsrc, opts->src_kind, 1 - par, t3, t2, t4))) return rc;
-    if ((rc = S.norm2(S.hi, rhs, all, SC_TMP)) || (rc = S.norm2(S.hi, t3, all, SC_TMP2)) || (rc = S.sync())) return rc;
+    // ---- |b|^2 ; bhat ; (sym) M5^-1 bhat ----------------------------------------------------------------
+    if ((rc = S.norm2(S.hi, rhs, all, SC_TMP)) || (rc = S.norm2(S.hi, opar, all, SC_TMP2)) || (rc = S.sync())) return rc;
     double bnorm[MDWF_MAX_RHS], stop_nr[MDWF_MAX_RHS], maxr[MDWF_MAX_RHS];
     int status[MDWF_MAX_RHS], iters[MDWF_MAX_RHS], nrel[MDWF_MAX_RHS];
     double tres[MDWF_MAX_RHS];
@@ -121,39 +188,59 @@ static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_o
         status[i] = -100;   // active
         iters[i] = 0; nrel[i] = 0; tres[i] = 0.0; stop_nr[i] = 0.0; maxr[i] = 0.0;
     }
-    if ((rc = op_ls(S.hi, t2, t3, MAT_AM5INV, nullptr, 0.0, 1.0, all))) return rc;
-    if ((rc = op_hop(S.hi, rhs, t2, par, 0, -1, &rhs, 1.0, 0.5, all))) return rc;           // bhat
+    for (int c0 = 0; c0 < nb; c0 += S.nhi) {
+        const RhsList rl = chunk_of(all, c0, S.nhi);
+        set_chunk(c0);
+        if ((rc = op_ls(S.hi, t2, opar, MAT_AM5INV, nullptr, 0.0, 1.0, rl))) return rc;
+        if ((rc = op_hop(S.hi, rhs, t2, par, 0, -1, rhs, 1.0, 0.5, rl))) return rc;           // bhat
+    }
     if (sym && (rc = op_ls(S.hi, rhs, rhs, MAT_M5INV, nullptr, 0.0, 1.0, all))) return rc;   // M5^-1 bhat
-    MDWF_CUDA(c, cudaMemsetAsync(f_x->v, 0, f_x->bytes, st));
-    MDWF_CUDA(c, cudaMemsetAsync(f_xl->v, 0, f_xl->bytes, st));
+    MDWF_CUDA(c, cudaMemsetAsync(xh->v, 0, xh->bytes, st));
+    MDWF_CUDA(c, cudaMemsetAsync(xl->v, 0, xl->bytes, st));
 
     RhsList act = all;
     int rrOld = SC_RR_A, rrNew = SC_RR_B;
 
     // reliable update over the active list: refreshes r (low precision), dsc(rrNew) = |r_hi|^2,
-    // tres[] / status[]; first == true: x_hi = 0 so rho = rhs.
+    // tres[] / status[]; first == true: x_hi = 0 so rho = rhs.  The fp64 temporaries serve nhi rhs at a time.
     auto reliable = [&](bool first) -> int {
         int rc2;
-        AxpbyArgs d;
-        d.out = t3; d.a = rhs; d.ca = 1.0; d.partial = sym ? nullptr : c->partial; d.rl = act;
         if (!first) {
             AxpbyArgs a;
-            a.out = xh; a.a = xh; a.b = xl; a.ca = 1.0; a.cb = 1.0; a.partial = nullptr; a.rl = act;
+            memset(&a, 0, sizeof(a));
+            a.out = xh->view(); a.a = xh->view(); a.b = xl->view(); a.ca = 1.0; a.cb = 1.0; a.partial = nullptr; a.rl = act;
             if ((rc2 = launch_axpby(c, 64, 64, S.px, a, st))) return rc2;
-            MDWF_CUDA(c, cudaMemsetAsync(f_xl->v, 0, f_xl->bytes, st));
-            if ((rc2 = op_schur(S.hi, t3, xh, par, 0, sym, t3, t2, act))) return rc2;
-            d.b = t3; d.cb = -1.0;
-        } else {
-            d.b = none; d.cb = 0.0;
+            MDWF_CUDA(c, cudaMemsetAsync(xl->v, 0, xl->bytes, st));
         }
-        if ((rc2 = launch_axpby(c, 64, 64, 64, d, st))) return rc2;                                   // rho -> t3
-        if (sym && (rc2 = op_ls(S.hi, t3, t3, MAT_M5, nullptr, 0.0, 1.0, act, c->partial, 0))) return rc2;   // |M5 rho|^2
-        if ((rc2 = launch_finish(c, 64, act, S.dsc(SC_TMP), S.hsc(SC_TMP), st))) return rc2;
-        if ((rc2 = op_schur(S.hi, t4, t3, par, 1, sym, t4, t2, act, c->partial))) return rc2;         // r = S^dag rho
-        if ((rc2 = launch_finish(c, 64, act, S.dsc(rrNew), S.hsc(rrNew), st))) return rc2;
-        AxpbyArgs cv;
-        cv.out = r; cv.a = t4; cv.b = none; cv.ca = 1.0; cv.cb = 0.0; cv.partial = nullptr; cv.rl = act;
-        if ((rc2 = launch_axpby(c, S.prec, 64, 64, cv, st))) return rc2;
+        for (int c0 = 0; c0 < nb; c0 += S.nhi) {
+            const RhsList rl = chunk_of(act, c0, S.nhi);
+            if (rl.nact == 0) continue;
+            set_chunk(c0);
+            AxpbyArgs d;
+            memset(&d, 0, sizeof(d));
+            d.out = t3->view(); d.a = rhs->view(); d.ca = 1.0; d.partial = sym ? nullptr : c->partial; d.rl = rl;
+            if (!first) {
+                if ((rc2 = op_schur(S.hi, t3, xh, par, 0, sym, t3, t2, rl))) return rc2;
+                d.b = t3->view(); d.cb = -1.0;
+            } else {
+                d.b = no_view(); d.cb = 0.0;
+            }
+            if ((rc2 = launch_axpby(c, 64, 64, 64, d, st))) return rc2;                                   // rho -> t3
+            if (sym && (rc2 = op_ls(S.hi, t3, t3, MAT_M5, nullptr, 0.0, 1.0, rl, c->partial, 0))) return rc2;   // |M5 rho|^2
+            if ((rc2 = launch_finish(c, rl, S.dsc(SC_TMP), S.hsc(SC_TMP), st))) return rc2;
+            if ((rc2 = op_schur(S.hi, t4, t3, par, 1, sym, t4, t2, rl, c->partial))) return rc2;         // r = S^dag rho
+            if ((rc2 = launch_finish(c, rl, S.dsc(rrNew), S.hsc(rrNew), st))) return rc2;
+            AxpbyArgs cv;
+            memset(&cv, 0, sizeof(cv));
+            cv.out = r->view(); cv.a = t4->view(); cv.b = no_view(); cv.ca = 1.0; cv.cb = 0.0; cv.partial = nullptr; cv.rl = rl;
+            if (r->meta) {       // scale of the fp16 residual from its measured norm
+                cv.sr.n = 1; cv.sr.out = r->wmeta();
+                cv.sr.t[0].nb = S.dsc(rrNew); cv.sr.t[0].sq = 1; cv.sr.t[0].coef = 1.001953125;
+            }
+            if ((rc2 = launch_axpby(c, S.prec, 64, 64, cv, st))) return rc2;
+        }
+        // every chunk wrote r through the same write slot: flip once
+        r->flip();
         if ((rc2 = S.sync())) return rc2;
         RhsList na;
         na.nact = 0;
@@ -177,12 +264,17 @@ static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_o
         act = na;
         return MDWF_OK;
     };
+    // fp16 only: the r slot that readers see must carry the scales of ALL rhs, also of those that are no longer
+    // active (they are never read again), so nothing else is needed after the flip above.
 
     if ((rc = reliable(true))) return rc;
     if (act.nact > 0) {
         AxpbyArgs cp;
-        cp.out = p; cp.a = r; cp.b = none; cp.ca = 1.0; cp.cb = 0.0; cp.partial = nullptr; cp.rl = act;
+        memset(&cp, 0, sizeof(cp));
+        cp.out = p->view(); cp.a = r->view(); cp.b = no_view(); cp.ca = 1.0; cp.cb = 0.0; cp.partial = nullptr; cp.rl = act;
+        cp.sr = rule_lin(p, r, 1.0);
         if ((rc = launch_axpby(c, S.prec, S.prec, S.prec, cp, st))) return rc;
+        p->flip();
         if ((rc = op_ls(S.lo, t, p, MAT_A, nullptr, 0.0, 1.0, act))) return rc;   // q = A p (later fused into the p-update)
         std::swap(rrOld, rrNew);   // dsc(rrOld) = |r_0|^2
     }
@@ -196,12 +288,20 @@ static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_o
         if (!open) { cudaEventRecord(e0, st); open = true; }
         // t = S p, pAp = |t|^2 ; Ap = S^dag t   (out may alias the first work field, see op_schur)
         if ((rc = op_schur(S.lo, t, p, par, 0, sym, t, wb, act, c->partial, 1))) break;   // t holds A p on entry
-        if ((rc = launch_finish(c, S.prec, act, S.dsc(SC_PAP), S.hsc(SC_PAP), st))) break;
+        if ((rc = launch_finish(c, act, S.dsc(SC_PAP), S.hsc(SC_PAP), st, t->nb_w()))) break;
         if ((rc = op_schur(S.lo, wa, t, par, 1, sym, wa, wb, act))) break;
         CgXrArgs u;
-        u.x = xl; u.r = r; u.p = p; u.Ap = wa; u.rr = S.dsc(rrOld); u.pAp = S.dsc(SC_PAP); u.partial = c->partial; u.rl = act;
+        memset(&u, 0, sizeof(u));
+        u.x = xl->view(); u.r = r->view(); u.p = p->view(); u.Ap = wa->view(); u.rr = S.dsc(rrOld); u.pAp = S.dsc(SC_PAP);
+        u.partial = c->partial; u.rl = act;
+        if (r->meta) {      // |r - alpha Ap| <= |r| + |alpha| |Ap|
+            u.sr.n = 2; u.sr.out = r->wmeta();
+            u.sr.t[0].nb = r->nb(); u.sr.t[0].coef = 1.0;
+            u.sr.t[1].nb = wa->nb(); u.sr.t[1].coef = 1.0; u.sr.t[1].num = S.dsc(rrOld); u.sr.t[1].den = S.dsc(SC_PAP);
+        }
         if ((rc = launch_cg_xr(c, S.px, S.prec, u, st))) break;
-        if ((rc = launch_finish(c, S.prec, act, S.dsc(rrNew), S.hsc(rrNew), st))) break;
+        r->flip();
+        if ((rc = launch_finish(c, act, S.dsc(rrNew), S.hsc(rrNew), st, r->nb_w()))) break;
         for (int k = 0; k < act.nact; ++k) iters[act.rhs[k]]++;
         bool need_update = false;
         if (++since_check >= S.check_every) {
@@ -222,14 +322,26 @@ static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_o
             cudaEventElapsedTime(&ms, e0, e1);
             *t_inner_ms += ms;
             open = false;
-            const int before = act.nact;
             if ((rc = reliable(false))) break;
-            (void)before;
             if (act.nact == 0) break;
         }
         CgPArgs q;
-        q.p = p; q.r = r; q.q = t; q.op = c->lsop[MAT_A]; q.rr_new = S.dsc(rrNew); q.rr_old = S.dsc(rrOld); q.rl = act;
+        memset(&q, 0, sizeof(q));
+        q.p = p->view(); q.r = r->view(); q.q = t->view(); q.op = c->lsop[MAT_A]; q.rr_new = S.dsc(rrNew); q.rr_old = S.dsc(rrOld); q.rl = act;
+        if (p->meta) {      // |r + beta p| <= |r| + beta |p| ; |A p| <= |A| |p| ; p's bound is then refreshed by its measured norm
+            for (int w = 0; w < 2; ++w) {
+                ScaleRule& sr = w ? q.sr_q : q.sr_p;
+                const double f = w ? c->lsop_norm[MAT_A] : 1.0;
+                sr.n = 2; sr.out = w ? t->wmeta() : p->wmeta();
+                sr.t[0].nb = S.dsc(rrNew); sr.t[0].sq = 1; sr.t[0].coef = 1.001953125 * f;
+                sr.t[1].nb = p->nb(); sr.t[1].coef = f; sr.t[1].num = S.dsc(rrNew); sr.t[1].den = S.dsc(rrOld);
+            }
+            q.partial = c->partial;
+        }
         if ((rc = launch_cg_p(c, S.prec, q, st))) break;
+        p->flip();
+        t->flip();
+        if (p->meta && (rc = launch_finish(c, act, S.dsc(SC_PP), nullptr, st, p->nb_w()))) break;
         std::swap(rrOld, rrNew);
     }
     if (open) {
@@ -243,25 +355,14 @@ static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_o
     cudaEventDestroy(e1);
     if (rc) return rc;
 
-    // ---- reconstruct psi_pbar = M5^-1 ( b_pbar + 1/2 H A psi_p ) and write the result ---------------
-    if ((rc = make_source(S, bsrc, opts->src_kind, 1 - par, t3, t2, t4))) return rc;   // b_pbar again (not kept: memory)
-    if ((rc = op_ls(S.hi, t2, xh, MAT_A, nullptr, 0.0, 1.0, all))) return rc;
-    if ((rc = op_hop(S.hi, t3, t2, 1 - par, 0, -1, &t3, 1.0, 0.5, all))) return rc;
-    if ((rc = op_ls(S.hi, t3, t3, MAT_M5INV, nullptr, 0.0, 1.0, all))) return rc;
-    if (opts->out_kind == 0) {
-        double* xo = x + (size_t)r0 * x5d;
-        PackArgs a;
-        a.canon = xo; a.Vc = 2ll * g.Vh; a.full = 1; a.nrhs = nb; a.rhs0 = 0;
-        a.f = xh; a.par = par;
-        if ((rc = launch_pack(c, 64, true, a, st))) return rc;
-        a.f = t3; a.par = 1 - par;
-        if ((rc = launch_pack(c, 64, true, a, st))) return rc;
-    } else {
-        double* xo = x + (size_t)r0 * x4d;
-        if ((rc = launch_wall_unpack(c, xo, xh, par, nb, st))) return rc;
-        if ((rc = launch_wall_unpack(c, xo, t3, 1 - par, nb, st))) return rc;
+    // ---- reconstruct psi_pbar = M5^-1 ( b_pbar + 1/2 H A psi_p ), in place in opar -----------------------
+    for (int c0 = 0; c0 < nb; c0 += S.nhi) {
+        const RhsList rl = chunk_of(all, c0, S.nhi);
+        set_chunk(c0);
+        if ((rc = op_ls(S.hi, t2, xh, MAT_A, nullptr, 0.0, 1.0, rl))) return rc;
+        if ((rc = op_hop(S.hi, opar, t2, 1 - par, 0, -1, opar, 1.0, 0.5, rl))) return rc;
     }
-    if ((rc = S.sync())) return rc;
+    if ((rc = op_ls(S.hi, opar, opar, MAT_M5INV, nullptr, 0.0, 1.0, all))) return rc;
     for (int i = 0; i < nb; ++i) {
         info->iters[r0 + i] = iters[i];
         info->reliable_updates[r0 + i] = nrel[i];
@@ -271,17 +372,36 @@ static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_o
     return MDWF_OK;
 }
 
-int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_opts* opts, mdwf_solve_info* info,
-               cudaStream_t st, bool host_buffers) {
-    if (!x || !b || !opts || !info) MDWF_FAIL(c, MDWF_EINVAL, "null argument");
-    if (nrhs < 1 || nrhs > MDWF_MAX_RHS) MDWF_FAIL(c, MDWF_EINVAL, "nrhs must be in 1..%d (got %d)", MDWF_MAX_RHS, nrhs);
+// one batch through canonical device buffers
+static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_opts* opts, mdwf_solve_info* info,
+                       int r0, double* t_inner_ms) {
+    mdwf_ctx* c = S.c;
+    const Geom& g = c->g;
+    Work W;
+    int rc = make_work(S, W, nullptr, nullptr);
+    if (rc) return rc;
+    const size_t x4d = (size_t)2 * g.Vh * 24, x5d = x4d * g.Ls;
+    const double* bsrc = b + (size_t)r0 * (opts->src_kind ? x4d : x5d);
+    if ((rc = make_source(S, W, bsrc, opts->src_kind, S.par, W.rhs))) return rc;
+    if ((rc = make_source(S, W, bsrc, opts->src_kind, 1 - S.par, W.opar))) return rc;
+    if ((rc = solve_core(S, W, info, r0, t_inner_ms))) return rc;
+    if (opts->out_kind == 0) {
+        double* xo = x + (size_t)r0 * x5d;
+        if ((rc = unpack_field(W.xh, xo, 1, S.par, S.st))) return rc;
+        if ((rc = unpack_field(W.opar, xo, 1, 1 - S.par, S.st))) return rc;
+    } else {
+        double* xo = x + (size_t)r0 * x4d;
+        if ((rc = launch_wall_unpack(c, xo, W.xh->view(), S.par, S.nb, S.st))) return rc;
+        if ((rc = launch_wall_unpack(c, xo, W.opar->view(), 1 - S.par, S.nb, S.st))) return rc;
+    }
+    return S.sync();
+}
+
+static int setup_solver(mdwf_ctx* c, Solver& S, const mdwf_solve_opts* opts, cudaStream_t st) {
     if (!(opts->tol > 0.0)) MDWF_FAIL(c, MDWF_EINVAL, "tol must be > 0");
     if (opts->parity != 0 && opts->parity != 1) MDWF_FAIL(c, MDWF_EINVAL, "parity must be 0 or 1");
     const int prec = opts->inner_prec;
     if (prec != 64 && prec != 32 && prec != 16) MDWF_FAIL(c, MDWF_EINVAL, "inner_prec must be 64, 32 or 16");
-    if (opts->src_kind == 0 && opts->out_kind == 0) { /* x may alias b */ }
-    else if (x == b) MDWF_FAIL(c, MDWF_EINVAL, "x may alias b only for 5D source and 5D solution");
-    Solver S;
     S.c = c; S.st = st;
     S.prec = prec;
     S.px = prec == 16 ? 32 : prec;
@@ -298,19 +418,46 @@ int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_o
     S.hi.gs = c->find_gauge(64, 18);
     if (!S.hi.gs) { S.hi.recon = opts->recon; S.hi.gs = c->find_gauge(64, opts->recon); }
     if (!S.hi.gs) MDWF_FAIL(c, MDWF_ESTATE, "outer fp64 gauge format (recon 18 or %d) not loaded", opts->recon);
+    return MDWF_OK;
+}
 
+// batch size and number of rhs served by the fp64 temporaries that fit in `avail` bytes (beyond `extra_per_rhs`)
+static int plan_batch(mdwf_ctx* c, const Solver& S, int nrhs, int want, size_t avail, size_t extra_per_rhs, bool own_src,
+                      int* nb_out, int* nhi_out) {
+    const Geom& g = c->g;
+    int nb = want > 0 ? std::min(want, nrhs) : nrhs;
+    for (; nb >= 1; --nb) {
+        for (int nhi = nb; nhi >= 1; nhi = nhi > 1 ? (nhi + 1) / 2 : 0) {
+            if (work_bytes(g, S.prec, S.px, nb, nhi, own_src) + extra_per_rhs * nb <= avail) { *nb_out = nb; *nhi_out = nhi; return MDWF_OK; }
+            if (nhi == 1) break;
+        }
+        if (want > 0) break;    // an explicit batch is honoured or refused
+    }
+    MDWF_FAIL(c, MDWF_ENOMEM, "not enough device memory for a batch of %d rhs (%zu bytes available)", std::max(1, want), avail);
+}
+
+static size_t avail_bytes(mdwf_ctx* c) {
+    if (c->ws_external) return c->ws_bytes;
+    size_t fr = 0, tot = 0;
+    if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return (size_t)(0.97 * (double)(fr + c->ws_bytes));     // our own cached workspace can be re-used or re-sized
+}
+
+int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_opts* opts, mdwf_solve_info* info,
+               cudaStream_t st, bool host_buffers) {
+    if (!x || !b || !opts || !info) MDWF_FAIL(c, MDWF_EINVAL, "null argument");
+    if (nrhs < 1 || nrhs > MDWF_MAX_RHS) MDWF_FAIL(c, MDWF_EINVAL, "nrhs must be in 1..%d (got %d)", MDWF_MAX_RHS, nrhs);
+    if (opts->src_kind == 0 && opts->out_kind == 0) { /* x may alias b */ }
+    else if (x == b) MDWF_FAIL(c, MDWF_EINVAL, "x may alias b only for 5D source and 5D solution");
+    Solver S;
+    int rc = setup_solver(c, S, opts, st);
+    if (rc) return rc;
     const Geom& g = c->g;
     const size_t in_per = (size_t)2 * g.Vh * 24 * 8 * (opts->src_kind ? 1 : g.Ls);
     const size_t out_per = (size_t)2 * g.Vh * 24 * 8 * (opts->out_kind ? 1 : g.Ls);
-    int nb = opts->batch > 0 ? std::min(opts->batch, nrhs) : nrhs;
-    if (opts->batch <= 0) {
-        size_t fr = 0, tot = 0;
-        MDWF_CUDA(c, cudaMemGetInfo(&fr, &tot));
-        const size_t per = per_rhs_bytes(g, S.prec, S.px) + (host_buffers ? 2 * (in_per + out_per) : 0);
-        const size_t fit = (size_t)(0.92 * (double)fr) / per;
-        if (fit < 1) MDWF_FAIL(c, MDWF_ENOMEM, "not enough free device memory for one rhs (%zu needed, %zu free)", per, fr);
-        nb = (int)std::min<size_t>(fit, (size_t)nrhs);
-    }
+    int nb = 1, nhi = 1;
+    const int nset_guess = (host_buffers && (opts->batch <= 0 || opts->batch < nrhs)) ? 2 : 1;
+    if ((rc = plan_batch(c, S, nrhs, opts->batch, avail_bytes(c), host_buffers ? nset_guess * (in_per + out_per) : 0, true, &nb, &nhi))) return rc;
     memset(info, 0, sizeof(*info));
     cudaEvent_t e0, e1;
     MDWF_CUDA(c, cudaEventCreate(&e0));
@@ -318,10 +465,11 @@ int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_o
     MDWF_CUDA(c, cudaEventRecord(e0, st));
     const long long l0 = c->launches;
     double inner_ms = 0.0;
-    int rc = MDWF_OK;
+    S.nhi = nhi;
     if (!host_buffers) {
         for (int r0 = 0; r0 < nrhs && rc == MDWF_OK; r0 += nb) {
             S.nb = std::min(nb, nrhs - r0);
+            S.nhi = std::min(nhi, S.nb);
             rc = solve_batch(S, (double*)x, (const double*)b, opts, info, r0, &inner_ms);
         }
     } else {
@@ -332,14 +480,17 @@ int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_o
         cudaStream_t cs = nullptr;
         cudaEvent_t up[2] = {nullptr, nullptr}, down[2] = {nullptr, nullptr}, solved = nullptr;
         const int nbatch = (nrhs + nb - 1) / nb, nset = nbatch > 1 ? 2 : 1;
-        cudaError_t e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
-        for (int k = 0; k < nset && e == cudaSuccess; ++k) {
+        // the workspace first, so that the staging buffers cannot starve it
+        rc = ensure_workspace(c, work_bytes(g, S.prec, S.px, nb, nhi, true));
+        cudaError_t e = cudaSuccess;
+        if (rc == MDWF_OK) e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
+        for (int k = 0; k < nset && e == cudaSuccess && rc == MDWF_OK; ++k) {
             e = cudaMalloc(&din[k], in_per * nb);
             if (e == cudaSuccess) e = cudaMalloc(&dout[k], out_per * nb);
             if (e == cudaSuccess) e = cudaEventCreateWithFlags(&up[k], cudaEventDisableTiming);
             if (e == cudaSuccess) e = cudaEventCreateWithFlags(&down[k], cudaEventDisableTiming);
         }
-        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&solved, cudaEventDisableTiming);
+        if (e == cudaSuccess && rc == MDWF_OK) e = cudaEventCreateWithFlags(&solved, cudaEventDisableTiming);
         if (e != cudaSuccess) {
             cudaGetLastError();
             c->err = std::string("staging buffers for host-buffer solve: ") + cudaGetErrorString(e);
@@ -355,6 +506,7 @@ int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_o
         for (int k = 0; k < nbatch && rc == MDWF_OK; ++k) {
             const int r0 = k * nb, set = k % nset;
             S.nb = std::min(nb, nrhs - r0);
+            S.nhi = std::min(nhi, S.nb);
             e = cudaStreamWaitEvent(st, up[set], 0);                           // batch k is on the device
             if (e == cudaSuccess && k >= nset) e = cudaStreamWaitEvent(st, down[set], 0);   // dout[set] has been drained
             // din[(k+1) % nset] was last read by batch k-1, which has completed (solve_batch returns synchronised)
@@ -396,6 +548,56 @@ int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_o
     info->seconds = ms * 1e-3;
     info->seconds_inner = inner_ms * 1e-3;
     info->kernel_launches = c->launches - l0;
+    info->batch = nb;
+    if (rc) return rc;
+    int worst = MDWF_OK;
+    for (int i = 0; i < nrhs; ++i) worst = std::max(worst, info->status[i]);
+    return worst;
+}
+
+// Packed in-place solve: psi[par] / psi[1-par] hold b on entry and the solution on exit (fp64 packed half-lattice
+// fields of nrhs columns each).  No canonical copies exist, so a whole batch of large-volume rhs fits on the device.
+int solve_packed_impl(mdwf_ctx* c, mdwf_field* even, mdwf_field* odd, const mdwf_solve_opts* opts, mdwf_solve_info* info,
+                      cudaStream_t st) {
+    if (!even || !odd || !opts || !info) MDWF_FAIL(c, MDWF_EINVAL, "null argument");
+    if (even->prec != 64 || odd->prec != 64 || even->nrhs != odd->nrhs || even->ctx != c || odd->ctx != c)
+        MDWF_FAIL(c, MDWF_EINVAL, "mdwf_solve_packed needs two fp64 fields of this context with equal nrhs");
+    if (opts->src_kind != 0 || opts->out_kind != 0) MDWF_FAIL(c, MDWF_EINVAL, "mdwf_solve_packed handles 5D sources and solutions only");
+    const int nrhs = even->nrhs;
+    Solver S;
+    int rc = setup_solver(c, S, opts, st);
+    if (rc) return rc;
+    int nb = 1, nhi = 1;
+    if ((rc = plan_batch(c, S, nrhs, nrhs, avail_bytes(c), 0, false, &nb, &nhi))) return rc;
+    memset(info, 0, sizeof(*info));
+    cudaEvent_t e0, e1;
+    MDWF_CUDA(c, cudaEventCreate(&e0));
+    MDWF_CUDA(c, cudaEventCreate(&e1));
+    MDWF_CUDA(c, cudaEventRecord(e0, st));
+    const long long l0 = c->launches;
+    double inner_ms = 0.0;
+    S.nb = nb; S.nhi = nhi;
+    {
+        Work W;
+        mdwf_field* fp = S.par == 0 ? even : odd;
+        mdwf_field* fo = S.par == 0 ? odd : even;
+        rc = make_work(S, W, fp, fo);
+        if (rc == MDWF_OK) rc = solve_core(S, W, info, 0, &inner_ms);
+        if (rc == MDWF_OK) {      // psi_p: x_hi -> the caller's field
+            MDWF_CUDA(c, cudaMemcpyAsync(fp->v, W.xh->v, fp->bytes, cudaMemcpyDeviceToDevice, st));
+            rc = S.sync();
+        }
+    }
+    cudaEventRecord(e1, st);
+    cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    info->seconds = ms * 1e-3;
+    info->seconds_inner = inner_ms * 1e-3;
+    info->kernel_launches = c->launches - l0;
+    info->batch = nb;
     if (rc) return rc;
     int worst = MDWF_OK;
     for (int i = 0; i < nrhs; ++i) worst = std::max(worst, info->status[i]);
@@ -408,11 +610,31 @@ extern "C" {
 int mdwf_solve(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_opts* opts, mdwf_solve_info* info,
                void* stream) {
     if (!c) return MDWF_EINVAL;
+    if (cudaSetDevice(c->geo.device) != cudaSuccess) return MDWF_ECUDA;
     return mdwf::solve_impl(c, x, b, nrhs, opts, info, (cudaStream_t)stream, false);
 }
 int mdwf_solve_host(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_opts* opts,
                     mdwf_solve_info* info, void* stream) {
     if (!c) return MDWF_EINVAL;
+    if (cudaSetDevice(c->geo.device) != cudaSuccess) return MDWF_ECUDA;
     return mdwf::solve_impl(c, x, b, nrhs, opts, info, (cudaStream_t)stream, true);
+}
+int mdwf_solve_packed(mdwf_ctx* c, mdwf_field* psi_even, mdwf_field* psi_odd, const mdwf_solve_opts* opts,
+                      mdwf_solve_info* info, void* stream) {
+    if (!c) return MDWF_EINVAL;
+    if (cudaSetDevice(c->geo.device) != cudaSuccess) return MDWF_ECUDA;
+    return mdwf::solve_packed_impl(c, psi_even, psi_odd, opts, info, (cudaStream_t)stream);
+}
+int mdwf_workspace_bytes(mdwf_ctx* c, int nrhs, int inner_prec, int packed, int64_t* bytes) {
+    if (!c || !bytes) return MDWF_EINVAL;
+    if (nrhs < 1 || nrhs > MDWF_MAX_RHS || (inner_prec != 64 && inner_prec != 32 && inner_prec != 16)) MDWF_FAIL(c, MDWF_EINVAL, "bad nrhs or precision");
+    *bytes = (int64_t)mdwf::work_bytes(c->g, inner_prec, inner_prec == 16 ? 32 : inner_prec, nrhs, 1, !packed);
+    return MDWF_OK;
+}
+int mdwf_set_workspace(mdwf_ctx* c, void* mem, int64_t bytes) {
+    if (!c) return MDWF_EINVAL;
+    if (c->ws && !c->ws_external) cudaFree(c->ws);
+    c->ws = mem; c->ws_bytes = mem ? (size_t)bytes : 0; c->ws_external = mem != nullptr;
+    return MDWF_OK;
 }
 }

@@ -80,7 +80,6 @@ def main():
         peak = float(json.load(open(pk))["hbm_gbs"])
     ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
     ctx.mdwf_set_tiling(a.zc)
-    print(json.dumps({"device_fp32_fma_TFLOPs_measured": round(ctx.mdwf_probe_fp32_fma(), 2)}), flush=True)
     if a.meas:
         measurement_kernels(ctx, cfg, a.iters, peak)
         return

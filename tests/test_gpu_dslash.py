@@ -116,21 +116,6 @@ def test_errors_are_loud():
         ctx.mdwf_dslash(mdwf.OP_HOP, x, prec=32, recon=12)   # gauge not loaded
 
 
-def test_tiled_shared_memory_hop_variant_matches_oracle():
-    """The experimental 4D-tile kernel (mdwf_hop_tile.cuh, opt-in through MDWF_HOP_TILED=1; slower than the default on
-    B200, see profiles/README.md) computes the same operator: run the op-level parity test in a subprocess with it."""
-    import os
-    import subprocess
-    import sys
-    env = dict(os.environ, MDWF_HOP_TILED="1")
-    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    r = subprocess.run([sys.executable, "-m", "pytest", "-q", "-x", "-m", "gpu", os.path.join(root, "tests", "test_gpu_dslash.py"),
-                        "-k", "test_all_ops_match_oracle and (32-12 or 16-12) and dims2"], env=env, cwd=root,
-                       capture_output=True, text=True, timeout=900)
-    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
-    assert "passed" in r.stdout
-
-
 def test_traversal_order_does_not_change_results():
     """the z-slab depth (mdwf_set_tiling) only reorders blocks: results are bit-identical for every legal depth"""
     dims, Ls = (8, 8, 8, 4), 8          # blocks are whole (x, y) planes here, so every divisor of Z is a legal depth

@@ -174,8 +174,8 @@ def test_bit_reproducible_and_packed_api_and_profile():
     assert torch.equal(torch.view_as_real(out), torch.view_as_real(ref))
     n5 = (V4 // 2) * Ls * 2
     assert n == 2 and ms > 0 and fl == 2 * 1320.0 * n5
-    assert by == (2 + 3) * 52.0 * n5 + 2 * 8 * 12 * 2 * (V4 // 2)      # one plain-input and one xpay-input fused hop
+    assert by == (2 + 3) * 48.0 * n5 + 2 * 8 * 12 * 2 * (V4 // 2)      # one plain-input and one xpay-input fused hop
     cb, cf = ctx.mdwf_dslash_cost(mdwf.OP_HOP, 16, 12, 2)
-    assert cb == 2 * 52.0 * n5 + 8 * 12 * 2 * (V4 // 2) and cf == 1320.0 * n5
+    assert cb == 2 * 48.0 * n5 + 8 * 12 * 2 * (V4 // 2) and cf == 1320.0 * n5
     with pytest.raises(mdwf.MdwfError):
         ctx.mdwf_dslash_packed(mdwf.OP_HOP, fin, fin, recon=12)          # out must not alias in
