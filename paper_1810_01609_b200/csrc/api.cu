@@ -203,7 +203,7 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     c->geo = *geo;
     c->M5 = M5; c->b5 = b5; c->c5 = c5; c->mf = mf;
     c->partial = nullptr; c->dscal = nullptr; c->hscal = nullptr; c->launches = 0; c->prof_on = 0; c->zc_forced = 0;
-    c->tile16 = nullptr; c->tile16_nw = 0; c->partial_nblk = 0; c->partial_cap = 0;
+    c->tile16[0] = c->tile16[1] = c->tile16[2] = nullptr; c->tile16_nw = 0; c->partial_nblk = 0; c->partial_cap = 0;
     c->ws = nullptr; c->ws_bytes = 0; c->ws_external = false;
     for (int i = 0; i < 4; ++i) c->tile16_forced[i] = 0;
     for (int i = 0; i < 3; ++i) { c->prof_ms[i] = c->prof_bytes[i] = c->prof_flops[i] = 0.0; c->prof_n[i] = 0; }
@@ -262,7 +262,7 @@ int mdwf_destroy(mdwf_ctx* c) {
     if (!c) return MDWF_OK;
     for (size_t i = 0; i < c->gauges.size(); ++i) free_gauge(&c->gauges[i]);
     for (auto& kv : c->temps) for (mdwf_field* f : kv.second) free_field(f);
-    if (c->tile16) { free_tile16(c->tile16); delete c->tile16; c->tile16 = nullptr; }
+    for (int i = 0; i < 3; ++i) if (c->tile16[i]) { free_tile16(c->tile16[i]); delete c->tile16[i]; c->tile16[i] = nullptr; }
     if (c->ws && !c->ws_external) cudaFree(c->ws);
     prof_drain(c);
     for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
@@ -366,7 +366,7 @@ namespace mdwf {
 
 static SpinorView no_view() {
     SpinorView v;
-    v.v = nullptr; v.m = nullptr; v.rs = 0;
+    memset(&v, 0, sizeof(v));
     return v;
 }
 
@@ -389,6 +389,7 @@ int op_hop(const OpCtx& o, mdwf_field* out, const mdwf_field* in, int out_par, i
     a.out = out->view(); a.in = in->view();
     a.xin = xin ? xin->view() : no_view();
     a.g.v[0] = o.gs->v[0]; a.g.v[1] = o.gs->v[1];
+    a.g.pl[0] = o.gs->pl[0]; a.g.pl[1] = o.gs->pl[1];
     if (mat >= 0) a.op = o.c->lsop[mat]; else { a.op = o.c->lsop[0]; a.op.kind = 0; }
     a.cx = cx; a.ch = ch; a.partial = partial; a.par = out_par; a.nact = rl.nact;
     for (int i = 0; i < 64; ++i) a.rhs_list[i] = rl.rhs[i];
@@ -497,11 +498,10 @@ extern "C" {
 int mdwf_set_hop16_tile(mdwf_ctx* c, int lx, int ly, int lz, int lt, int warps) {
     if (!c) return MDWF_EINVAL;
     if (warps < 0 || warps > MDWF_H16_MAXW) MDWF_FAIL(c, MDWF_EINVAL, "warps must be in 0..%d", MDWF_H16_MAXW);
-    if (c->tile16) { free_tile16(c->tile16); delete c->tile16; c->tile16 = nullptr; }
+    for (int i = 0; i < 3; ++i) if (c->tile16[i]) { free_tile16(c->tile16[i]); delete c->tile16[i]; c->tile16[i] = nullptr; }
     c->tile16_forced[0] = lx; c->tile16_forced[1] = ly; c->tile16_forced[2] = lz; c->tile16_forced[3] = lt;
     c->tile16_nw = warps;
-    Tile16Host* th;
-    return get_tile16(c, &th);
+    return MDWF_OK;     // checked when the next fp16 stencil launch builds its tables
 }
 
 int mdwf_field_create(mdwf_ctx* c, int prec, int nrhs, mdwf_field** out) {

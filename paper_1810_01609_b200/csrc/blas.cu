@@ -4,12 +4,25 @@
 
 namespace mdwf {
 
-static size_t rhs_bytes(const Geom& g, int prec) {
-    if (prec == 16) return ((size_t)g.N5h * 48 + 255) / 256 * 256;       // site-major, 48 bytes per 5D site
+// fp16: rhs interleave of a field with nrhs columns (log2): groups of 4 when there are at least 4, else 2, else 1
+// (the RI * Ls rows of a site are at most 48 = three m16 tiles of the tensor-core stencil)
+int half_ril(int nrhs, int Ls) {
+    for (int ril = 2; ril > 0; --ril)
+        if ((1 << ril) <= nrhs && (Ls << ril) <= 48) return ril;
+    return 0;
+}
+static size_t rhs_bytes(const Geom& g, int prec, int nrhs) {      // stride between rhs (fp16: between rhs groups)
+    if (prec == 16) return ((((size_t)g.N5h * 48) << half_ril(nrhs, g.Ls)) + 255) / 256 * 256;
     const size_t nb = ((size_t)g.N5h + 31) / 32;
     return nb * (size_t)((24 * (prec / 8) / 16) * 512);
 }
-size_t field_bytes(const Geom& g, int prec, int nrhs) { return rhs_bytes(g, prec) * nrhs; }
+size_t field_bytes(const Geom& g, int prec, int nrhs) {
+    if (prec == 16) {
+        const int ri = 1 << half_ril(nrhs, g.Ls);
+        return rhs_bytes(g, prec, nrhs) * ((nrhs + ri - 1) / ri);
+    }
+    return rhs_bytes(g, prec, nrhs) * nrhs;
+}
 
 static int make_field(mdwf_ctx* c, int prec, int nrhs, void* mem, void* meta_mem, mdwf_field** out) {
     if (prec != 64 && prec != 32 && prec != 16) MDWF_FAIL(c, MDWF_EINVAL, "prec must be 64, 32 or 16 (got %d)", prec);
@@ -25,8 +38,10 @@ static int make_field(mdwf_ctx* c, int prec, int nrhs, void* mem, void* meta_mem
     f->rhs0 = 0;
     f->owns = mem == nullptr;
     f->owns_meta = false;
+    f->rs = rhs_bytes(c->g, prec, nrhs);
     if (!mem) {
         cudaError_t e = cudaMalloc(&f->v, f->bytes);
+        if (e == cudaSuccess && prec == 16) e = cudaMemset(f->v, 0, f->bytes);     // padding rhs of the last group
         if (e != cudaSuccess) {
             delete f;
             cudaGetLastError();
@@ -244,8 +259,11 @@ int launch_pack(mdwf_ctx* c, int prec, bool unpack, PackArgs& a, cudaStream_t st
 
 mdwf::SpinorView mdwf_field::view() const {
     mdwf::SpinorView s;
-    s.rs = (long long)(bytes / nrhs);
+    s.rs = (long long)rs;
     s.v = reinterpret_cast<char*>(v) - (long long)rhs0 * s.rs;
     s.m = rmeta();
+    s.ril = prec == 16 ? mdwf::half_ril(nrhs, ctx->g.Ls) : 0;
+    s.Ls = ctx->g.Ls;
+    s.dLs = ctx->g.dLs;
     return s;
 }

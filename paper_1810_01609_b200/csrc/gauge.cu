@@ -55,10 +55,34 @@ __global__ void __launch_bounds__(256) gauge_pack_kernel(const Geom g, const Gau
     }
 }
 
+// Stencil-ready links for 16-bit storage (GaugeView::pl): for every output site of parity `par` and leg l the matrix
+// exactly as the stencil multiplies it -- decoded from the packed fp16 format (18/12/8 reals), daggered for backward
+// legs, boundary sign folded (stage_link, mdwf_hop.cuh) -- rounded to half.  288 bytes per site; it replaces the
+// per-block reconstruction (and makes the 12/8-real decode a load-time cost) for the tensor-core stencil.
+template <int R>
+__global__ void __launch_bounds__(256) gauge_prepare16_kernel(const Geom g, GaugeView gv, uint32_t* pl, int par) {
+    const int task = blockIdx.x * blockDim.x + threadIdx.x;
+    if (task >= g.Vh * 8) return;
+    const int xh = task >> 3, l = task & 7;
+    SiteCoord c;
+    uint32_t row, xx, r2, y, t, z;
+    g.dXH.divmod((uint32_t)xh, row, xx);
+    g.dY.divmod(row, r2, y);
+    g.dZ.divmod(r2, t, z);
+    c.xh = xh; c.xx = xx; c.y = y; c.z = z; c.t = t;
+    c.o = (par + y + z + t) & 1;
+    float V[MDWF_LROW];
+    stage_link<__half, R>(g, gv, par, c, l, V);
+    uint32_t* dst = pl + (long long)xh * 72 + l;
+#pragma unroll
+    for (int e = 0; e < 9; ++e) dst[e * 8] = f2h(V[2 * e], V[2 * e + 1]);
+}
+
 void free_gauge(GaugeSet* gs) {
     for (int p = 0; p < 2; ++p) {
         if (gs->v[p]) cudaFree(gs->v[p]);
-        gs->v[p] = nullptr;
+        if (gs->pl[p]) cudaFree(gs->pl[p]);
+        gs->v[p] = nullptr; gs->pl[p] = nullptr;
     }
 }
 
@@ -87,6 +111,7 @@ int pack_gauge(mdwf_ctx* c, const void* U, int prec, int recon, GaugeSet* gs, cu
     gs->recon = recon;
     gs->bytes_per_parity = (size_t)4 * ngv * c->g.Vh * vbytes;
     gs->v[0] = gs->v[1] = nullptr;
+    gs->pl[0] = gs->pl[1] = nullptr;
     int* bad = nullptr;
     for (int p = 0; p < 2; ++p) {
         cudaError_t e = cudaMalloc(&gs->v[p], gs->bytes_per_parity);
@@ -118,6 +143,25 @@ int pack_gauge(mdwf_ctx* c, const void* U, int prec, int recon, GaugeSet* gs, cu
         snprintf(b, sizeof(b), "8-real link format cannot represent %d links with |U01|^2+|U02|^2 -> 0 (SURVEY A12); use recon 12 or 18", nbad);
         c->err = b;
         rc = MDWF_EINVAL;
+    }
+    if (rc == MDWF_OK && prec == 16) {
+        GaugeView gv;
+        gv.v[0] = gs->v[0]; gv.v[1] = gs->v[1];
+        gv.pl[0] = gv.pl[1] = nullptr;
+        const int ntask = c->g.Vh * 8, grid = (ntask + 255) / 256;
+        for (int p = 0; p < 2 && rc == MDWF_OK; ++p) {
+            if (cudaMalloc(&gs->pl[p], (size_t)c->g.Vh * 288) != cudaSuccess) {
+                cudaGetLastError();
+                c->err = "cudaMalloc of the stencil-ready fp16 links failed";
+                rc = MDWF_ENOMEM;
+                break;
+            }
+            if (recon == 18) gauge_prepare16_kernel<18><<<grid, 256, 0, st>>>(c->g, gv, gs->pl[p], p);
+            else if (recon == 12) gauge_prepare16_kernel<12><<<grid, 256, 0, st>>>(c->g, gv, gs->pl[p], p);
+            else gauge_prepare16_kernel<8><<<grid, 256, 0, st>>>(c->g, gv, gs->pl[p], p);
+            if (cudaGetLastError() != cudaSuccess) { c->err = "gauge_prepare16_kernel launch failed"; rc = MDWF_ECUDA; }
+            c->launches++;
+        }
     }
     if (rc != MDWF_OK) free_gauge(gs);
     return rc;

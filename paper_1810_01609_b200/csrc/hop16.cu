@@ -44,9 +44,9 @@ static void build_vcode(uint32_t vcode[2][32]) {
 
 static inline int pack4(int x, int y, int z, int t) { return x | (y << 8) | (z << 16) | (t << 24); }
 
-struct Plan16 { int ns, nip[2], nrun[2]; size_t smem; };
+struct Plan16 { int ns, spw, nst, nip[2], nrun[2]; size_t off_nbr, off_links, off_wpart, off_stage, stage, off_epi, smem; };
 // counts and shared-memory need of a box without building tables
-static Plan16 plan_tile16(const int L[4], int Ls, int nw) {
+static Plan16 plan_tile16(const int L[4], int rows, int nw) {      // rows = RI * Ls of one site
     Plan16 p;
     const int vol = L[0] * L[1] * L[2] * L[3];
     p.ns = vol / 2;
@@ -62,21 +62,23 @@ static Plan16 plan_tile16(const int L[4], int Ls, int nw) {
         }
         p.nip[pat] = ni; p.nrun[pat] = nr;
     }
-    const int MT = (Ls + 15) / 16;
+    const int MT = (rows + 15) / 16;
+    p.spw = (p.ns + nw - 1) / nw;
     size_t off = MDWF_H16_HDR;
-    off += ((size_t)p.ns * 8 * 2 + 15) / 16 * 16;
-    off += ((size_t)p.ns * 4 + 15) / 16 * 16;
-    off += (size_t)p.ns * 8 * MDWF_H16_LREC;
-    off += 64;
+    p.off_nbr = off; off += ((size_t)2 * p.ns * 8 * 4 + (size_t)2 * p.ns * 4 + 15) / 16 * 16;
+    p.off_links = off; off += (size_t)nw * p.spw * MDWF_H16_SREC;
+    p.off_wpart = off; off += (size_t)64 * nw * 8;
+    p.off_epi = off; off += (size_t)nw * MT * 16 * 24 * 4;
     off = (off + 127) / 128 * 128;
-    const size_t stage = ((size_t)std::max(p.nip[0], p.nip[1]) * Ls * 48 + 127) / 128 * 128;
-    off += 2 * stage;
-    off += (size_t)nw * MT * 16 * 24 * 4;
-    p.smem = off;
+    p.off_stage = off;
+    p.stage = ((size_t)std::max(p.nip[0], p.nip[1]) * rows * 48 + 127) / 128 * 128;
+    const size_t cap = 227 * 1024 - 256;
+    p.nst = off + 2 * p.stage > cap ? 2 : (int)std::min<size_t>(MDWF_H16_MAXST, (cap - off) / p.stage);
+    p.smem = off + (size_t)p.nst * p.stage;
     return p;
 }
 
-static int build_tile16(mdwf_ctx* c, const int L[4], int nw, Tile16Host* th) {
+static int build_tile16(mdwf_ctx* c, const int L[4], int rows, int nw, Tile16Host* th) {
     const Geom& g = c->g;
     Tile16& tl = th->t;
     memset(&tl, 0, sizeof(tl));
@@ -128,18 +130,10 @@ static int build_tile16(mdwf_ctx* c, const int L[4], int nw, Tile16Host* th) {
         th->dev[3 * pat] = d0; th->dev[3 * pat + 1] = d1; th->dev[3 * pat + 2] = d2;
         tl.outc[pat] = (const int*)d0; tl.run[pat] = (const int4*)d1; tl.nbr[pat] = (const unsigned short*)d2;
     }
-    const int MT = (g.Ls + 15) / 16;
-    size_t off = MDWF_H16_HDR;
-    tl.off_nbr = (int)off; off += ((size_t)tl.ns * 8 * 2 + 15) / 16 * 16;
-    tl.off_oxh = (int)off; off += ((size_t)tl.ns * 4 + 15) / 16 * 16;
-    tl.off_links = (int)off; off += (size_t)tl.ns * 8 * MDWF_H16_LREC;
-    tl.off_zero = (int)off; off += 64;
-    off = (off + 127) / 128 * 128;
-    tl.off_stage = (int)off;
-    tl.stage_bytes = (int)(((size_t)std::max(tl.nip[0], tl.nip[1]) * g.Ls * 48 + 127) / 128 * 128);
-    off += 2 * (size_t)tl.stage_bytes;
-    tl.off_epi = (int)off; off += (size_t)nw * MT * 16 * 24 * 4;
-    tl.smem_total = (int)off;
+    const Plan16 pl = plan_tile16(L, rows, nw);
+    tl.spw = pl.spw; tl.nst = pl.nst;
+    tl.off_nbr = (int)pl.off_nbr; tl.off_links = (int)pl.off_links; tl.off_wpart = (int)pl.off_wpart; tl.off_epi = (int)pl.off_epi;
+    tl.off_stage = (int)pl.off_stage; tl.stage_bytes = (int)pl.stage; tl.smem_total = (int)pl.smem;
     tl.dTx = make_fastdiv(tl.nT[0]); tl.dTy = make_fastdiv(tl.nT[1]); tl.dTt = make_fastdiv(tl.nT[3]);
     tl.zc_t = tl.nT[2]; tl.dTzs = make_fastdiv(tl.zc_t);
     build_vcode(tl.vcode);
@@ -150,17 +144,21 @@ void free_tile16(Tile16Host* th) {
     for (int i = 0; i < 6; ++i) if (th->dev[i]) { cudaFree(th->dev[i]); th->dev[i] = nullptr; }
 }
 
-// Tile choice: among the boxes that divide the lattice and fit in shared memory, the one with the fewest input-site
-// fetches per output site (ni/ns: 8 without any reuse, 4 for a 4x4x2x2 box), with a mild penalty for boxes whose sites
-// do not spread evenly over the warps.  MDWF_TILE16="lx,ly,lz,lt" forces a box (tuning runs).
-static int choose_tile16(mdwf_ctx* c, int nw, int L[4]) {
+// Tile choice: among the boxes that divide the lattice and fit in shared memory (with at least two staging buffers),
+// the one with the fewest input-site fetches per output site (ni/ns: 8 without any reuse, 5 for a 2^4 box, 4 for
+// 4x4x2x2).  Warps per block: one per output site up to 16 (then 2..4 sites per warp).  mdwf_set_hop16_tile forces a box.
+static int warps_for(int ns) { return ns >= 16 ? 16 : ns >= 8 ? 8 : 4; }
+static int choose_tile16(mdwf_ctx* c, int rows, int L[4], int* nw_out) {
     const Geom& g = c->g;
     const int dims[4] = {g.X, g.Y, g.Z, g.T};
     const size_t cap = 227 * 1024 - 256;
     if (c->tile16_forced[0] > 0) {
         for (int d = 0; d < 4; ++d) L[d] = c->tile16_forced[d];
         for (int d = 0; d < 4; ++d) if (L[d] < 1 || dims[d] % L[d] || (d == 0 && (L[d] & 1))) MDWF_FAIL(c, MDWF_EINVAL, "forced fp16 tile does not divide the lattice");
-        if (plan_tile16(L, g.Ls, nw).smem > cap) MDWF_FAIL(c, MDWF_EINVAL, "forced fp16 tile does not fit in shared memory");
+        const int nw = c->tile16_nw > 0 ? c->tile16_nw : warps_for(L[0] * L[1] * L[2] * L[3] / 2);
+        const Plan16 pf = plan_tile16(L, rows, nw);
+        if (pf.smem > cap || pf.spw > 4) MDWF_FAIL(c, MDWF_EINVAL, "forced fp16 tile does not fit in shared memory (or has more than 4 sites per warp)");
+        *nw_out = nw;
         return MDWF_OK;
     }
     double best = 1e30;
@@ -168,29 +166,32 @@ static int choose_tile16(mdwf_ctx* c, int nw, int L[4]) {
     for (int lx = 2; lx <= 8; lx += 2) for (int ly = 1; ly <= 8; ++ly) for (int lz = 1; lz <= 8; ++lz) for (int lt = 1; lt <= 8; ++lt) {
         if (dims[0] % lx || dims[1] % ly || dims[2] % lz || dims[3] % lt) continue;
         const int cand[4] = {lx, ly, lz, lt};
-        const Plan16 p = plan_tile16(cand, g.Ls, nw);
-        if (p.ns > 128 || p.smem > cap) continue;
+        const int nw = warps_for(lx * ly * lz * lt / 2);
+        const Plan16 p = plan_tile16(cand, rows, nw);
+        if (p.spw > 4 || p.smem > cap) continue;
         const double fetch = (double)std::max(p.nip[0], p.nip[1]) / p.ns;
         const double imbal = (double)((p.ns + nw - 1) / nw * nw) / p.ns;
         const double cost = fetch * (1.0 + 0.25 * (imbal - 1.0));
-        if (cost < best - 1e-12) { best = cost; L[0] = lx; L[1] = ly; L[2] = lz; L[3] = lt; }
+        if (cost < best - 1e-12) { best = cost; L[0] = lx; L[1] = ly; L[2] = lz; L[3] = lt; *nw_out = nw; }
     }
-    if (!L[0]) MDWF_FAIL(c, MDWF_EINVAL, "no fp16 stencil tile fits in shared memory (Ls = %d)", g.Ls);
+    if (!L[0]) MDWF_FAIL(c, MDWF_EINVAL, "no fp16 stencil tile fits in shared memory (%d rows per site)", rows);
     return MDWF_OK;
 }
 
-int get_tile16(mdwf_ctx* c, Tile16Host** out) {
-    if (!c->tile16) {
-        const int nw = c->tile16_nw > 0 ? c->tile16_nw : MDWF_H16_MAXW;
-        int L[4];
-        int rc = choose_tile16(c, nw, L);
+// tiles are cached per rhs interleave (the staging buffers hold RI * Ls rows per site)
+int get_tile16(mdwf_ctx* c, int ril, Tile16Host** out) {
+    if (ril < 0 || ril > 2) MDWF_FAIL(c, MDWF_EINVAL, "internal: bad rhs interleave");
+    if (!c->tile16[ril]) {
+        const int rows = c->g.Ls << ril;
+        int L[4], nw = 0;
+        int rc = choose_tile16(c, rows, L, &nw);
         if (rc) return rc;
         Tile16Host* th = new Tile16Host;
-        rc = build_tile16(c, L, nw, th);
+        rc = build_tile16(c, L, rows, nw, th);
         if (rc) { free_tile16(th); delete th; return rc; }
-        c->tile16 = th;
+        c->tile16[ril] = th;
     }
-    *out = c->tile16;
+    *out = c->tile16[ril];
     return MDWF_OK;
 }
 
@@ -200,7 +201,7 @@ static int pick_zc16(const Geom& g, const Tile16& tl, int nact) {
     int best = 1;
     for (int z = 1; z <= tl.nT[2]; ++z) {
         if (tl.nT[2] % z) continue;
-        const double layer = (double)g.XH * g.Y * (z * tl.L[2]) * tl.L[3] * g.Ls * 48.0 * nact;
+        const double layer = (double)g.XH * g.Y * (z * tl.L[2]) * tl.L[3] * g.Ls * 48.0 * nact;   // nact rhs = groups x RI
         if (3.0 * layer <= 40.0e6) best = z;
     }
     return best;
@@ -209,21 +210,25 @@ static int pick_zc16(const Geom& g, const Tile16& tl, int nact) {
 int launch_hop_f16(mdwf_ctx* c, int recon, int dagger, int fused, HopArgs& a, cudaStream_t st) {
     (void)fused;
     Tile16Host* th;
-    int rc = get_tile16(c, &th);
+    int rc = get_tile16(c, a.in.ril, &th);
     if (rc) return rc;
-    if (recon != 18 && recon != 12 && recon != 8) MDWF_FAIL(c, MDWF_EINVAL, "recon must be 18, 12 or 8 (got %d)", recon);
+    (void)recon;       // the stencil-ready links were decoded from the (prec 16, recon) format at load time
+    if (!a.g.pl[0] || !a.g.pl[1]) MDWF_FAIL(c, MDWF_ESTATE, "internal: stencil-ready fp16 links missing");
     if (!a.in.m || !a.out.m || (a.xin.v && !a.xin.m) || a.sr.n < 1) MDWF_FAIL(c, MDWF_EINVAL, "internal: fp16 hop without field scales");
+    if (a.out.ril != a.in.ril || (a.xin.v && a.xin.ril != a.in.ril)) MDWF_FAIL(c, MDWF_EINVAL, "internal: fp16 hop on fields with different rhs interleave");
+    const int rows = c->g.Ls << a.in.ril;
     Tile16 tl = th->t;
     tl.zc_t = c->zc_forced > 0 && c->zc_forced % tl.L[2] == 0 && tl.nT[2] % (c->zc_forced / tl.L[2]) == 0 ? c->zc_forced / tl.L[2]
                                                                                                         : pick_zc16(c->g, tl, a.nact);
     tl.dTzs = make_fastdiv(tl.zc_t);
     const int grid = std::min(tl.ntiles, c->sm_count), block = th->nw * 32;
-    auto kern = c->g.Ls <= 16 ? hop16_kernel<1> : hop16_kernel<2>;
+    auto kern = rows <= 16 ? hop16_kernel<1> : rows <= 32 ? hop16_kernel<2> : hop16_kernel<3>;
+    if (rows > 48) MDWF_FAIL(c, MDWF_EINVAL, "internal: %d rows per site", rows);
     if (!c->attr_raised.count((const void*)kern)) {
         MDWF_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         c->attr_raised.insert((const void*)kern);
     }
-    kern<<<grid, block, tl.smem_total, st>>>(c->g, tl, a, recon, dagger ? 1 : 0);
+    kern<<<grid, block, tl.smem_total, st>>>(c->g, tl, a, dagger ? 1 : 0);
     MDWF_CUDA(c, cudaGetLastError());
     c->launches++;
     c->partial_nblk = grid;

@@ -9,10 +9,14 @@
 //        r = c*RPV .. c*RPV+RPV-1.  A thread owns one 5D site idx = xh*Ls + s (s fastest), so a warp
 //        reads 512 contiguous bytes per vector index.  rhs are separate fields (stride in bytes).
 //   spinor fp16 ("16-bit storage, single-precision computation"; reading R11):
-//        site-major, 48 bytes per 5D site: half[colour 3][spin 4][re,im] -- one 16-byte chunk per colour, so
-//        that (a) the Ls slices of a 4D site are Ls*48 contiguous bytes (one bulk copy into shared memory) and
-//        (b) an ldmatrix row (16 bytes) is a K-slice of the tensor-core stencil whose lane <-> spin mapping is
-//        regular (mdwf_hop16.cuh).  One power-of-two fp32 scale per (field, rhs): value = e * half.
+//        site-major, 48 bytes per 5D site: half[colour 3][spin 4][re,im] -- one 16-byte chunk per colour -- with
+//        the rhs interleaved in groups of RI = 1, 2 or 4 inside a 4D site:  [group][xh][rhs in group][s][48 B], so
+//        that (a) all Ls slices of all rhs of a group at one 4D site are RI*Ls*48 contiguous bytes (one bulk copy
+//        of ~2 KB into shared memory: the size from which such copies run at full bandwidth), (b) they are the
+//        rows of ONE m16 x K tile sequence of the tensor-core stencil, sharing its link fragments (north_star:
+//        links "reused across the Ls slices and across multiple right-hand sides"), and (c) an ldmatrix row
+//        (16 bytes) is a K-slice whose lane <-> spin mapping is regular (mdwf_hop16.cuh).
+//        One power-of-two fp32 scale per (field, rhs): value = e * half.
 //   gauge, per (site parity, mu): vec[c][xh]   fp64: double2 x ceil(R/2), fp32: float4 x ceil(R/4),
 //        fp16: 4 x half (8 bytes) x ceil(R/4);  R = 18 | 12 | 8 reals.
 #pragma once
@@ -115,11 +119,18 @@ __device__ __forceinline__ float eval_scale(const ScaleRule& r, int rhs, bool wr
 struct SpinorView {
     void* v;          // vectors
     FieldMeta* m;     // fp16 only: scales / norm bounds of the CURRENT content (read side)
-    long long rs;     // rhs stride in BYTES
+    long long rs;     // rhs stride in BYTES (fp16: stride of a GROUP of 1 << ril rhs)
+    int ril;          // fp16 only: log2 of the rhs interleave RI
+    int Ls;           // fp16 only
+    FastDiv dLs;      // fp16 only: idx -> (xh, s)
 };
 
 struct GaugeView {
     const void* v[2];   // per parity of the link's base site; [mu][c][xh] vectors
+    // fp16 storage only: per parity of the OUTPUT site, the 8 stencil links of every site as the half-precision matrices
+    // the stencil multiplies (reconstructed, daggered for backward legs, boundary sign folded): word (re, im) of entry e
+    // of leg l at [xh][e 9][l 8]
+    const uint32_t* pl[2];
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -162,7 +173,13 @@ __device__ __forceinline__ uint32_t f2h(float a, float b) {
 template <typename S> struct Blk { static constexpr int BYTES = Store<S>::NV * 512; };
 template <typename S>
 __device__ __forceinline__ const char* site_ptr(const SpinorView& f, int r, int idx) {
-    if (Store<S>::HALF) return reinterpret_cast<const char*>(f.v) + (long long)r * f.rs + (long long)idx * 48;
+    if (Store<S>::HALF) {
+        uint32_t xh, sl;
+        f.dLs.divmod((uint32_t)idx, xh, sl);
+        const int ri = r & ((1 << f.ril) - 1);
+        return reinterpret_cast<const char*>(f.v) + (long long)(r >> f.ril) * f.rs +
+               ((((long long)xh << f.ril) + ri) * f.Ls + sl) * 48;
+    }
     return reinterpret_cast<const char*>(f.v) + (long long)r * f.rs + (long long)(idx >> 5) * Blk<S>::BYTES + (idx & 31) * 16;
 }
 

@@ -16,6 +16,7 @@ struct GaugeSet {
     int prec, recon;
     void* v[2];
     size_t bytes_per_parity;
+    uint32_t* pl[2];    // prec 16: stencil-ready half-precision links (GaugeView::pl), else nullptr
 };
 
 // A packed field set.  fp16 fields own two FieldMeta slots (scales / norm bounds, mdwf_device.cuh): readers use slot
@@ -29,6 +30,7 @@ struct mdwf_field {
     int cur;
     int rhs0;                  // rhs id of slot 0 (temporaries that serve a window of a larger batch), normally 0
     size_t bytes;
+    size_t rs;                 // bytes between rhs (fp16: between rhs groups)
     bool owns, owns_meta;      // v / meta were cudaMalloc'ed by alloc_field (else they live in a workspace)
     mdwf::SpinorView view() const;
     mdwf::FieldMeta* rmeta() const { return meta ? meta + cur : nullptr; }
@@ -68,7 +70,7 @@ struct mdwf_ctx {
     long long prof_n[3];
     int sm_count;
     double lsop_norm[MAT_COUNT];   // 2-norm bounds of the s-direction operators (fp16 scale rules)
-    mdwf::Tile16Host* tile16;      // tile tables of the fp16 tensor-core stencil (built on first use)
+    mdwf::Tile16Host* tile16[3];   // tile tables of the fp16 tensor-core stencil per rhs interleave (built on first use)
     int tile16_forced[4], tile16_nw;
     std::set<const void*> attr_raised;   // kernels whose dynamic shared-memory limit was raised on THIS device
     int partial_nblk;              // partial sums per rhs written by the last kernel that filled `partial`
@@ -107,6 +109,7 @@ inline RhsList all_rhs(int n) {
 }
 
 size_t field_bytes(const Geom& g, int prec, int nrhs);
+int half_ril(int nrhs, int Ls);
 int alloc_field(mdwf_ctx* c, int prec, int nrhs, mdwf_field** out);
 // a field whose vectors live at `mem` (field_bytes() bytes, 256-byte aligned) instead of their own allocation
 int wrap_field(mdwf_ctx* c, int prec, int nrhs, void* mem, void* meta_mem, mdwf_field** out);
@@ -153,7 +156,7 @@ int op_schur(const OpCtx& o, mdwf_field* out, const mdwf_field* in, int par, int
              int first_factor_done = 0);   // non-dagger only: t1 already holds A*in (fused into the CG p-update)
 // fp16 scale rule  nb_out = ca nb(a) + cb nb(b)  (b optional); n = 0 when out is not fp16
 ScaleRule rule_lin(const mdwf_field* out, const mdwf_field* a, double ca, const mdwf_field* b = nullptr, double cb = 0.0);
-int get_tile16(mdwf_ctx* c, Tile16Host** out);
+int get_tile16(mdwf_ctx* c, int ril, Tile16Host** out);
 void free_tile16(Tile16Host* th);
 
 int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_opts* opts, mdwf_solve_info* info,

@@ -116,6 +116,8 @@ int make_work(Solver& S, Work& W, mdwf_field* ext_rhs, mdwf_field* ext_opar) {
         if (r2 == MDWF_OK) {
             W.all.push_back(*f);
             if (meta) MDWF_CUDA(c, cudaMemsetAsync(meta, 0, 2 * sizeof(FieldMeta), S.st));
+            // padding rhs of the last interleave group must hold finite numbers
+            if (prec == 16 && (n & ((1 << half_ril(n, g.Ls)) - 1))) MDWF_CUDA(c, cudaMemsetAsync(mem, 0, field_bytes(g, prec, n), S.st));
         }
         return r2;
     };
@@ -141,7 +143,7 @@ RhsList chunk_of(const RhsList& act, int c0, int n) {
 
 SpinorView no_view() {
     SpinorView v;
-    v.v = nullptr; v.m = nullptr; v.rs = 0;
+    memset(&v, 0, sizeof(v));
     return v;
 }
 

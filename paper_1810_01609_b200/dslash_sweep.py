@@ -71,6 +71,7 @@ def main():
     ap.add_argument("--rotate", type=int, default=4)
     ap.add_argument("--zc", type=int, default=0)
     ap.add_argument("--dagger", type=int, default=0)
+    ap.add_argument("--tile", default="", help="fp16 stencil box and warps per block: lx,ly,lz,lt[,warps]")
     ap.add_argument("--meas", action="store_true", help="time the sequential-source and nucleon 2-pt kernels instead")
     a = ap.parse_args()
     cfg = synth.CONFIGS[a.config]
@@ -80,6 +81,9 @@ def main():
         peak = float(json.load(open(pk))["hbm_gbs"])
     ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
     ctx.mdwf_set_tiling(a.zc)
+    if a.tile:
+        t = [int(v) for v in a.tile.split(",")]
+        ctx.mdwf_set_hop16_tile(t[0], t[1], t[2], t[3], t[4] if len(t) > 4 else 0)
     if a.meas:
         measurement_kernels(ctx, cfg, a.iters, peak)
         return
