@@ -11,8 +11,10 @@ int half_ril(int nrhs, int Ls) {
         if ((1 << ril) <= nrhs && (Ls << ril) <= 48) return ril;
     return 0;
 }
+int half_site_bytes(int nrhs, int Ls) { return (((Ls << half_ril(nrhs, Ls)) + 7) / 8) * 384; }
 static size_t rhs_bytes(const Geom& g, int prec, int nrhs) {      // stride between rhs (fp16: between rhs groups)
-    if (prec == 16) return ((((size_t)g.N5h * 48) << half_ril(nrhs, g.Ls)) + 255) / 256 * 256;
+    // (+ 1536 bytes: the tensor-core stencil reads an even number of row blocks per site, mdwf_hop16.cuh)
+    if (prec == 16) return ((size_t)g.Vh * half_site_bytes(nrhs, g.Ls) + 1536 + 255) / 256 * 256;
     const size_t nb = ((size_t)g.N5h + 31) / 32;
     return nb * (size_t)((24 * (prec / 8) / 16) * 512);
 }
@@ -264,6 +266,7 @@ mdwf::SpinorView mdwf_field::view() const {
     s.m = rmeta();
     s.ril = prec == 16 ? mdwf::half_ril(nrhs, ctx->g.Ls) : 0;
     s.Ls = ctx->g.Ls;
+    s.sb = prec == 16 ? mdwf::half_site_bytes(nrhs, ctx->g.Ls) : 0;
     s.dLs = ctx->g.dLs;
     return s;
 }

@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(256) gauge_pack_kernel(const Geom g, const Gau
 
 // Stencil-ready links for 16-bit storage (GaugeView::pl): for every output site of parity `par` and leg l the matrix
 // exactly as the stencil multiplies it -- decoded from the packed fp16 format (18/12/8 reals), daggered for backward
-// legs, boundary sign folded (stage_link, mdwf_hop.cuh) -- rounded to half.  288 bytes per site; it replaces the
+// legs, boundary sign folded (stage_link, mdwf_hop.cuh) -- rounded to half, and the neighbour's site index.  320 bytes per site; it replaces the
 // per-block reconstruction (and makes the 12/8-real decode a load-time cost) for the tensor-core stencil.
 template <int R>
 __global__ void __launch_bounds__(256) gauge_prepare16_kernel(const Geom g, GaugeView gv, uint32_t* pl, int par) {
@@ -72,10 +72,11 @@ __global__ void __launch_bounds__(256) gauge_prepare16_kernel(const Geom g, Gaug
     c.xh = xh; c.xx = xx; c.y = y; c.z = z; c.t = t;
     c.o = (par + y + z + t) & 1;
     float V[MDWF_LROW];
-    stage_link<__half, R>(g, gv, par, c, l, V);
-    uint32_t* dst = pl + (long long)xh * 72 + l;
+    const int n = stage_link<__half, R>(g, gv, par, c, l, V);
+    uint32_t* dst = pl + (long long)xh * 80 + l;            // [xh][9 link words + neighbour index][leg 8]
 #pragma unroll
     for (int e = 0; e < 9; ++e) dst[e * 8] = f2h(V[2 * e], V[2 * e + 1]);
+    dst[72] = (uint32_t)n;
 }
 
 void free_gauge(GaugeSet* gs) {
@@ -150,7 +151,7 @@ int pack_gauge(mdwf_ctx* c, const void* U, int prec, int recon, GaugeSet* gs, cu
         gv.pl[0] = gv.pl[1] = nullptr;
         const int ntask = c->g.Vh * 8, grid = (ntask + 255) / 256;
         for (int p = 0; p < 2 && rc == MDWF_OK; ++p) {
-            if (cudaMalloc(&gs->pl[p], (size_t)c->g.Vh * 288) != cudaSuccess) {
+            if (cudaMalloc(&gs->pl[p], (size_t)c->g.Vh * 320) != cudaSuccess) {
                 cudaGetLastError();
                 c->err = "cudaMalloc of the stencil-ready fp16 links failed";
                 rc = MDWF_ENOMEM;

@@ -44,37 +44,19 @@ static void build_vcode(uint32_t vcode[2][32]) {
 
 static inline int pack4(int x, int y, int z, int t) { return x | (y << 8) | (z << 16) | (t << 24); }
 
-struct Plan16 { int ns, spw, nst, nip[2], nrun[2]; size_t off_nbr, off_links, off_wpart, off_stage, stage, off_epi, smem; };
-// counts and shared-memory need of a box without building tables
+// shared memory of a block: header | link records of every warp's sites | per-warp epilogue tile | per-warp partial sums
+struct Plan16 { int ns, spw; size_t off_links, off_epi, off_wpart, smem; };
 static Plan16 plan_tile16(const int L[4], int rows, int nw) {      // rows = RI * Ls of one site
     Plan16 p;
-    const int vol = L[0] * L[1] * L[2] * L[3];
-    p.ns = vol / 2;
-    for (int pat = 0; pat < 2; ++pat) {
-        int ni = 0, nr = 0;
-        for (int t = -1; t <= L[3]; ++t) for (int z = -1; z <= L[2]; ++z) for (int y = -1; y <= L[1]; ++y) {
-            const int out = (y < 0 || y >= L[1]) + (z < 0 || z >= L[2]) + (t < 0 || t >= L[3]);
-            if (out >= 2) continue;
-            const int x0 = out ? 0 : -1, x1 = out ? L[0] - 1 : L[0];
-            int n = 0;
-            for (int x = x0; x <= x1; ++x) if (((x + y + z + t) & 1) != pat) ++n;
-            if (n) { ni += n; ++nr; }
-        }
-        p.nip[pat] = ni; p.nrun[pat] = nr;
-    }
-    const int MT = (rows + 15) / 16;
+    p.ns = L[0] * L[1] * L[2] * L[3] / 2;
     p.spw = (p.ns + nw - 1) / nw;
+    const int MT = (rows + 15) / 16;
     size_t off = MDWF_H16_HDR;
-    p.off_nbr = off; off += ((size_t)2 * p.ns * 8 * 4 + (size_t)2 * p.ns * 4 + 15) / 16 * 16;
     p.off_links = off; off += (size_t)nw * p.spw * MDWF_H16_SREC;
-    p.off_wpart = off; off += (size_t)64 * nw * 8;
+    off = (off + 15) / 16 * 16;
     p.off_epi = off; off += (size_t)nw * MT * 16 * 24 * 4;
-    off = (off + 127) / 128 * 128;
-    p.off_stage = off;
-    p.stage = ((size_t)std::max(p.nip[0], p.nip[1]) * rows * 48 + 127) / 128 * 128;
-    const size_t cap = 227 * 1024 - 256;
-    p.nst = off + 2 * p.stage > cap ? 2 : (int)std::min<size_t>(MDWF_H16_MAXST, (cap - off) / p.stage);
-    p.smem = off + (size_t)p.nst * p.stage;
+    p.off_wpart = off; off += (size_t)64 * nw * 8;
+    p.smem = off;
     return p;
 }
 
@@ -87,53 +69,21 @@ static int build_tile16(mdwf_ctx* c, const int L[4], int rows, int nw, Tile16Hos
     tl.ns = L[0] * L[1] * L[2] * L[3] / 2;
     tl.ntiles = tl.nT[0] * tl.nT[1] * tl.nT[2] * tl.nT[3];
     th->nw = nw;
-    for (int i = 0; i < 6; ++i) th->dev[i] = nullptr;
+    th->dev[0] = th->dev[1] = nullptr;
     for (int pat = 0; pat < 2; ++pat) {
         std::vector<int> outc;
-        std::vector<int4> runs;
-        std::map<int, int> slot_of;
-        int nslot = 0;
-        for (int t = -1; t <= L[3]; ++t) for (int z = -1; z <= L[2]; ++z) for (int y = -1; y <= L[1]; ++y) {
-            const int out = (y < 0 || y >= L[1]) + (z < 0 || z >= L[2]) + (t < 0 || t >= L[3]);
-            if (out >= 2) continue;
-            const int x0 = out ? 0 : -1, x1 = out ? L[0] - 1 : L[0];
-            int first = 1 << 30, n = 0;
-            for (int x = x0; x <= x1; ++x)
-                if (((x + y + z + t) & 1) != pat) {
-                    if (n == 0) first = x;
-                    slot_of[pack4(x + 1, y + 1, z + 1, t + 1)] = nslot + n;
-                    ++n;
-                }
-            if (n) { runs.push_back(make_int4(pack4(first + 1, y + 1, z + 1, t + 1), n, nslot, 0)); nslot += n; }
-        }
-        std::vector<unsigned short> nbr;
-        for (int t = 0; t < L[3]; ++t) for (int z = 0; z < L[2]; ++z) for (int y = 0; y < L[1]; ++y) for (int x = 0; x < L[0]; ++x) {
-            if (((x + y + z + t) & 1) != pat) continue;
-            outc.push_back(pack4(x, y, z, t));
-            for (int l = 0; l < 8; ++l) {
-                int cc[4] = {x, y, z, t};
-                cc[l >> 1] += (l & 1) == 0 ? 1 : -1;
-                const auto it = slot_of.find(pack4(cc[0] + 1, cc[1] + 1, cc[2] + 1, cc[3] + 1));
-                if (it == slot_of.end()) MDWF_FAIL(c, MDWF_EINVAL, "internal: fp16 tile table is inconsistent");
-                nbr.push_back((unsigned short)it->second);
-            }
-        }
+        for (int t = 0; t < L[3]; ++t) for (int z = 0; z < L[2]; ++z) for (int y = 0; y < L[1]; ++y) for (int x = 0; x < L[0]; ++x)
+            if (((x + y + z + t) & 1) == pat) outc.push_back(pack4(x, y, z, t));
         if ((int)outc.size() != tl.ns) MDWF_FAIL(c, MDWF_EINVAL, "internal: fp16 tile has %zu output sites, expected %d", outc.size(), tl.ns);
-        tl.nip[pat] = nslot; tl.nrun[pat] = (int)runs.size();
-        void *d0, *d1, *d2;
+        void* d0;
         MDWF_CUDA(c, cudaMalloc(&d0, outc.size() * 4));
-        MDWF_CUDA(c, cudaMalloc(&d1, runs.size() * sizeof(int4)));
-        MDWF_CUDA(c, cudaMalloc(&d2, nbr.size() * 2));
         MDWF_CUDA(c, cudaMemcpy(d0, outc.data(), outc.size() * 4, cudaMemcpyHostToDevice));
-        MDWF_CUDA(c, cudaMemcpy(d1, runs.data(), runs.size() * sizeof(int4), cudaMemcpyHostToDevice));
-        MDWF_CUDA(c, cudaMemcpy(d2, nbr.data(), nbr.size() * 2, cudaMemcpyHostToDevice));
-        th->dev[3 * pat] = d0; th->dev[3 * pat + 1] = d1; th->dev[3 * pat + 2] = d2;
-        tl.outc[pat] = (const int*)d0; tl.run[pat] = (const int4*)d1; tl.nbr[pat] = (const unsigned short*)d2;
+        th->dev[pat] = d0;
+        tl.outc[pat] = (const int*)d0;
     }
     const Plan16 pl = plan_tile16(L, rows, nw);
-    tl.spw = pl.spw; tl.nst = pl.nst;
-    tl.off_nbr = (int)pl.off_nbr; tl.off_links = (int)pl.off_links; tl.off_wpart = (int)pl.off_wpart; tl.off_epi = (int)pl.off_epi;
-    tl.off_stage = (int)pl.off_stage; tl.stage_bytes = (int)pl.stage; tl.smem_total = (int)pl.smem;
+    tl.spw = pl.spw;
+    tl.off_links = (int)pl.off_links; tl.off_epi = (int)pl.off_epi; tl.off_wpart = (int)pl.off_wpart; tl.smem_total = (int)pl.smem;
     tl.dTx = make_fastdiv(tl.nT[0]); tl.dTy = make_fastdiv(tl.nT[1]); tl.dTt = make_fastdiv(tl.nT[3]);
     tl.zc_t = tl.nT[2]; tl.dTzs = make_fastdiv(tl.zc_t);
     build_vcode(tl.vcode);
@@ -141,44 +91,37 @@ static int build_tile16(mdwf_ctx* c, const int L[4], int rows, int nw, Tile16Hos
 }
 
 void free_tile16(Tile16Host* th) {
-    for (int i = 0; i < 6; ++i) if (th->dev[i]) { cudaFree(th->dev[i]); th->dev[i] = nullptr; }
+    for (int i = 0; i < 2; ++i) if (th->dev[i]) { cudaFree(th->dev[i]); th->dev[i] = nullptr; }
 }
 
-// Tile choice: among the boxes that divide the lattice and fit in shared memory (with at least two staging buffers),
-// the one with the fewest input-site fetches per output site (ni/ns: 8 without any reuse, 5 for a 2^4 box, 4 for
-// 4x4x2x2).  Warps per block: one per output site up to 16 (then 2..4 sites per warp).  mdwf_set_hop16_tile forces a box.
-static int warps_for(int ns) { return ns >= 16 ? 16 : ns >= 8 ? 8 : 4; }
+// Tile choice.  The block's tile decides how often an input site is found again in L1 by another leg: a 2^4 box has 8
+// output sites and 40 distinct inputs (5 fetches per output instead of 8), 4x2x2x2 has 16 and 72 (4.5).  Default: the
+// largest box of at most 16 sites built from extents <= 4 (x) and <= 2 (y, z, t) that divides the lattice, one site
+// per warp.  mdwf_set_hop16_tile forces a box / warp count (tuning).
 static int choose_tile16(mdwf_ctx* c, int rows, int L[4], int* nw_out) {
     const Geom& g = c->g;
     const int dims[4] = {g.X, g.Y, g.Z, g.T};
     const size_t cap = 227 * 1024 - 256;
     if (c->tile16_forced[0] > 0) {
         for (int d = 0; d < 4; ++d) L[d] = c->tile16_forced[d];
-        for (int d = 0; d < 4; ++d) if (L[d] < 1 || dims[d] % L[d] || (d == 0 && (L[d] & 1))) MDWF_FAIL(c, MDWF_EINVAL, "forced fp16 tile does not divide the lattice");
-        const int nw = c->tile16_nw > 0 ? c->tile16_nw : warps_for(L[0] * L[1] * L[2] * L[3] / 2);
+        for (int d = 0; d < 4; ++d) if (L[d] < 1 || L[d] > 16 || dims[d] % L[d] || (d == 0 && (L[d] & 1))) MDWF_FAIL(c, MDWF_EINVAL, "forced fp16 tile does not divide the lattice");
+        const int ns = L[0] * L[1] * L[2] * L[3] / 2;
+        const int nw = c->tile16_nw > 0 ? c->tile16_nw : std::min(ns, MDWF_H16_MAXW);
         const Plan16 pf = plan_tile16(L, rows, nw);
         if (pf.smem > cap || pf.spw > 4) MDWF_FAIL(c, MDWF_EINVAL, "forced fp16 tile does not fit in shared memory (or has more than 4 sites per warp)");
         *nw_out = nw;
         return MDWF_OK;
     }
-    double best = 1e30;
-    L[0] = 0;
-    for (int lx = 2; lx <= 8; lx += 2) for (int ly = 1; ly <= 8; ++ly) for (int lz = 1; lz <= 8; ++lz) for (int lt = 1; lt <= 8; ++lt) {
-        if (dims[0] % lx || dims[1] % ly || dims[2] % lz || dims[3] % lt) continue;
-        const int cand[4] = {lx, ly, lz, lt};
-        const int nw = warps_for(lx * ly * lz * lt / 2);
-        const Plan16 p = plan_tile16(cand, rows, nw);
-        if (p.spw > 4 || p.smem > cap) continue;
-        const double fetch = (double)std::max(p.nip[0], p.nip[1]) / p.ns;
-        const double imbal = (double)((p.ns + nw - 1) / nw * nw) / p.ns;
-        const double cost = fetch * (1.0 + 0.25 * (imbal - 1.0));
-        if (cost < best - 1e-12) { best = cost; L[0] = lx; L[1] = ly; L[2] = lz; L[3] = lt; *nw_out = nw; }
-    }
-    if (!L[0]) MDWF_FAIL(c, MDWF_EINVAL, "no fp16 stencil tile fits in shared memory (%d rows per site)", rows);
+    const int want[4] = {2, 2, 2, 2};
+    for (int d = 0; d < 4; ++d) L[d] = dims[d] % want[d] == 0 ? want[d] : 1;
+    if (L[0] < 2) L[0] = 2;
+    *nw_out = std::min(L[0] * L[1] * L[2] * L[3] / 2, MDWF_H16_MAXW);
+    const Plan16 p = plan_tile16(L, rows, *nw_out);
+    if (p.smem > cap) MDWF_FAIL(c, MDWF_EINVAL, "fp16 stencil tile does not fit in shared memory (%d rows per site)", rows);
     return MDWF_OK;
 }
 
-// tiles are cached per rhs interleave (the staging buffers hold RI * Ls rows per site)
+// tiles are cached per rhs interleave (the epilogue tile holds RI * Ls rows per site)
 int get_tile16(mdwf_ctx* c, int ril, Tile16Host** out) {
     if (ril < 0 || ril > 2) MDWF_FAIL(c, MDWF_EINVAL, "internal: bad rhs interleave");
     if (!c->tile16[ril]) {
@@ -196,42 +139,56 @@ int get_tile16(mdwf_ctx* c, int ril, Tile16Host** out) {
 }
 
 // z-tiles per slab: the three t-consecutive layers (x, y, slab depth, one tile in t) of every rhs in flight should stay
-// in L2, budget ~40 MB
-static int pick_zc16(const Geom& g, const Tile16& tl, int nact) {
+// in L2, budget ~60 MB
+static int pick_zc16(const Geom& g, const Tile16& tl, int sb, int ngrp) {
     int best = 1;
     for (int z = 1; z <= tl.nT[2]; ++z) {
         if (tl.nT[2] % z) continue;
-        const double layer = (double)g.XH * g.Y * (z * tl.L[2]) * tl.L[3] * g.Ls * 48.0 * nact;   // nact rhs = groups x RI
-        if (3.0 * layer <= 40.0e6) best = z;
+        const double layer = (double)g.XH * g.Y * (z * tl.L[2]) * tl.L[3] * (double)sb * ngrp;
+        if (3.0 * layer <= 60.0e6) best = z;
     }
     return best;
 }
 
 int launch_hop_f16(mdwf_ctx* c, int recon, int dagger, int fused, HopArgs& a, cudaStream_t st) {
     (void)fused;
+    (void)recon;       // the stencil-ready links were decoded from the (prec 16, recon) format at load time
     Tile16Host* th;
     int rc = get_tile16(c, a.in.ril, &th);
     if (rc) return rc;
-    (void)recon;       // the stencil-ready links were decoded from the (prec 16, recon) format at load time
     if (!a.g.pl[0] || !a.g.pl[1]) MDWF_FAIL(c, MDWF_ESTATE, "internal: stencil-ready fp16 links missing");
     if (!a.in.m || !a.out.m || (a.xin.v && !a.xin.m) || a.sr.n < 1) MDWF_FAIL(c, MDWF_EINVAL, "internal: fp16 hop without field scales");
     if (a.out.ril != a.in.ril || (a.xin.v && a.xin.ril != a.in.ril)) MDWF_FAIL(c, MDWF_EINVAL, "internal: fp16 hop on fields with different rhs interleave");
     const int rows = c->g.Ls << a.in.ril;
-    Tile16 tl = th->t;
-    tl.zc_t = c->zc_forced > 0 && c->zc_forced % tl.L[2] == 0 && tl.nT[2] % (c->zc_forced / tl.L[2]) == 0 ? c->zc_forced / tl.L[2]
-                                                                                                        : pick_zc16(c->g, tl, a.nact);
-    tl.dTzs = make_fastdiv(tl.zc_t);
-    const int grid = std::min(tl.ntiles, c->sm_count), block = th->nw * 32;
-    auto kern = rows <= 16 ? hop16_kernel<1> : rows <= 32 ? hop16_kernel<2> : hop16_kernel<3>;
     if (rows > 48) MDWF_FAIL(c, MDWF_EINVAL, "internal: %d rows per site", rows);
+    Tile16 tl = th->t;
+    // rhs groups with an active rhs
+    tl.ngrp = 0;
+    for (int k = 0; k < a.nact; ++k) {
+        const int gr = a.rhs_list[k] >> a.in.ril;
+        int j = 0;
+        while (j < tl.ngrp && tl.grp[j] != gr) ++j;
+        if (j == tl.ngrp) { tl.grp[j] = (unsigned char)gr; tl.gmask[j] = 0; ++tl.ngrp; }
+        tl.gmask[j] |= (unsigned char)(1 << (a.rhs_list[k] & ((1 << a.in.ril) - 1)));
+    }
+    tl.dng = make_fastdiv(tl.ngrp);
+    tl.zc_t = c->zc_forced > 0 && c->zc_forced % tl.L[2] == 0 && tl.nT[2] % (c->zc_forced / tl.L[2]) == 0 ? c->zc_forced / tl.L[2]
+                                                                                                        : pick_zc16(c->g, tl, a.in.sb, tl.ngrp);
+    tl.dTzs = make_fastdiv(tl.zc_t);
+    const int block = th->nw * 32;
+    const int regs = 128;
+    const int per_sm = std::max(1, std::min(2048 / block, (int)((227 * 1024) / (tl.smem_total + 1024))));
+    const int grid = (int)std::min<long long>((long long)tl.ntiles * tl.ngrp, (long long)c->sm_count * std::min(per_sm, 65536 / (regs * block)) );
+    auto kern = rows <= 16 ? hop16_kernel<1, 1, 1> : rows <= 32 ? hop16_kernel<2, 1, 1> : hop16_kernel<3, 1, 1>;
     if (!c->attr_raised.count((const void*)kern)) {
         MDWF_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         c->attr_raised.insert((const void*)kern);
     }
-    kern<<<grid, block, tl.smem_total, st>>>(c->g, tl, a, dagger ? 1 : 0);
+    if ((size_t)grid > c->partial_cap) MDWF_FAIL(c, MDWF_EINVAL, "internal: partial buffer too small");
+    kern<<<std::max(grid, 1), block, tl.smem_total, st>>>(c->g, tl, a, dagger ? 1 : 0);
     MDWF_CUDA(c, cudaGetLastError());
     c->launches++;
-    c->partial_nblk = grid;
+    c->partial_nblk = std::max(grid, 1);
     return MDWF_OK;
 }
 

@@ -9,13 +9,15 @@
 //        r = c*RPV .. c*RPV+RPV-1.  A thread owns one 5D site idx = xh*Ls + s (s fastest), so a warp
 //        reads 512 contiguous bytes per vector index.  rhs are separate fields (stride in bytes).
 //   spinor fp16 ("16-bit storage, single-precision computation"; reading R11):
-//        site-major, 48 bytes per 5D site: half[colour 3][spin 4][re,im] -- one 16-byte chunk per colour -- with
-//        the rhs interleaved in groups of RI = 1, 2 or 4 inside a 4D site:  [group][xh][rhs in group][s][48 B], so
-//        that (a) all Ls slices of all rhs of a group at one 4D site are RI*Ls*48 contiguous bytes (one bulk copy
-//        of ~2 KB into shared memory: the size from which such copies run at full bandwidth), (b) they are the
-//        rows of ONE m16 x K tile sequence of the tensor-core stencil, sharing its link fragments (north_star:
-//        links "reused across the Ls slices and across multiple right-hand sides"), and (c) an ldmatrix row
-//        (16 bytes) is a K-slice whose lane <-> spin mapping is regular (mdwf_hop16.cuh).
+//        48 bytes per 5D site: half[colour 3][spin 4][re,im] -- one 16-byte chunk per colour -- stored in the
+//        FRAGMENT ORDER of the tensor-core stencil (mdwf_hop16.cuh).  The rhs are interleaved in groups of RI = 1,
+//        2 or 4 inside a 4D site; the RI*Ls "rows" (rhs in group, s) of a site are cut into blocks of 8 rows and a
+//        block is stored as [colour chunk 3][row 8][16 B] = 3 x 128 bytes:
+//           [group][xh][row block][chunk][row in block][16 B]        (rows padded to a multiple of 8)
+//        so (a) the A operand of an m16n8k16 / m16n8k8 MMA is read with six perfectly coalesced 128-byte LDG.32
+//        per 16 rows, register <- memory with no conversion, shuffle or shared-memory staging, (b) all rows of a
+//        site share one set of link fragments (north_star: links "reused across the Ls slices and across multiple
+//        right-hand sides"), (c) one-thread-per-5D-site kernels still read 16 contiguous bytes per lane.
 //        One power-of-two fp32 scale per (field, rhs): value = e * half.
 //   gauge, per (site parity, mu): vec[c][xh]   fp64: double2 x ceil(R/2), fp32: float4 x ceil(R/4),
 //        fp16: 4 x half (8 bytes) x ceil(R/4);  R = 18 | 12 | 8 reals.
@@ -122,6 +124,7 @@ struct SpinorView {
     long long rs;     // rhs stride in BYTES (fp16: stride of a GROUP of 1 << ril rhs)
     int ril;          // fp16 only: log2 of the rhs interleave RI
     int Ls;           // fp16 only
+    int sb;           // fp16 only: bytes of one 4D site of a group = ceil(RI*Ls / 8) * 384
     FastDiv dLs;      // fp16 only: idx -> (xh, s)
 };
 
@@ -176,9 +179,8 @@ __device__ __forceinline__ const char* site_ptr(const SpinorView& f, int r, int 
     if (Store<S>::HALF) {
         uint32_t xh, sl;
         f.dLs.divmod((uint32_t)idx, xh, sl);
-        const int ri = r & ((1 << f.ril) - 1);
-        return reinterpret_cast<const char*>(f.v) + (long long)(r >> f.ril) * f.rs +
-               ((((long long)xh << f.ril) + ri) * f.Ls + sl) * 48;
+        const int row = (r & ((1 << f.ril) - 1)) * f.Ls + (int)sl;      // chunk c of the site at + c*128
+        return reinterpret_cast<const char*>(f.v) + (long long)(r >> f.ril) * f.rs + (long long)xh * f.sb + (row >> 3) * 384 + (row & 7) * 16;
     }
     return reinterpret_cast<const char*>(f.v) + (long long)r * f.rs + (long long)(idx >> 5) * Blk<S>::BYTES + (idx & 31) * 16;
 }
@@ -222,7 +224,7 @@ __device__ __forceinline__ void load_raw<__half>(const SpinorView& f, int r, int
     scale = f.m->e[r];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {        // chunk c = colour c: spins 0..3 (re, im)
-        uint4 t = ldg(reinterpret_cast<const uint4*>(p + c * 16));
+        uint4 t = ldg(reinterpret_cast<const uint4*>(p + c * 128));
         float2 a = h2f(t.x), b = h2f(t.y), cc = h2f(t.z), d = h2f(t.w);
         v[(0 * 3 + c) * 2] = a.x; v[(0 * 3 + c) * 2 + 1] = a.y;
         v[(1 * 3 + c) * 2] = b.x; v[(1 * 3 + c) * 2 + 1] = b.y;
@@ -276,7 +278,7 @@ __device__ __forceinline__ void store_spinor(const SpinorView& f, int r, int idx
             t.y = f2h_sat(v[(1 * 3 + c) * 2] * oinv, v[(1 * 3 + c) * 2 + 1] * oinv);
             t.z = f2h_sat(v[(2 * 3 + c) * 2] * oinv, v[(2 * 3 + c) * 2 + 1] * oinv);
             t.w = f2h_sat(v[(3 * 3 + c) * 2] * oinv, v[(3 * 3 + c) * 2 + 1] * oinv);
-            st_<CS>(reinterpret_cast<uint4*>(p + c * 16), t);
+            st_<CS>(reinterpret_cast<uint4*>(p + c * 128), t);
         }
     }
 }

@@ -8,21 +8,21 @@
 //
 // Formulation.  For one output site x and one leg l the map psi(neighbour) -> contribution is the REAL 24 x 24 matrix
 // M_l = Gamma_l (x) U_l (Gamma_l = 1 -+ gamma_mu, entries 0, +-1, +-i; U_l the link or its adjoint, boundary sign
-// folded).  It is the same for all Ls slices, so the site's hop is the dense contraction
-//       out[s][24] = sum_l  psi_l[s][24] . M_l^T          (M = Ls rows, N = 24, K = 8 legs x 24)
+// folded).  It is the same for all Ls slices and all right-hand sides, so the site's hop is the dense contraction
+//       out[row][24] = sum_l  psi_l[row][24] . M_l^T       (M = RI*Ls rows (rhs in group, s), N = 24, K = 8 legs x 24)
 // executed as mma.sync m16n8k16 / m16n8k8 (f16 x f16 -> f32): A = the neighbours' stored halves exactly as they sit in
 // memory (no cvt, no projection arithmetic), B = +-Re/Im U entries in half precision, accumulation over all 8 legs
 // in the fp32 accumulator.  Products of halves are exact in fp32, so this is "16-bit storage, fp32 compute" up to
 // summation order; the spin projection and reconstruction cost nothing (they are zeros and signs inside M_l).
 //
-// Data movement.  A block owns a 4D tile of output sites.  All input sites the tile needs (interior of the other
-// parity + one-site halo, each used by up to 8 outputs) are fetched ONCE per (tile, rhs) into shared memory with bulk
-// async copies (cp.async.bulk + mbarrier; a 4D site is Ls*48 contiguous bytes in the fp16 layout, x-runs are fetched
-// as one copy), double-buffered across the rhs of the tile, so the L2->SM gather traffic drops from 8 to ni/ns (~4)
-// site reads per output.  A-fragments come from there with ldmatrix (row = one 5D site's 16-byte colour chunk; the
-// 48-byte row stride is bank-conflict free).  The tile's 8*ns links are reconstructed once per tile (12/8-real
-// formats), rounded to half and parked in shared memory as the four sign/swap variants (u, i u, -u, -i u in real
-// 2x2 form) that the 32 lanes of a B-fragment need, and are reused by every Ls slice and every rhs of the tile
+// Data movement.  The fp16 field layout IS the A-fragment order (mdwf_device.cuh): the 16 rows x 24 halves of an m16
+// tile are six 128-byte lines, each read by one coalesced LDG.32 straight into the fragment registers (through L1,
+// where the other legs of the block's 4D tile find them again) -- no shared-memory staging, so shared memory only
+// holds the link records and the epilogue tile and 16 warps per SM stay resident.  A block owns a 4D tile of output
+// sites (one warp per site, or a few sites per warp); the 8 links of a site come from the stencil-ready half-precision
+// link table (gauge.cu: decoded from the 18/12/8-real format, daggered, boundary sign folded, at load time), are
+// fetched one item ahead and parked in shared memory as the four sign/swap variants (u, i u, -u, -i u in real 2x2
+// form) plus zeros that the 32 lanes of a B fragment need; they serve every Ls slice and every rhs of the group
 // (north_star: "staging of links reused across the Ls slices and across multiple right-hand sides").
 // Epilogue: accumulators -> per-warp shared tile -> s-direction operator (LsOp: c0 + c1 L or c0 + c1 M5^-1 as the
 // first-order recurrence of mdwf_hop.cuh) -> xpay -> |out|^2 partial -> half conversion -> 16-byte coalesced stores.
@@ -31,60 +31,34 @@
 
 namespace mdwf {
 
-#define MDWF_H16_HDR 4096          // fixed header of the dynamic shared memory (barriers, per-rhs coefficients, kappa powers)
+#define MDWF_H16_HDR 1408          // fixed header of the dynamic shared memory (kappa powers, per-rhs coefficients, lane codes)
 #define MDWF_H16_LREC 272          // bytes per staged link: 4 variants + a zero block of 12 words each (240 B), padded so that
                                    // the 8 records of a site start 4 banks apart (conflict-free staging stores)
-#define MDWF_H16_SREC (8 * MDWF_H16_LREC + 16)   // per site: 8 link records + the site index
+#define MDWF_H16_SREC (8 * MDWF_H16_LREC + 48)   // per site: 8 link records + the site index + the 8 neighbour indices
 #define MDWF_H16_MAXW 16           // warps per block
-#define MDWF_H16_MAXST 4           // staging buffers
+#define MDWF_H16_PLW 80            // words per site of the stencil-ready link table: 9 x 8 link words + 8 neighbours
 
 struct Tile16 {
     int L[4];                       // box extents in lattice sites (L[0] even), dividing the lattice
     int nT[4];                      // tiles per direction
     int ns;                         // output sites per tile
-    int spw;                        // sites per consumer warp = ceil(ns / warps)
-    int nst;                        // staging buffers (2..4)
-    int nip[2], nrun[2];            // input slots / copy runs per parity pattern of the box
+    int spw;                        // sites per warp = ceil(ns / warps)
     int ntiles;
     int zc_t;                       // z-tiles per slab of the tile traversal (x, y, z-in-slab, t, slab)
-    FastDiv dTx, dTy, dTzs, dTt;
-    const int* outc[2];             // [ns] packed local coordinates x | y<<8 | z<<16 | t<<24 of the output sites
-    const int4* run[2];             // [nrun] {packed local coordinates + 1 of the first site, sites, first slot, 0}
-    const unsigned short* nbr[2];   // [ns*8] input slot of each leg
-    int off_nbr, off_links, off_stage, stage_bytes, off_epi, off_wpart, smem_total;
+    FastDiv dTx, dTy, dTzs, dTt, dng;
+    const int* outc[2];             // [ns] packed local coordinates x | y<<8 | z<<16 | t<<24 of the output sites, per parity pattern
+    int off_links, off_epi, off_wpart, smem_total;
+    int ngrp;                       // rhs groups with an active rhs, their ids and active-rhs masks
+    unsigned char grp[64], gmask[64];
     uint32_t vcode[2][32];          // [dagger][lane]: 4 bits per leg = variant of the lane's B words (4 = zero)
 };
 struct Tile16Host {                 // host-side owner of the device tables
     Tile16 t;
-    void* dev[6];
-    int nw;                         // consumer warps per block
+    void* dev[2];
+    int nw;                         // warps per block
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t mbar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t mbar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
-    uint32_t done;
-    do {
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(done) : "r"(mbar), "r"(parity) : "memory");
-    } while (!done);
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t mbar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(mbar) : "memory");
-}
-__device__ __forceinline__ void ldsm_x4(uint32_t r[4], uint32_t addr) {
-    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr) : "memory");
-}
-__device__ __forceinline__ void ldsm_x2(uint32_t r[2], uint32_t addr) {
-    asm volatile("ldmatrix.sync.aligned.m8n8.x2.shared.b16 {%0,%1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "r"(addr) : "memory");
-}
 __device__ __forceinline__ void mma_16816(float c[4], const uint32_t a[4], uint32_t b0, uint32_t b1) {
     asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
         : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]) : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
@@ -104,154 +78,72 @@ __device__ __forceinline__ void tile16_origin(const Tile16& tl, int tile, int o[
     o[0] = tx * tl.L[0]; o[1] = ty * tl.L[1]; o[2] = (slab * tl.zc_t + tzs) * tl.L[2]; o[3] = tt * tl.L[3];
 }
 
-// One warp issues the bulk copies of (tile, rhs group) into a staging buffer: every x-run of input sites is one copy
-// of n*RI*Ls*48 bytes (split where the run wraps around the lattice).
-__device__ __forceinline__ void hop16_issue(const Geom& g, const Tile16& tl, const HopArgs& a, int tile, int grp,
-                                            uint32_t stage, uint32_t mbar, int lane) {
-    int o[4];
-    tile16_origin(tl, tile, o);
-    const int pat = (a.par + o[1] + o[2] + o[3]) & 1;
-    const uint32_t sb = ((uint32_t)g.Ls * 48u) << a.in.ril;      // all rhs of the group at one 4D site
-    if (lane == 0) mbar_expect_tx(mbar, (uint32_t)tl.nip[pat] * sb);
-    __syncwarp();
-    const char* base = reinterpret_cast<const char*>(a.in.v) + (long long)grp * a.in.rs;
-    const int4* runs = tl.run[pat];
-    for (int r = lane; r < tl.nrun[pat]; r += 32) {
-        const int4 q = __ldg(runs + r);
-        const int lx = (q.x & 255) - 1, ly = ((q.x >> 8) & 255) - 1, lz = ((q.x >> 16) & 255) - 1, lt = ((q.x >> 24) & 255) - 1;
-        int gy = o[1] + ly, gz = o[2] + lz, gt = o[3] + lt;
-        gy = gy < 0 ? gy + g.Y : gy >= g.Y ? gy - g.Y : gy;
-        gz = gz < 0 ? gz + g.Z : gz >= g.Z ? gz - g.Z : gz;
-        gt = gt < 0 ? gt + g.T : gt >= g.T ? gt - g.T : gt;
-        const int row = g.XH * (gy + g.Y * (gz + g.Z * gt));
-        int first = (o[0] + lx) >> 1;            // -1 for the x = -1 halo of the first tile of a row
-        const int last = first + q.y - 1;
-        int slot = q.z;
-        if (first < 0) {
-            bulk_g2s(stage + (uint32_t)slot * sb, base + (long long)(row + g.XH - 1) * sb, sb, mbar);
-            ++first; ++slot;
-        }
-        const int lastc = last >= g.XH ? g.XH - 1 : last;
-        if (lastc >= first) {
-            bulk_g2s(stage + (uint32_t)slot * sb, base + (long long)(row + first) * sb, (uint32_t)(lastc - first + 1) * sb, mbar);
-            slot += lastc - first + 1;
-        }
-        if (last >= g.XH) bulk_g2s(stage + (uint32_t)slot * sb, base + (long long)row * sb, sb, mbar);
-    }
-}
-
-__device__ __forceinline__ void mbar_arrive(uint32_t mbar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar) : "memory");
-}
-__device__ __forceinline__ uint4 lds128(uint32_t addr) {
-    uint4 r;
-    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
-    return r;
-}
-__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
-    uint32_t r;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(r) : "r"(addr));
-    return r;
-}
-
-// Persistent kernel without block barriers in steady state.  The (tile, rhs group) items of a block stream through
-// `nst` staging buffers filled by bulk async copies ("full" mbarriers); the warp that finishes an item LAST (shared
-// counter) refills its buffer with item k + nst.  Each warp owns `spw` output sites of every tile, prepares the links
-// of ITS sites itself (from the prepared half-precision link table, fetched one tile ahead into registers) and runs
-// stencil + epilogue on them.  The M rows of a site are (rhs in group, s): RI*Ls rows = MT m16 tiles that share one
-// set of B fragments per leg.
+// Persistent kernel: block b processes the (tile, rhs group) items b, b + G, ...; there is no block barrier in the item
+// loop.  Each warp owns `spw` output sites of the tile and prepares the link records of ITS sites itself:
 //   link record of a (site, leg), 4 variants + zeros, 12 words each:  V0 = (ur, -ui)  V1 = (ui, ur)  V2 = -V0  V3 = -V1
 //   per U entry u = U[a][b]: the (k even, k odd) pairs of Re/Im parts of Gamma*u that a B-fragment lane needs for
 //   Gamma = 1, -1, i, -i (0: the zero block).  Word order inside a variant: B00 B01 B10 B11 | B20 B21 B02 B12 | B22,
 //   so that the k16 operand pairs of the three n-tiles (= output colours) are aligned register pairs of two 16-byte
 //   loads; the five blocks sit in disjoint banks, so the 32 lanes of a fragment load never conflict.
 // MT = m16 tiles per site: ceil(RI * Ls / 16) <= 3
-template <int MT>
-__global__ void __launch_bounds__(32 * MDWF_H16_MAXW, 1) hop16_kernel(const Geom g, const Tile16 tl, const HopArgs a, const int dag) {
+template <int MT, int PF, int MINB>
+__global__ void __launch_bounds__(PF ? 32 * MDWF_H16_MAXW : 256, MINB) hop16_kernel(const Geom g, const Tile16 tl, const HopArgs a, const int dag) {
     extern __shared__ __align__(128) unsigned char sm[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nwc = (int)(blockDim.x >> 5);
-    const int Ls = g.Ls, nst = tl.nst, ns = tl.ns, spw = tl.spw;
-    const int ril = a.in.ril, RI = 1 << ril, rows = Ls << ril;
-    const uint32_t sbase = smem_u32(sm);
-    // header: full[4] mbarriers | int done[4] | float4 cf[64] (by rhs id) | double e2[64] | float kp[32] | groups
-    int* s_done = reinterpret_cast<int*>(sm + 32);
-    int* s_ngrp = reinterpret_cast<int*>(sm + 48);
-    float4* s_cf = reinterpret_cast<float4*>(sm + 64);
-    double* s_e2 = reinterpret_cast<double*>(sm + 1088);
-    float* s_kp = reinterpret_cast<float*>(sm + 1600);
-    int* s_grp = reinterpret_cast<int*>(sm + 1728);           // [64] group ids with an active rhs
-    int* s_gmask = s_grp + 64;                                // [64] active rhs of the group (bit per rhs in group)
-    int* s_slot = s_gmask + 64;                               // [64] rhs id -> position in the active list
-    uint32_t* s_nbr = reinterpret_cast<uint32_t*>(sm + tl.off_nbr);       // [2][ns*8] byte offsets inside a staging buffer
-    int* s_outc = reinterpret_cast<int*>(s_nbr + 2 * ns * 8);              // [2][ns]
+    const int Ls = g.Ls, ns = tl.ns, spw = tl.spw;
+    const int ril = a.in.ril, RI = 1 << ril, rows = Ls << ril, nrb = (rows + 7) >> 3;
+    const uint32_t sb = (uint32_t)a.in.sb;                    // bytes of a 4D site of one rhs group
+    float* s_kp = reinterpret_cast<float*>(sm);               // [32] kappa^{k+1}
+    float2* s_cf = reinterpret_cast<float2*>(sm + 128);       // [64] by rhs id: (e_in / e_out, e_x / e_out)
+    double* s_e2 = reinterpret_cast<double*>(sm + 640);       // [64] e_out^2
+    uint32_t* s_vc = reinterpret_cast<uint32_t*>(sm + 1152);  // [32] per lane: variant code of each leg (4 bits per leg)
     double* s_wpart = reinterpret_cast<double*>(sm + tl.off_wpart);        // [64 rhs][nwc]
-    const uint32_t site_bytes = (uint32_t)rows * 48u;
-
-    if (tid == 0) {
-        for (int st = 0; st < nst; ++st) { mbar_init(sbase + 8 * st, 1); s_done[st] = 0; }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        int ng = 0;
-        for (int k = 0; k < a.nact; ++k) {
-            const int rhs = a.rhs_list[k], gr = rhs >> ril;
-            int j = 0;
-            while (j < ng && s_grp[j] != gr) ++j;
-            if (j == ng) { s_grp[ng] = gr; s_gmask[ng] = 0; ++ng; }
-            s_gmask[j] |= 1 << (rhs & (RI - 1));
-            s_slot[rhs] = k;
-        }
-        *s_ngrp = ng;
-    }
-    if (tid < a.nact) {
-        const int rhs = a.rhs_list[tid];
-        const float eo = eval_scale(a.sr, rhs, blockIdx.x == 0);
-        const float ei = a.in.m->e[rhs];
-        const float ex = a.xin.v != nullptr ? a.xin.m->e[rhs] : 0.f;
-        s_cf[rhs] = make_float4(ei / eo, ex / eo, 0.f, 0.f);
-        s_e2[rhs] = (double)eo * (double)eo;
-    }
     if (tid < 32) {
         float v = (float)a.op.kappa;
         for (int i = 0; i < tid; ++i) v *= (float)a.op.kappa;
-        s_kp[tid] = v;                                  // kappa^{k+1}
-    }
-    for (int i = tid; i < 2 * ns * 8; i += blockDim.x) {
-        const int pat = i >= ns * 8 ? 1 : 0;
-        s_nbr[i] = (uint32_t)__ldg(tl.nbr[pat] + (i - pat * ns * 8)) * site_bytes;
-    }
-    for (int i = tid; i < 2 * ns; i += blockDim.x) {
-        const int pat = i >= ns ? 1 : 0;
-        s_outc[i] = __ldg(tl.outc[pat] + (i - pat * ns));
+        s_kp[tid] = v;
+        s_vc[tid] = tl.vcode[dag ? 1 : 0][tid];
     }
     for (int i = tid; i < nwc * spw * 8 * 12; i += blockDim.x) {      // the zero block of every link record
         const int rec = i / 12;
         reinterpret_cast<uint32_t*>(sm + tl.off_links + (rec >> 3) * MDWF_H16_SREC + (rec & 7) * MDWF_H16_LREC + 192)[i % 12] = 0u;
     }
-    for (int i = tid; i < 64 * nwc; i += blockDim.x) s_wpart[i] = 0.0;
+    if (a.partial != nullptr)
+        for (int i = tid; i < 64 * nwc; i += blockDim.x) s_wpart[i] = 0.0;
+    // the scale of the output: every block evaluates the rule (same inputs, same result); block 0 stores it
+    if (tid < a.nact) {
+        const int rhs = a.rhs_list[tid];
+        const float eo = eval_scale(a.sr, rhs, blockIdx.x == 0);
+        const float ei = a.in.m->e[rhs];
+        const float ex = a.xin.v != nullptr ? a.xin.m->e[rhs] : 0.f;
+        s_cf[rhs] = make_float2(ei / eo, ex / eo);
+        s_e2[rhs] = (double)eo * (double)eo;
+    }
     __syncthreads();
 
-    const int G = gridDim.x, ngrp = *s_ngrp;
-    const int nmy = (tl.ntiles - (int)blockIdx.x + G - 1) / G;
-    const int nitems = nmy * ngrp;
-    if (warp == 0)
-        for (int k = 0; k < nst && k < nitems; ++k)
-            hop16_issue(g, tl, a, blockIdx.x + (k / ngrp) * G, s_grp[k % ngrp], sbase + tl.off_stage + k * tl.stage_bytes, sbase + 8 * k, lane);
-
+    const int G = gridDim.x, ngrp = tl.ngrp;
+    const int nitems = tl.ntiles * ngrp;
     const int gq = lane >> 2, tq = lane & 3;
-    const uint32_t vc = tl.vcode[dag ? 1 : 0][lane];
+    const uint32_t vc = s_vc[lane];
     uint32_t cl[8];                       // offset of the lane's variant block (or the zero block) inside a site record
 #pragma unroll
     for (int l = 0; l < 8; ++l) cl[l] = (uint32_t)l * MDWF_H16_LREC + ((vc >> (4 * l)) & 7u) * 48u;
-    uint32_t rowoff4[MT], rowoff2[MT];
+    // A-fragment addressing inside a site: row block rb at rb*384, chunk c at + c*128, this lane at + gq*16 + tq*4.
+    // Row blocks 2*mt and 2*mt + 1 are read at compile-time offsets; when the site has an odd number of row blocks the
+    // last read runs into the next site (fields carry that much slack at their end) and feeds rows that are discarded.
+    const uint32_t lane_off = (uint32_t)gq * 16u + (uint32_t)tq * 4u;
+    constexpr int NQ = (MT * 48 + 31) / 32;
+    // epilogue work items of this lane: 16-byte piece q = lane + 32 qi of the site in memory order (row block q / 24,
+    // colour chunk (q % 24) / 8, row q % 8), packed as  E offset of (rhs, chunk) | s << 16 | rhs-in-group << 24, or -1
+    int qd[NQ];
 #pragma unroll
-    for (int mt = 0; mt < MT; ++mt) {
-        int r4 = mt * 16 + (lane & 7) + 8 * ((lane >> 3) & 1), r2 = mt * 16 + (lane & 15);
-        r4 = r4 < rows ? r4 : rows - 1;
-        r2 = r2 < rows ? r2 : rows - 1;
-        rowoff4[mt] = (uint32_t)r4 * 48u + (uint32_t)(lane >> 4) * 16u;
-        rowoff2[mt] = (uint32_t)r2 * 48u + 32u;
+    for (int qi = 0; qi < NQ; ++qi) {
+        const int q = lane + 32 * qi;
+        const int rb = (q * 171) >> 12, rem = q - rb * 24, c = rem >> 3, row = rb * 8 + (rem & 7);
+        const int ri = (row >= Ls) + (row >= 2 * Ls) + (row >= 3 * Ls), s = row - ri * Ls;
+        qd[qi] = (row < rows && q < nrb * 24) ? ((ri * Ls * 24 + c * 8) | (s << 16) | (ri << 24)) : -1;
     }
-    constexpr int NQ = (MT * 16 * 3 + 31) / 32;
     unsigned char* wl = sm + tl.off_links + warp * spw * MDWF_H16_SREC;      // this warp's site records
     const uint32_t wl_addr = smem_u32(wl);
     float* E = reinterpret_cast<float*>(sm + tl.off_epi) + warp * (MT * 16 * 24);
@@ -262,28 +154,33 @@ __global__ void __launch_bounds__(32 * MDWF_H16_MAXW, 1) hop16_kernel(const Geom
     const uint32_t* plt = a.g.pl[a.par];
 
     uint32_t raw[9];
-    int rxh = 0, rpat = 0;
-    // prepared links (and output site index) of this lane's (site, leg) in tile `tile`
+    int rxh = 0, rnb = 0, rtile = -1;
+    // stencil-ready links, neighbour index and output site index of this lane's (site, leg) in tile `tile`
     auto fetch_links = [&](int tile) {
-        int o[4];
-        tile16_origin(tl, tile, o);
-        rpat = (a.par + o[1] + o[2] + o[3]) & 1;
+        rtile = tile;
         if (has_link) {
-            const int pc = s_outc[rpat * ns + warp * spw + il_me];
+            int o[4];
+            tile16_origin(tl, tile, o);
+            const int pat = (a.par + o[1] + o[2] + o[3]) & 1;
+            const int pc = __ldg(tl.outc[pat] + warp * spw + il_me);
             const int gx = o[0] + (pc & 255);
             rxh = (gx >> 1) + g.XH * (o[1] + ((pc >> 8) & 255) + g.Y * (o[2] + ((pc >> 16) & 255) + g.Z * (o[3] + ((pc >> 24) & 255))));
-            const uint32_t* p = plt + (long long)rxh * 72 + l_me;
+            const uint32_t* p = plt + (long long)rxh * MDWF_H16_PLW + l_me;
 #pragma unroll
             for (int e = 0; e < 9; ++e) raw[e] = __ldg(p + e * 8);
+            rnb = (int)__ldg(p + 72);
         }
     };
-    if (nitems > 0) fetch_links(blockIdx.x);
+    int cur_tile = -1;
+    if ((int)blockIdx.x < nitems) fetch_links((int)tl.dng.div(blockIdx.x));
 
-    int st = 0, use = 0, tix = 0, gi = 0, pat = 0;
-    for (int k = 0; k < nitems; ++k) {
-        if (gi == 0) {
-            // ---- new tile: this warp's link records from the fetched words, then fetch the next tile's ------------
-            pat = rpat;
+    for (int k = blockIdx.x; k < nitems; k += G) {
+        uint32_t tile_u, gi_u;
+        tl.dng.divmod((uint32_t)k, tile_u, gi_u);
+        const int tile = (int)tile_u, grp = tl.grp[gi_u], gmask = tl.gmask[gi_u];
+        if (tile != cur_tile) {
+            // ---- new tile: this warp's link records from the fetched words, then fetch the next item's ------------
+            if (rtile != tile) fetch_links(tile);
             if (has_link) {
                 uint32_t w[4][12];
 #pragma unroll
@@ -303,14 +200,19 @@ __global__ void __launch_bounds__(32 * MDWF_H16_MAXW, 1) hop16_kernel(const Geom
                 for (int v = 0; v < 4; ++v)
 #pragma unroll
                     for (int q = 0; q < 3; ++q) dst[v * 3 + q] = make_uint4(w[v][4 * q], w[v][4 * q + 1], w[v][4 * q + 2], w[v][4 * q + 3]);
-                if (l_me == 0) *reinterpret_cast<int*>(wl + il_me * MDWF_H16_SREC + 8 * MDWF_H16_LREC) = rxh;
+                int* meta = reinterpret_cast<int*>(wl + il_me * MDWF_H16_SREC + 8 * MDWF_H16_LREC);
+                meta[4 + l_me] = rnb;
+                if (l_me == 0) meta[0] = rxh;
             }
             __syncwarp();
-            if (tix + 1 < nmy) fetch_links(blockIdx.x + (tix + 1) * G);
+            cur_tile = tile;
+            const int k2 = k + G;
+            if (k2 < nitems) {
+                const int t2 = (int)tl.dng.div((uint32_t)k2);
+                if (t2 != tile) fetch_links(t2);
+            }
         }
-        const int grp = s_grp[gi], gmask = s_gmask[gi];
-        mbar_wait(sbase + 8 * st, (uint32_t)(use & 1));
-        const uint32_t stg = sbase + tl.off_stage + st * tl.stage_bytes;
+        const char* ibase = reinterpret_cast<const char*>(a.in.v) + (long long)grp * a.in.rs;
         const char* xbase = a.xin.v != nullptr ? reinterpret_cast<const char*>(a.xin.v) + (long long)grp * a.xin.rs : nullptr;
         char* obase = reinterpret_cast<char*>(a.out.v) + (long long)grp * a.out.rs;
         float s2r[4] = {0.f, 0.f, 0.f, 0.f};
@@ -318,9 +220,9 @@ __global__ void __launch_bounds__(32 * MDWF_H16_MAXW, 1) hop16_kernel(const Geom
             const int i = warp * spw + il;
             if (i >= ns) break;
             const uint32_t srec = wl_addr + il * MDWF_H16_SREC;
-            const uint4 n0 = lds128(sbase + tl.off_nbr + (uint32_t)(pat * ns + i) * 32u);
-            const uint4 n1 = lds128(sbase + tl.off_nbr + (uint32_t)(pat * ns + i) * 32u + 16u);
-            const uint32_t noff[8] = {n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, n1.z, n1.w};
+            const int* smeta = reinterpret_cast<const int*>(wl + il * MDWF_H16_SREC + 8 * MDWF_H16_LREC);
+            const int4 nb0 = *reinterpret_cast<const int4*>(smeta + 4), nb1 = *reinterpret_cast<const int4*>(smeta + 8);
+            const int nxh[8] = {nb0.x, nb0.y, nb0.z, nb0.w, nb1.x, nb1.y, nb1.z, nb1.w};
             float acc[MT][3][4];
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt)
@@ -328,25 +230,37 @@ __global__ void __launch_bounds__(32 * MDWF_H16_MAXW, 1) hop16_kernel(const Geom
                 for (int n = 0; n < 3; ++n)
 #pragma unroll
                     for (int e = 0; e < 4; ++e) acc[mt][n][e] = 0.f;
-#pragma unroll
-            for (int l = 0; l < 8; ++l) {
-                const uint32_t in_addr = stg + noff[l];
-                const uint32_t baddr = srec + cl[l];
-                const uint4 b0 = lds128(baddr), b1 = lds128(baddr + 16u);
-                const uint32_t b2 = lds32(baddr + 32u);
+            uint32_t A[2][MT][6];
+            // A fragments of one leg: per m16 tile six 128-byte lines (rows 0-7 / 8-15 x colour chunk 0, 1, 2)
+            auto load_A = [&](int l, uint32_t (&dst)[MT][6]) {
+                const uint32_t* np = reinterpret_cast<const uint32_t*>(ibase + ((long long)nxh[l] * sb + lane_off));
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) {
-                    uint32_t A[4], A2[2];
-                    ldsm_x4(A, in_addr + rowoff4[mt]);
-                    ldsm_x2(A2, in_addr + rowoff2[mt]);
-                    mma_16816(acc[mt][0], A, b0.x, b0.y);
-                    mma_16816(acc[mt][1], A, b0.z, b0.w);
-                    mma_16816(acc[mt][2], A, b1.x, b1.y);
-                    mma_1688(acc[mt][0], A2, b1.z);
-                    mma_1688(acc[mt][1], A2, b1.w);
-                    mma_1688(acc[mt][2], A2, b2);
+                    dst[mt][0] = __ldg(np + mt * 192); dst[mt][1] = __ldg(np + mt * 192 + 96);
+                    dst[mt][2] = __ldg(np + mt * 192 + 32); dst[mt][3] = __ldg(np + mt * 192 + 128);
+                    dst[mt][4] = __ldg(np + mt * 192 + 64); dst[mt][5] = __ldg(np + mt * 192 + 160);
+                }
+            };
+            if (PF) load_A(0, A[0]);
+#pragma unroll
+            for (int l = 0; l < 8; ++l) {
+                if (PF) { if (l < 7) load_A(l + 1, A[(l + 1) & 1]); }
+                else load_A(l, A[l & 1]);
+                const uint4 b0 = *reinterpret_cast<const uint4*>(wl + il * MDWF_H16_SREC + cl[l]);
+                const uint4 b1 = *reinterpret_cast<const uint4*>(wl + il * MDWF_H16_SREC + cl[l] + 16);
+                const uint32_t b2 = *reinterpret_cast<const uint32_t*>(wl + il * MDWF_H16_SREC + cl[l] + 32);
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    const uint32_t* Ac = A[l & 1][mt];
+                    mma_16816(acc[mt][0], Ac, b0.x, b0.y);
+                    mma_16816(acc[mt][1], Ac, b0.z, b0.w);
+                    mma_16816(acc[mt][2], Ac, b1.x, b1.y);
+                    mma_1688(acc[mt][0], Ac + 4, b1.z);
+                    mma_1688(acc[mt][1], Ac + 4, b1.w);
+                    mma_1688(acc[mt][2], Ac + 4, b2);
                 }
             }
+            (void)srec;
             // ---- epilogue of site i: accumulators -> E[row][colour*8 + spin*2 + reim], row = rhs-in-group * Ls + s -----
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt)
@@ -373,17 +287,16 @@ __global__ void __launch_bounds__(32 * MDWF_H16_MAXW, 1) hop16_kernel(const Geom
                 }
                 __syncwarp();
             }
-            const long long idx0 = (long long)*reinterpret_cast<const int*>(wl + il * MDWF_H16_SREC + 8 * MDWF_H16_LREC) * site_bytes;
+            const long long idx0 = (long long)smeta[0] * sb;
 #pragma unroll
             for (int qi = 0; qi < NQ; ++qi) {
                 const int q = lane + 32 * qi;
-                if (q < rows * 3) {
-                    const int row = (q * 171) >> 9, c = q - 3 * row;
-                    const int ri = (row >= Ls) + (row >= 2 * Ls) + (row >= 3 * Ls), s = row - ri * Ls;
+                if (qd[qi] >= 0) {
+                    const int ri = qd[qi] >> 24, s = (qd[qi] >> 16) & 255;
                     if ((gmask >> ri) & 1) {
-                        const float4 cf = s_cf[(grp << ril) + ri];
+                        const float2 cf = s_cf[(grp << ril) + ri];
                         const float chc = (float)a.ch * cf.x;                       // ch * e_in / e_out
-                        const float* Er = E + ri * Ls * 24 + c * 8;                 // this rhs, this colour chunk, row s at + s*24
+                        const float* Er = E + (qd[qi] & 0xffff);                    // this rhs, this colour chunk, row s at + s*24
                         float o8[8];
                         if (op.kind == 0) {
                             const float4 lo = *reinterpret_cast<const float4*>(Er + s * 24);
@@ -423,10 +336,10 @@ __global__ void __launch_bounds__(32 * MDWF_H16_MAXW, 1) hop16_kernel(const Geom
                             o8[4] = ia * pm.x + ck * qm.x + gm * tm.x; o8[5] = ia * pm.y + ck * qm.y + gm * tm.y;
                             o8[6] = ia * pm.z + ck * qm.z + gm * tm.z; o8[7] = ia * pm.w + ck * qm.w + gm * tm.w;
                         }
-                        const long long off = idx0 + row * 48 + c * 16;
+                        const long long off = idx0 + q * 16;
                         if (xbase != nullptr) {
                             const float cxs = (float)a.cx * cf.y;                   // cx * e_x / e_out
-                            const uint4 xv = ldg(reinterpret_cast<const uint4*>(xbase + off));
+                            const uint4 xv = __ldcs(reinterpret_cast<const uint4*>(xbase + off));
                             const float2 x0 = h2f(xv.x), x1 = h2f(xv.y), x2 = h2f(xv.z), x3 = h2f(xv.w);
                             o8[0] = fmaf(cxs, x0.x, o8[0]); o8[1] = fmaf(cxs, x0.y, o8[1]);
                             o8[2] = fmaf(cxs, x1.x, o8[2]); o8[3] = fmaf(cxs, x1.y, o8[3]);
@@ -448,19 +361,6 @@ __global__ void __launch_bounds__(32 * MDWF_H16_MAXW, 1) hop16_kernel(const Geom
             }
             __syncwarp();
         }
-        // this warp is done with the staging buffer; the last warp to get here refills it with item k + nst
-        int last = 0;
-        if (lane == 0) {
-            __threadfence_block();
-            last = atomicAdd(&s_done[st], 1) == nwc - 1;
-            if (last) s_done[st] = 0;
-        }
-        last = __shfl_sync(0xffffffffu, last, 0);
-        if (last && k + nst < nitems) {
-            const int k2 = k + nst;
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            hop16_issue(g, tl, a, blockIdx.x + (k2 / ngrp) * G, s_grp[k2 % ngrp], stg, sbase + 8 * st, lane);
-        }
         if (a.partial != nullptr) {
             // fixed-order sums: lanes (shuffle tree) -> this warp's running sum per rhs -> warps (serial, at the end)
 #pragma unroll
@@ -473,8 +373,6 @@ __global__ void __launch_bounds__(32 * MDWF_H16_MAXW, 1) hop16_kernel(const Geom
                 }
             }
         }
-        if (++st == nst) { st = 0; ++use; }
-        if (++gi == ngrp) { gi = 0; ++tix; }
     }
     if (a.partial != nullptr) {
         __syncthreads();

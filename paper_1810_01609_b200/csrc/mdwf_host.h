@@ -110,6 +110,7 @@ inline RhsList all_rhs(int n) {
 
 size_t field_bytes(const Geom& g, int prec, int nrhs);
 int half_ril(int nrhs, int Ls);
+int half_site_bytes(int nrhs, int Ls);
 int alloc_field(mdwf_ctx* c, int prec, int nrhs, mdwf_field** out);
 // a field whose vectors live at `mem` (field_bytes() bytes, 256-byte aligned) instead of their own allocation
 int wrap_field(mdwf_ctx* c, int prec, int nrhs, void* mem, void* meta_mem, mdwf_field** out);

@@ -116,8 +116,9 @@ int make_work(Solver& S, Work& W, mdwf_field* ext_rhs, mdwf_field* ext_opar) {
         if (r2 == MDWF_OK) {
             W.all.push_back(*f);
             if (meta) MDWF_CUDA(c, cudaMemsetAsync(meta, 0, 2 * sizeof(FieldMeta), S.st));
-            // padding rhs of the last interleave group must hold finite numbers
-            if (prec == 16 && (n & ((1 << half_ril(n, g.Ls)) - 1))) MDWF_CUDA(c, cudaMemsetAsync(mem, 0, field_bytes(g, prec, n), S.st));
+            // padding rhs of the last interleave group and padding rows of a site must hold finite numbers
+            if (prec == 16 && ((n & ((1 << half_ril(n, g.Ls)) - 1)) || ((g.Ls << half_ril(n, g.Ls)) & 7)))
+                MDWF_CUDA(c, cudaMemsetAsync(mem, 0, field_bytes(g, prec, n), S.st));
         }
         return r2;
     };
