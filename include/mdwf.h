@@ -93,6 +93,9 @@ int mdwf_field_destroy(mdwf_field* f);
 /* canonical half-lattice fp64 [rhs][s][xh][4][3][2] (device) <-> packed */
 int mdwf_field_pack(mdwf_field* f, const void* canonical, void* stream);
 int mdwf_field_unpack(const mdwf_field* f, void* canonical, void* stream);
+/* the same for column `rhs` alone (canonical [s][xh][4][3][2] of one rhs); fp64 / fp32 fields only */
+int mdwf_field_pack_rhs(mdwf_field* f, int rhs, const void* canonical, void* stream);
+int mdwf_field_unpack_rhs(const mdwf_field* f, int rhs, void* canonical, void* stream);
 /* out = op(in) on packed half-lattice fields of equal prec/nrhs (op != FULL); out must not alias in. */
 int mdwf_dslash_packed(mdwf_ctx* ctx, int op, int parity, int dagger, int recon, mdwf_field* out,
                        const mdwf_field* in, void* stream);

@@ -25,7 +25,7 @@ EXPORTS = [
     "mdwf_field_destroy", "mdwf_field_pack", "mdwf_field_unpack", "mdwf_dslash_packed", "mdwf_dslash_cost",
     "mdwf_solve", "mdwf_solve_host", "mdwf_seq_source", "mdwf_nucleon_2pt", "mdwf_wall_inject",
     "mdwf_wall_project", "mdwf_launch_count", "mdwf_set_tiling", "mdwf_profile", "mdwf_profile_read", "mdwf_selftest_host", "mdwf_solve_packed",
-    "mdwf_workspace_bytes", "mdwf_set_workspace", "mdwf_set_hop16_tile",
+    "mdwf_workspace_bytes", "mdwf_set_workspace", "mdwf_set_hop16_tile", "mdwf_field_pack_rhs", "mdwf_field_unpack_rhs",
 ]
 
 
@@ -95,6 +95,8 @@ def lib():
         L.mdwf_workspace_bytes.argtypes = [vp, ci, ci, ci, ctypes.POINTER(ctypes.c_int64)]
         L.mdwf_set_workspace.argtypes = [vp, vp, ctypes.c_int64]
         L.mdwf_set_hop16_tile.argtypes = [vp, ci, ci, ci, ci, ci]
+        L.mdwf_field_pack_rhs.argtypes = [vp, ci, vp, vp]
+        L.mdwf_field_unpack_rhs.argtypes = [vp, ci, vp, vp]
         _lib = L
     return _lib
 
@@ -151,6 +153,12 @@ class Field:
 
     def mdwf_field_unpack(self, canonical: torch.Tensor):
         self.ctx._chk(lib().mdwf_field_unpack(self._h, _dev(canonical), _stream()))
+
+    def mdwf_field_pack_rhs(self, rhs: int, canonical: torch.Tensor):
+        self.ctx._chk(lib().mdwf_field_pack_rhs(self._h, rhs, _dev(canonical), _stream()))
+
+    def mdwf_field_unpack_rhs(self, rhs: int, canonical: torch.Tensor):
+        self.ctx._chk(lib().mdwf_field_unpack_rhs(self._h, rhs, _dev(canonical), _stream()))
 
     def mdwf_field_destroy(self):
         if self._h:

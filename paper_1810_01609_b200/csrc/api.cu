@@ -205,6 +205,7 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     c->partial = nullptr; c->dscal = nullptr; c->hscal = nullptr; c->launches = 0; c->prof_on = 0; c->zc_forced = 0;
     c->tile16[0] = c->tile16[1] = c->tile16[2] = nullptr; c->tile16_nw = 0; c->partial_nblk = 0; c->partial_cap = 0;
     c->ws = nullptr; c->ws_bytes = 0; c->ws_external = false;
+    c->dctl = nullptr; c->hctl_stage = nullptr; c->hctl = nullptr;
     for (int i = 0; i < 4; ++i) c->tile16_forced[i] = 0;
     for (int i = 0; i < 3; ++i) { c->prof_ms[i] = c->prof_bytes[i] = c->prof_flops[i] = 0.0; c->prof_n[i] = 0; }
     *out = c;   // returned even on failure so that mdwf_last_error can be read; caller destroys it
@@ -253,6 +254,11 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     MDWF_CUDA(c, cudaMalloc(&c->dscal, sizeof(double) * 16 * 64));
     MDWF_CUDA(c, cudaMemset(c->dscal, 0, sizeof(double) * 16 * 64));
     MDWF_CUDA(c, cudaHostAlloc(&c->hscal, sizeof(double) * 16 * 64, cudaHostAllocDefault));
+    MDWF_CUDA(c, cudaMalloc(&c->dctl, sizeof(CgCtl)));
+    MDWF_CUDA(c, cudaMemset(c->dctl, 0, sizeof(CgCtl)));
+    MDWF_CUDA(c, cudaHostAlloc(&c->hctl_stage, sizeof(CgCtl), cudaHostAllocDefault));
+    MDWF_CUDA(c, cudaHostAlloc(&c->hctl, sizeof(CgCtlHost), cudaHostAllocDefault));
+    memset((void*)c->hctl, 0, sizeof(CgCtlHost));
     build_lsops(g.Ls, M5, b5, c5, mf, c->lsop);
     build_lsop_norms(g.Ls, M5, b5, c5, mf, c->lsop, c->lsop_norm);
     return MDWF_OK;
@@ -264,6 +270,9 @@ int mdwf_destroy(mdwf_ctx* c) {
     for (auto& kv : c->temps) for (mdwf_field* f : kv.second) free_field(f);
     for (int i = 0; i < 3; ++i) if (c->tile16[i]) { free_tile16(c->tile16[i]); delete c->tile16[i]; c->tile16[i] = nullptr; }
     if (c->ws && !c->ws_external) cudaFree(c->ws);
+    if (c->dctl) cudaFree(c->dctl);
+    if (c->hctl_stage) cudaFreeHost(c->hctl_stage);
+    if (c->hctl) cudaFreeHost((void*)c->hctl);
     prof_drain(c);
     for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
     if (c->partial) cudaFree(c->partial);
@@ -376,7 +385,7 @@ int op_ls(const OpCtx& o, mdwf_field* out, const mdwf_field* in, int mat, const 
     a.out = out->view(); a.in = in->view();
     a.xin = xin ? xin->view() : no_view();
     if (mat >= 0) a.op = o.c->lsop[mat]; else a.op.kind = 0;
-    a.cx = cx; a.ch = ch; a.partial = partial; a.write = write; a.rl = rl;
+    a.cx = cx; a.ch = ch; a.partial = partial; a.write = write; a.rl = rl; a.stop = o.stop;
     a.sr = write ? rule_lin(out, in, std::fabs(ch) * (mat >= 0 ? o.c->lsop_norm[mat] : 1.0), xin, std::fabs(cx)) : rule_lin(nullptr, nullptr, 0.0);
     const int rc = launch_ls(o.c, o.prec, a, o.st);
     if (write) out->flip();
@@ -391,7 +400,7 @@ int op_hop(const OpCtx& o, mdwf_field* out, const mdwf_field* in, int out_par, i
     a.g.v[0] = o.gs->v[0]; a.g.v[1] = o.gs->v[1];
     a.g.pl[0] = o.gs->pl[0]; a.g.pl[1] = o.gs->pl[1];
     if (mat >= 0) a.op = o.c->lsop[mat]; else { a.op = o.c->lsop[0]; a.op.kind = 0; }
-    a.cx = cx; a.ch = ch; a.partial = partial; a.par = out_par; a.nact = rl.nact;
+    a.cx = cx; a.ch = ch; a.partial = partial; a.par = out_par; a.nact = rl.nact; a.stop = o.stop;
     for (int i = 0; i < 64; ++i) a.rhs_list[i] = rl.rhs[i];
     // |H_{p<-pbar}| <= 8: each of the 8 legs is (1 -+ gamma_mu) x unitary = 2 x (projector x unitary)
     a.sr = rule_lin(out, in, 8.0 * std::fabs(ch) * (mat >= 0 ? o.c->lsop_norm[mat] : 1.0), xin, std::fabs(cx));
@@ -519,6 +528,24 @@ int mdwf_field_pack(mdwf_field* f, const void* canonical, void* stream) {
 int mdwf_field_unpack(const mdwf_field* f, void* canonical, void* stream) {
     if (!f || !canonical) return MDWF_EINVAL;
     return unpack_field(f, (double*)canonical, 0, 0, (cudaStream_t)stream);
+}
+// one column at a time (so that a large multi-rhs field can be filled from a single-rhs canonical buffer)
+static int pack_one(mdwf_field* f, int rhs, double* canonical, bool unpack, cudaStream_t st) {
+    mdwf_ctx* c = f->ctx;
+    if (rhs < 0 || rhs >= f->nrhs) MDWF_FAIL(c, MDWF_EINVAL, "rhs %d out of range", rhs);
+    if (f->prec == 16) MDWF_FAIL(c, MDWF_EINVAL, "column-wise packing is for fp64/fp32 fields (an fp16 field is scaled as a whole)");
+    PackArgs a;
+    memset(&a, 0, sizeof(a));
+    a.f = f->view(); a.canon = canonical; a.Vc = c->g.Vh; a.full = 0; a.par = 0; a.nrhs = 1; a.rhs0 = rhs;
+    return launch_pack(c, f->prec, unpack, a, st);
+}
+int mdwf_field_pack_rhs(mdwf_field* f, int rhs, const void* canonical, void* stream) {
+    if (!f || !canonical) return MDWF_EINVAL;
+    return pack_one(f, rhs, (double*)canonical, false, (cudaStream_t)stream);
+}
+int mdwf_field_unpack_rhs(const mdwf_field* f, int rhs, void* canonical, void* stream) {
+    if (!f || !canonical) return MDWF_EINVAL;
+    return pack_one(const_cast<mdwf_field*>(f), rhs, (double*)canonical, true, (cudaStream_t)stream);
 }
 
 int mdwf_dslash_packed(mdwf_ctx* c, int op, int parity, int dagger, int recon, mdwf_field* out,

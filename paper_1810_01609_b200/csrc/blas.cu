@@ -213,8 +213,10 @@ int launch_cg_p(mdwf_ctx* c, int prec, CgPArgs& a, cudaStream_t st) {
     MDWF_FAIL(c, MDWF_EINVAL, "bad precision %d", prec);
 }
 
-int launch_finish(mdwf_ctx* c, const RhsList& rl, double* out, double* out2, cudaStream_t st, double* nb) {
+int launch_finish(mdwf_ctx* c, const RhsList& rl, double* out, double* out2, cudaStream_t st, double* nb, const FinishCtl* fc) {
     FinishArgs f;
+    memset(&f, 0, sizeof(f));
+    if (fc) { f.stop = fc->stop; f.ctl = fc->ctl; f.hctl = fc->hctl; f.pap = fc->pap; f.seq = fc->seq; }
     f.partial = c->partial;
     f.nblk = c->partial_nblk;
     f.out = out;

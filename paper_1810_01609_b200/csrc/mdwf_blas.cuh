@@ -22,11 +22,13 @@ struct LsArgs {
     int write;
     RhsList rl;
     ScaleRule sr;       // fp16 output only
+    const int* stop;    // optional: non-zero -> no-op (see HopArgs)
 };
 template <typename S>
 __global__ void __launch_bounds__(256) ls_kernel(const Geom g, const LsArgs a) {
     typedef typename Store<S>::real T;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (a.stop != nullptr && *a.stop != 0) return;
     const int slot = blockIdx.x % a.rl.nact, tile = blockIdx.x / a.rl.nact, rhs = a.rl.rhs[slot];
     const int idx = tile * blockDim.x + threadIdx.x;
     const bool live = idx < g.N5h;
@@ -115,12 +117,14 @@ struct CgXrArgs {
     double* partial;
     RhsList rl;
     ScaleRule sr;         // fp16 r only: scale of the updated r
+    const int* stop;      // optional: non-zero -> no-op
 };
 template <typename SX, typename S>
 __global__ void __launch_bounds__(256) cg_update_xr_kernel(const Geom g, const CgXrArgs a) {
     typedef typename Store<S>::real T;
     typedef typename Store<SX>::real TX;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (a.stop != nullptr && *a.stop != 0) return;
     const int slot = blockIdx.x % a.rl.nact, tile = blockIdx.x / a.rl.nact, rhs = a.rl.rhs[slot];
     const int idx = tile * blockDim.x + threadIdx.x;
     const bool live = idx < g.N5h;
@@ -158,11 +162,13 @@ struct CgPArgs {
     double* partial;      // optional |p_new|^2 partials (fp16: refreshes p's norm bound)
     RhsList rl;
     ScaleRule sr_p, sr_q; // fp16 only: scales of the updated p and of q
+    const int* stop;      // optional: non-zero -> no-op
 };
 template <typename S>
 __global__ void __launch_bounds__(256) cg_update_p_kernel(const Geom g, const CgPArgs a) {
     typedef typename Store<S>::real T;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (a.stop != nullptr && *a.stop != 0) return;
     const int slot = blockIdx.x % a.rl.nact, tile = blockIdx.x / a.rl.nact, rhs = a.rl.rhs[slot];
     const int idx = tile * blockDim.x + threadIdx.x;
     const bool live = idx < g.N5h;
@@ -193,7 +199,25 @@ __global__ void __launch_bounds__(256) cg_update_p_kernel(const Geom g, const Cg
     }
 }
 
-// out[rhs] = sum_b partial[slot][b] in a fixed order; optionally mirrored to (mapped) host memory
+// out[rhs] = sum_b partial[slot][b] in a fixed order; optionally mirrored to (mapped) host memory.
+// With `ctl` the kernel is the loop control of the inner CG (solver.cu): after |r|^2 of every active rhs is known it
+// decides ON THE DEVICE whether the inner loop must be left (reliable update due, target reached, breakdown, iteration
+// cap) and raises ctl->stop, which turns every kernel queued behind it into a no-op; the host, which runs a few
+// iterations ahead, only polls the pinned mirror.  Iteration counts are therefore exactly those of a loop that
+// synchronises after every iteration.
+struct CgCtl {
+    int stop;            // device flag read by the gated kernels
+    int done_blocks;     // blocks of the current finish launch that are through
+    int iters;           // iterations completed since the flag was cleared
+    int iter_cap;        // leave the loop when iters reaches this
+    double delta;
+    double stop_nr[64], maxr[64];
+};
+struct CgCtlHost {       // pinned mirror, written by the last block of every loop-control launch
+    volatile int seq;    // sequence number of the last loop-control launch that ran (also when it was a no-op)
+    volatile int stop;
+    volatile int iters;
+};
 struct FinishArgs {
     const double* partial;
     int nblk;
@@ -201,23 +225,51 @@ struct FinishArgs {
     double* out2;       // optional second destination (e.g. host-mapped), may be nullptr
     double* nb;         // optional: norm bound of the fp16 field that was just measured, nb[rhs] = sqrt(sum) (1 + 2^-9)
     RhsList rl;
+    const int* stop;    // optional: non-zero -> no-op
+    CgCtl* ctl;         // optional: loop control (this launch finishes |r|^2)
+    CgCtlHost* hctl;
+    const double* pap;  // loop control: <p, A p> of the iteration (breakdown check)
+    int seq;
 };
 static __global__ void __launch_bounds__(256) finish_sum_kernel(const FinishArgs a) {
     __shared__ double red[256];
     const int slot = blockIdx.x, rhs = a.rl.rhs[slot];
-    const double* p = a.partial + (long long)slot * a.nblk;
-    double s = 0.0;
-    for (int i = threadIdx.x; i < a.nblk; i += 256) s += p[i];
-    red[threadIdx.x] = s;
-    __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
-        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+    const bool skip = a.stop != nullptr && *a.stop != 0;
+    bool want_stop = false;
+    if (!skip) {
+        const double* p = a.partial + (long long)slot * a.nblk;
+        double s = 0.0;
+        for (int i = threadIdx.x; i < a.nblk; i += 256) s += p[i];
+        red[threadIdx.x] = s;
         __syncthreads();
+        for (int o = 128; o > 0; o >>= 1) {
+            if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) {
+            a.out[rhs] = red[0];
+            if (a.out2) a.out2[rhs] = red[0];
+            if (a.nb) a.nb[rhs] = sqrt(red[0]) * 1.001953125;
+            if (a.ctl) {
+                const double rn = sqrt(red[0]), pap = a.pap[rhs];
+                want_stop = !(rn == rn) || !(pap > 0.0) || rn <= a.ctl->stop_nr[rhs] || rn < a.ctl->delta * a.ctl->maxr[rhs] ||
+                            a.ctl->iters + 1 >= a.ctl->iter_cap;
+                if (rn > a.ctl->maxr[rhs]) a.ctl->maxr[rhs] = rn;
+            }
+        }
     }
-    if (threadIdx.x == 0) {
-        a.out[rhs] = red[0];
-        if (a.out2) a.out2[rhs] = red[0];
-        if (a.nb) a.nb[rhs] = sqrt(red[0]) * 1.001953125;
+    if (a.ctl && threadIdx.x == 0) {
+        if (want_stop) atomicExch(&a.ctl->stop, 1);
+        __threadfence();
+        if (atomicAdd(&a.ctl->done_blocks, 1) == (int)gridDim.x - 1) {      // last block of this launch
+            a.ctl->done_blocks = 0;
+            if (!skip) a.ctl->iters += 1;
+            __threadfence();
+            a.hctl->iters = a.ctl->iters;
+            a.hctl->stop = *(volatile int*)&a.ctl->stop;
+            __threadfence_system();
+            a.hctl->seq = a.seq;
+        }
     }
 }
 

@@ -292,6 +292,8 @@ struct HopArgs {
     int nact;                  // active rhs count; blockIdx.x = tile*nact + slot
     int rhs_list[64];
     ScaleRule sr;              // fp16 output only (mdwf_hop16.cuh)
+    const int* stop;           // optional device flag: non-zero -> the launch is a no-op (CG iterations queued behind the
+                               // point where the device decided to leave the inner loop, solver.cu)
 };
 
 // (tile, site-in-tile) -> coordinates; see Geom for the traversal order
@@ -387,6 +389,7 @@ __global__ void __launch_bounds__(256, (sizeof(S) == 8 ? MDWF_HOP_MINB64 : sizeo
     typedef typename Store<S>::real T;
     typedef Pack16<T> P;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (a.stop != nullptr && *a.stop != 0) return;
     const int Ls = g.Ls;
     const int nsite = g.nsite;
     T* links = reinterpret_cast<T*>(smem_raw);

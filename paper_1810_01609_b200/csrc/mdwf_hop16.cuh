@@ -89,6 +89,7 @@ __device__ __forceinline__ void tile16_origin(const Tile16& tl, int tile, int o[
 template <int MT, int PF, int MINB>
 __global__ void __launch_bounds__(PF ? 32 * MDWF_H16_MAXW : 256, MINB) hop16_kernel(const Geom g, const Tile16 tl, const HopArgs a, const int dag) {
     extern __shared__ __align__(128) unsigned char sm[];
+    if (a.stop != nullptr && *a.stop != 0) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nwc = (int)(blockDim.x >> 5);
     const int Ls = g.Ls, ns = tl.ns, spw = tl.spw;

@@ -75,6 +75,9 @@ struct mdwf_ctx {
     std::set<const void*> attr_raised;   // kernels whose dynamic shared-memory limit was raised on THIS device
     int partial_nblk;              // partial sums per rhs written by the last kernel that filled `partial`
     size_t partial_cap;            // doubles per rhs in `partial`
+    mdwf::CgCtl* dctl;             // device-side loop control of the inner CG (mdwf_blas.cuh) and its pinned staging copy / mirror
+    mdwf::CgCtl* hctl_stage;
+    mdwf::CgCtlHost* hctl;
     void* ws;                      // solver workspace: library-owned (kept between calls) or caller-supplied
     size_t ws_bytes;
     bool ws_external;
@@ -127,7 +130,9 @@ int launch_cg_xr(mdwf_ctx* c, int prec_x, int prec, CgXrArgs& a, cudaStream_t st
 int launch_cg_p(mdwf_ctx* c, int prec, CgPArgs& a, cudaStream_t st);
 // sums the partials of the LAST kernel that wrote them (c->partial_nblk per rhs); nb: optional norm-bound slot of the
 // fp16 field that was just measured
-int launch_finish(mdwf_ctx* c, const RhsList& rl, double* out, double* out2, cudaStream_t st, double* nb = nullptr);
+struct FinishCtl { const int* stop; CgCtl* ctl; CgCtlHost* hctl; const double* pap; int seq; };
+int launch_finish(mdwf_ctx* c, const RhsList& rl, double* out, double* out2, cudaStream_t st, double* nb = nullptr,
+                  const FinishCtl* fc = nullptr);
 inline int cls_of(int prec) { return prec == 16 ? 0 : prec == 32 ? 1 : 2; }
 int launch_pack(mdwf_ctx* c, int prec, bool unpack, PackArgs& a, cudaStream_t st);
 int pack_field(mdwf_field* f, const double* canon, int full, int par, cudaStream_t st);
@@ -142,6 +147,7 @@ struct OpCtx {
     int prec, recon;
     const GaugeSet* gs;
     cudaStream_t st;
+    const int* stop = nullptr;   // gate of the launches (HopArgs::stop)
 };
 // simple helpers: out = cx*xin + ch*G*in ; out = cx*xin + ch*G*H(in).  All fields of one call have precision o.prec;
 // for fp16 the scale rule of the output is built here (operator-norm bounds x the inputs' norm bounds) and the

@@ -17,7 +17,8 @@
 // x_lo (fp32 for 16-bit inner vectors); the three fp64 temporaries of the reliable updates are shared by `nhi` <= batch
 // rhs at a time.  Everything lives in one workspace (library-owned and kept between calls, or supplied by the caller
 // through mdwf_set_workspace).  The inner loop never waits for the host: the decision to leave it is taken on the
-// device (finish_rr_kernel) and the kernels of iterations already queued behind that point turn into no-ops.
+// device (finish_sum_kernel with loop control) and the kernels of iterations already queued behind that point turn
+// into no-ops, so iteration counts equal those of a loop that synchronises after every iteration.
 #include "mdwf_host.h"
 #include <cmath>
 #include <algorithm>
@@ -58,6 +59,7 @@ struct Solver {
     int nb, nhi, par, sym, prec, px;
     double tol, delta;
     int max_iter, check_every;
+    int seq = 0;        // sequence number of the loop-control launches (CgCtlHost::seq)
 
     double* dsc(int k) { return c->dscal + 64 * k; }
     double* hsc(int k) { return c->hscal + 64 * k; }
@@ -284,53 +286,20 @@ static int solve_core(Solver& S, Work& W, mdwf_solve_info* info, int r0, double*
     cudaEvent_t e0, e1;
     MDWF_CUDA(c, cudaEventCreate(&e0));
     MDWF_CUDA(c, cudaEventCreate(&e1));
-    int since_check = 0;
-    bool open = false;
     rc = MDWF_OK;
-    while (act.nact > 0 && rc == MDWF_OK) {
-        if (!open) { cudaEventRecord(e0, st); open = true; }
-        // t = S p, pAp = |t|^2 ; Ap = S^dag t   (out may alias the first work field, see op_schur)
-        if ((rc = op_schur(S.lo, t, p, par, 0, sym, t, wb, act, c->partial, 1))) break;   // t holds A p on entry
-        if ((rc = launch_finish(c, act, S.dsc(SC_PAP), S.hsc(SC_PAP), st, t->nb_w()))) break;
-        if ((rc = op_schur(S.lo, wa, t, par, 1, sym, wa, wb, act))) break;
-        CgXrArgs u;
-        memset(&u, 0, sizeof(u));
-        u.x = xl->view(); u.r = r->view(); u.p = p->view(); u.Ap = wa->view(); u.rr = S.dsc(rrOld); u.pAp = S.dsc(SC_PAP);
-        u.partial = c->partial; u.rl = act;
-        if (r->meta) {      // |r - alpha Ap| <= |r| + |alpha| |Ap|
-            u.sr.n = 2; u.sr.out = r->wmeta();
-            u.sr.t[0].nb = r->nb(); u.sr.t[0].coef = 1.0;
-            u.sr.t[1].nb = wa->nb(); u.sr.t[1].coef = 1.0; u.sr.t[1].num = S.dsc(rrOld); u.sr.t[1].den = S.dsc(SC_PAP);
-        }
-        if ((rc = launch_cg_xr(c, S.px, S.prec, u, st))) break;
-        r->flip();
-        if ((rc = launch_finish(c, act, S.dsc(rrNew), S.hsc(rrNew), st, r->nb_w()))) break;
-        for (int k = 0; k < act.nact; ++k) iters[act.rhs[k]]++;
-        bool need_update = false;
-        if (++since_check >= S.check_every) {
-            since_check = 0;
-            if ((rc = S.sync())) break;
-            for (int k = 0; k < act.nact; ++k) {
-                const int i = act.rhs[k];
-                const double rn = std::sqrt(S.hsc(rrNew)[i]), pap = S.hsc(SC_PAP)[i];
-                if (!(rn == rn) || !(pap > 0.0)) need_update = true;          // breakdown: let the fp64 update decide
-                if (rn <= stop_nr[i] || rn < S.delta * maxr[i] || iters[i] >= S.max_iter) need_update = true;
-                if (rn > maxr[i]) maxr[i] = rn;
-            }
-        }
-        if (need_update) {
-            cudaEventRecord(e1, st);
-            cudaEventSynchronize(e1);
-            float ms = 0.f;
-            cudaEventElapsedTime(&ms, e0, e1);
-            *t_inner_ms += ms;
-            open = false;
-            if ((rc = reliable(false))) break;
-            if (act.nact == 0) break;
-        }
+    // Inner loop.  The host queues iterations a few ahead of the device and never waits for a result: the last kernel
+    // of an iteration (finish_sum_kernel with loop control) decides on the device whether the loop must be left and
+    // turns everything queued behind it into no-ops (gate `ctl->stop`).  One cycle = arm the control block, (pending
+    // p-update), iterations until the gate closes, drain, fp64 reliable update.
+    const int* gate = &c->dctl->stop;
+    const int kRunAhead = 6;
+    bool pending_p = false;
+    auto p_update = [&](const int* stop) -> int {
+        int rc2;
         CgPArgs q;
         memset(&q, 0, sizeof(q));
         q.p = p->view(); q.r = r->view(); q.q = t->view(); q.op = c->lsop[MAT_A]; q.rr_new = S.dsc(rrNew); q.rr_old = S.dsc(rrOld); q.rl = act;
+        q.stop = stop;
         if (p->meta) {      // |r + beta p| <= |r| + beta |p| ; |A p| <= |A| |p| ; p's bound is then refreshed by its measured norm
             for (int w = 0; w < 2; ++w) {
                 ScaleRule& sr = w ? q.sr_q : q.sr_p;
@@ -341,18 +310,89 @@ static int solve_core(Solver& S, Work& W, mdwf_solve_info* info, int r0, double*
             }
             q.partial = c->partial;
         }
-        if ((rc = launch_cg_p(c, S.prec, q, st))) break;
+        if ((rc2 = launch_cg_p(c, S.prec, q, st))) return rc2;
         p->flip();
         t->flip();
-        if (p->meta && (rc = launch_finish(c, act, S.dsc(SC_PP), nullptr, st, p->nb_w()))) break;
+        if (p->meta) {
+            FinishCtl fc;
+            memset(&fc, 0, sizeof(fc));
+            fc.stop = stop;
+            if ((rc2 = launch_finish(c, act, S.dsc(SC_PP), nullptr, st, p->nb_w(), &fc))) return rc2;
+        }
         std::swap(rrOld, rrNew);
-    }
-    if (open) {
+        return MDWF_OK;
+    };
+    while (act.nact > 0 && rc == MDWF_OK) {
+        // ---- arm the loop control ------------------------------------------------------------------------------
+        CgCtl* hs = c->hctl_stage;
+        memset(hs, 0, sizeof(*hs));
+        hs->delta = S.delta;
+        int cap = 1 << 30;
+        for (int k = 0; k < act.nact; ++k) {
+            const int i = act.rhs[k];
+            hs->stop_nr[i] = stop_nr[i];
+            hs->maxr[i] = maxr[i];
+            cap = std::min(cap, std::max(1, S.max_iter - iters[i]));
+        }
+        hs->iter_cap = cap;
+        MDWF_CUDA(c, cudaMemcpyAsync(c->dctl, hs, sizeof(CgCtl), cudaMemcpyHostToDevice, st));
+        c->hctl->stop = 0;
+        c->hctl->iters = 0;
+        cudaEventRecord(e0, st);
+        if (pending_p && (rc = p_update(nullptr))) break;
+        pending_p = false;
+        S.lo.stop = gate;
+        // meta slots / rr slots as they are before the first iteration of this cycle (flips of no-op launches are undone below)
+        const int cur0[5] = {r->cur, p->cur, t->cur, wa->cur, wb->cur};
+        const int rrOld0 = rrOld, rrNew0 = rrNew;
+        int queued = 0;
+        while (rc == MDWF_OK) {
+            // t = S p, pAp = |t|^2 ; Ap = S^dag t   (out may alias the first work field, see op_schur)
+            FinishCtl fg;
+            memset(&fg, 0, sizeof(fg));
+            fg.stop = gate;
+            if ((rc = op_schur(S.lo, t, p, par, 0, sym, t, wb, act, c->partial, 1))) break;   // t holds A p on entry
+            if ((rc = launch_finish(c, act, S.dsc(SC_PAP), S.hsc(SC_PAP), st, t->nb_w(), &fg))) break;
+            if ((rc = op_schur(S.lo, wa, t, par, 1, sym, wa, wb, act))) break;
+            CgXrArgs u;
+            memset(&u, 0, sizeof(u));
+            u.x = xl->view(); u.r = r->view(); u.p = p->view(); u.Ap = wa->view(); u.rr = S.dsc(rrOld); u.pAp = S.dsc(SC_PAP);
+            u.partial = c->partial; u.rl = act; u.stop = gate;
+            if (r->meta) {      // |r - alpha Ap| <= |r| + |alpha| |Ap|
+                u.sr.n = 2; u.sr.out = r->wmeta();
+                u.sr.t[0].nb = r->nb(); u.sr.t[0].coef = 1.0;
+                u.sr.t[1].nb = wa->nb(); u.sr.t[1].coef = 1.0; u.sr.t[1].num = S.dsc(rrOld); u.sr.t[1].den = S.dsc(SC_PAP);
+            }
+            if ((rc = launch_cg_xr(c, S.px, S.prec, u, st))) break;
+            r->flip();
+            FinishCtl fc;
+            memset(&fc, 0, sizeof(fc));
+            fc.stop = gate; fc.ctl = c->dctl; fc.hctl = c->hctl; fc.pap = S.dsc(SC_PAP); fc.seq = ++S.seq;
+            if ((rc = launch_finish(c, act, S.dsc(rrNew), S.hsc(rrNew), st, r->nb_w(), &fc))) break;
+            ++queued;
+            if ((rc = p_update(gate))) break;           // a no-op if this iteration closed the gate: redone after the update
+            while (S.seq - c->hctl->seq > kRunAhead && cudaStreamQuery(st) == cudaErrorNotReady) {}
+            if (c->hctl->stop) break;
+        }
+        S.lo.stop = nullptr;
+        if (rc) break;
         cudaEventRecord(e1, st);
         cudaEventSynchronize(e1);
         float ms = 0.f;
         cudaEventElapsedTime(&ms, e0, e1);
         *t_inner_ms += ms;
+        const int done = c->hctl->iters;          // iterations that really ran; the last one is complete up to its |r|^2
+        if (done < 1 || done > queued) { c->err = "internal: inner-loop control out of step"; rc = MDWF_ECUDA; break; }
+        // host-side bookkeeping as if only `done` iterations had been queued: `done` x-r updates, done - 1 p-updates
+        r->cur = cur0[0] ^ (done & 1);
+        p->cur = cur0[1] ^ ((done - 1) & 1);
+        // t: written once (Mhat) or twice (Dhat: M5 p, then the hop) per operator application and once per p-update (q = A p)
+        t->cur = cur0[2] ^ ((done * (sym ? 1 : 2) + done - 1) & 1);
+        wa->cur = cur0[3]; wb->cur = cur0[4];      // an even number of flips per iteration
+        if ((done - 1) & 1) { rrOld = rrNew0; rrNew = rrOld0; } else { rrOld = rrOld0; rrNew = rrNew0; }
+        for (int k = 0; k < act.nact; ++k) iters[act.rhs[k]] += done;
+        if ((rc = reliable(false))) break;
+        pending_p = true;
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
