@@ -83,18 +83,43 @@ def aggregate(sec_per_rhs_per_replica, world):
     return sec_per_rhs_per_replica / world
 
 
-def oracle_baseline(cfg, budget_s=20.0):
-    """The CPU oracle as it stands (oracle.solve_eo: its own even-odd CG, fp64, OpenMP over the host cores),
-    timed on a bounded sample of the workload: the same operator parameters and link recipe on a small
-    sub-lattice, one Gaussian rhs, same tolerance.  Returns (dict, seconds per (5D site x CG iteration))."""
+def sample_dims(cfg):
+    """the bounded sub-lattice of the workload that the CPU oracle is timed on"""
+    return tuple(min(d, s) for d, s in zip(cfg.dims, (8, 8, 8, 16)))
+
+
+def oracle_baseline(cfg, workload_iters=None):
+    """The CPU oracle as it stands (fp64, OpenMP over the host cores), timed on a bounded sample of the workload: the
+    same operator parameters and link recipe on a small sub-lattice.  (i) hop and Mhat applications (median of 3;
+    sites/s, GB/s and GFLOP/s under the same byte / flop convention as the GPU lines); (ii) its own
+    even-odd CG (oracle.solve_eo) on one Gaussian rhs at the workload's tolerance.
+    Returns (dict, seconds per (5D site x CG iteration))."""
     import numpy as np
     import oracle
     import synth
-    dims = tuple(min(d, s) for d, s in zip(cfg.dims, (8, 8, 8, 16)))
+    dims = sample_dims(cfg)
     p = oracle.Params(dims=dims, Ls=cfg.Ls, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=cfg.mf, bc=cfg.bc)
     U = synth.gauge_field(dims, cfg.eps, synth.seed_for(cfg.index, 1)).numpy()
     b = synth.gaussian_spinor(dims, cfg.Ls, 1, synth.seed_for(cfg.index, 2)).numpy()
     oracle.schur(p, U, b, 0, False, True)          # warm-up (page in, OpenMP team)
+    n5h = int(np.prod(dims)) // 2 * cfg.Ls         # 5D sites of one parity
+    other = oracle.mask(p, b, 1)
+    same = oracle.mask(p, b, 0)
+
+    def med3(fn):
+        ts = []
+        for _ in range(3):
+            t0 = time.time()
+            fn()
+            ts.append(time.time() - t0)
+        return sorted(ts)[1]
+
+    t_hop = med3(lambda: oracle.hop(p, U, other, dagger=False, out_parity=0))
+    t_mhat = med3(lambda: oracle.schur(p, U, same, 0, False, True))
+    # same convention as mdwf_dslash_cost for fp64 / 18 reals: hop 2*192 B + links, 1320 flop; Mhat 5 passes + 2 link passes
+    links = 8 * 18 * 8 * (int(np.prod(dims)) // 2)
+    hop_bytes, hop_flops = 2 * 192.0 * n5h + links, 1320.0 * n5h
+    mh_bytes, mh_flops = 5 * 192.0 * n5h + 2 * links, (2832.0 + 96.0 * cfg.Ls) * n5h
     t0 = time.time()
     x, its, _ = oracle.solve_eo(p, U, b, parity=0, symmetric=True, tol=cfg.tol, max_iter=100000)
     dt = time.time() - t0
@@ -105,12 +130,21 @@ def oracle_baseline(cfg, budget_s=20.0):
          "sample": "oracle.solve_eo (fp64 even-odd CG, symmetric) on a %s x Ls=%d sub-lattice of the workload "
                    "(same M5,b5,c5,mf, link recipe and tol %.0e), 1 Gaussian rhs: %d iterations in %.2f s, "
                    "true residual %.2e" % ("x".join(map(str, dims)), cfg.Ls, cfg.tol, its[0], dt, tr),
-         "s_per_5Dsite_iteration": per_site_iter, "iterations": its[0]}
+         "s_per_5Dsite_iteration": per_site_iter, "iterations": its[0],
+         "dslash": {"sample_lattice": list(dims), "hop_ms": t_hop * 1e3, "hop_sites_per_s": n5h / t_hop,
+                    "hop_GBps": hop_bytes / t_hop / 1e9, "hop_GFLOPs": hop_flops / t_hop / 1e9,
+                    "mhat_ms": t_mhat * 1e3, "mhat_sites_per_s": n5h / t_mhat, "mhat_GBps": mh_bytes / t_mhat / 1e9,
+                    "mhat_GFLOPs": mh_flops / t_mhat / 1e9, "convention": "fp64, 18-real links; median of 3"}}
+    if workload_iters:
+        d["extrapolated_s_per_rhs_on_workload"] = per_site_iter * cfg.V4 * cfg.Ls * workload_iters
+        d["note"] = ("value is the measured sample; the extrapolation multiplies the measured s/(5D site x iteration) by the "
+                     "workload's 5D volume and the workload's own iteration count (%d)" % workload_iters)
     return d, per_site_iter
 
 
 def run_reference(args):
-    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only).  Each step is the bounded sample
+    described in cpu_baseline.sample; config.workload names that sub-lattice (it is NOT the GPU arm's workload)."""
     import synth
     if int(os.environ.get("RANK", "0")) != 0:
         return
@@ -123,13 +157,104 @@ def run_reference(args):
             vals.append(base["value"])
     v = sum(vals) / len(vals)
     base["value"] = v
+    sd = sample_dims(cfg)
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "s/RHS", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": v * 1e3, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfg.name, "note": "each step is the bounded sample described in cpu_baseline.sample"},
+            "config": {"workload": "oracle sample %s_Ls%d of %s" % ("x".join(map(str, sd)), cfg.Ls, cfg.name),
+                       "of_workload": cfg.name, "sites_ratio_workload_to_sample": cfg.V4 / float(sd[0] * sd[1] * sd[2] * sd[3]),
+                       "note": "each step is the bounded sample described in cpu_baseline.sample, not the GPU arm's workload"},
             "cpu_baseline": base,
             "e2e": {"value": v, "unit": "s/RHS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
+
+
+def fill_packed_rhs(fields, cfg, nrhs, seed, dev, scratch):
+    """Gaussian complex 5D right-hand sides, drawn by the seeded device generator one (rhs, parity) half-lattice
+    column at a time and packed straight into the fp64 half-lattice fields (no canonical full-lattice copy exists)."""
+    import torch
+    g = torch.Generator(device=dev)
+    for par in (0, 1):
+        for r in range(nrhs):
+            g.manual_seed(int(seed) * 1000 + 2 * r + par)
+            torch.view_as_real(scratch).normal_(0.0, 1.0, generator=g)
+            fields[par].mdwf_field_pack_rhs(r, scratch)
+
+
+def dslash_legs(ctx, cfg, nrhs, formats, dev, hbm_peak, iters=10):
+    """Dslash-only leg through mdwf_dslash_packed on the bench lattice: plain hop and Mhat per (prec, recon), CUDA events
+    around `iters` back-to-back calls; algorithmic bytes / flops from mdwf_dslash_cost."""
+    import torch
+    import synth
+    import paper_1810_01609_b200 as mdwf
+    out = []
+    Vh = cfg.V4 // 2
+    g = torch.Generator(device=dev).manual_seed(synth.seed_for(cfg.index, 3))
+    for prec, recon in formats:
+        fin, fout = ctx.mdwf_field_create(prec, nrhs), ctx.mdwf_field_create(prec, nrhs)
+        src = torch.empty((nrhs, cfg.Ls, Vh, 4, 3), dtype=torch.complex128, device=dev)
+        torch.view_as_real(src).normal_(0.0, 1.0, generator=g)
+        fin.mdwf_field_pack(src)
+        del src
+        for name, op in (("hop", mdwf.OP_HOP), ("mhat", mdwf.OP_DHAT_SYM)):
+            for _ in range(3):
+                ctx.mdwf_dslash_packed(op, fout, fin, 0, False, recon)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(iters):
+                ctx.mdwf_dslash_packed(op, fout, fin, 0, False, recon)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / iters
+            by, fl = ctx.mdwf_dslash_cost(op, prec, recon, nrhs)
+            out.append({"lattice": cfg.name, "nrhs": nrhs, "prec": prec, "recon": recon, "op": name, "ms": ms,
+                        "GBps": by / ms / 1e6, "GFLOPs": fl / ms / 1e6, "frac_of_measured_hbm": by / ms / 1e6 / hbm_peak})
+        fin.mdwf_field_destroy()
+        fout.mdwf_field_destroy()
+        torch.cuda.empty_cache()
+    return out
+
+
+def config2_sweep(dev, hbm_peak, rotate=4, iters=20):
+    """BASELINE.json configs[1]: 16^3x32, Ls=8 Dslash-only sweep over {fp64, fp32, fp16} x {18, 12, 8 reals}; the lattice
+    fits in L2, so `rotate` independent in/out buffer sets are cycled (SURVEY 8(d) config-2 caveat)."""
+    import torch
+    import synth
+    import paper_1810_01609_b200 as mdwf
+    cfg = synth.CONFIGS[2]
+    ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc, device=dev.index or 0)
+    U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(2, 1), device=dev)
+    Vh = cfg.V4 // 2
+    g = torch.Generator(device=dev).manual_seed(synth.seed_for(2, 2))
+    rows = []
+    for prec in (64, 32, 16):
+        for recon in (18, 12, 8):
+            ctx.mdwf_load_gauge(U, prec, recon)
+            fin = [ctx.mdwf_field_create(prec, 1) for _ in range(rotate)]
+            fout = [ctx.mdwf_field_create(prec, 1) for _ in range(rotate)]
+            for f in fin:
+                src = torch.empty((1, cfg.Ls, Vh, 4, 3), dtype=torch.complex128, device=dev)
+                torch.view_as_real(src).normal_(0.0, 1.0, generator=g)
+                f.mdwf_field_pack(src)
+            for name, op in (("hop", mdwf.OP_HOP), ("mhat", mdwf.OP_DHAT_SYM)):
+                for k in range(3):
+                    ctx.mdwf_dslash_packed(op, fout[k % rotate], fin[k % rotate], 0, False, recon)
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for k in range(iters):
+                    ctx.mdwf_dslash_packed(op, fout[k % rotate], fin[k % rotate], 0, False, recon)
+                e1.record()
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1) / iters
+                by, fl = ctx.mdwf_dslash_cost(op, prec, recon, 1)
+                rows.append({"prec": prec, "recon": recon, "op": name, "ms": ms, "GBps": by / ms / 1e6,
+                             "GFLOPs": fl / ms / 1e6, "frac_of_measured_hbm": by / ms / 1e6 / hbm_peak})
+            for f in fin + fout:
+                f.mdwf_field_destroy()
+    ctx.mdwf_destroy()
+    return {"lattice": cfg.name, "rotate": rotate, "rows": rows}
 
 
 def run_ours(args):
@@ -141,6 +266,9 @@ def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != max(1, args.gpus):
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d (launch with torchrun --nproc-per-node %d, or let bench.py "
+                         "spawn the ranks by not setting WORLD_SIZE)" % (args.gpus, world, args.gpus))
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
@@ -149,20 +277,28 @@ def run_ours(args):
     nrhs = args.nrhs or cfg.nrhs
     inner, recon = args.inner, args.recon
     hbm_peak, peak_src = peaks()
+    Vh = cfg.V4 // 2
 
-    # ---- inputs (untimed): links of the config's recipe, Gaussian 5D right-hand sides --------------------
+    # ---- inputs (untimed): links of the config's recipe, Gaussian 5D right-hand sides as packed fp64 halves ----
     ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc, device=local)
     U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(cfg.index, 1), device=dev)
     ctx.mdwf_load_gauge(U, 64, 18)
     ctx.mdwf_load_gauge(U, inner, recon)
     del U
     torch.cuda.empty_cache()
-    b = synth.gaussian_spinor_device(cfg.dims, cfg.Ls, nrhs, synth.seed_for(cfg.index, 2) + 7 * rank, device=dev)
-    x = torch.empty_like(b)
-    kw = dict(tol=cfg.tol, inner_prec=inner, recon=recon, symmetric=not args.asym, batch=args.batch, check_every=args.check_every, delta=args.delta)
+    # the solver workspace comes from PyTorch's allocator (mdwf_set_workspace)
+    ws = torch.empty(ctx.mdwf_workspace_bytes(nrhs, inner, packed=True) + (1 << 20), dtype=torch.uint8, device=dev)
+    ctx.mdwf_set_workspace(ws)
+    psi = [ctx.mdwf_field_create(64, nrhs), ctx.mdwf_field_create(64, nrhs)]
+    scratch = torch.empty((1, cfg.Ls, Vh, 4, 3), dtype=torch.complex128, device=dev)
+    seed = synth.seed_for(cfg.index, 2) + 7 * rank
+    kw = dict(tol=cfg.tol, inner_prec=inner, recon=recon, symmetric=not args.asym, delta=args.delta)
 
     def step():
-        _, res = ctx.mdwf_solve(b, out=x, **kw)
+        # the solve is in place (b -> psi), so every step first restores the right-hand sides (inside the timed region:
+        # ~0.3 % of a config-5 step)
+        fill_packed_rhs(psi, cfg, nrhs, seed, dev, scratch)
+        res = ctx.mdwf_solve_packed(psi[0], psi[1], **kw)
         if res.status != 0:
             raise RuntimeError("solve did not converge: %r" % (res,))
         return res
@@ -178,7 +314,6 @@ def run_ours(args):
     sampler = ClockSampler(local)
     sampler.start()
     l0 = ctx.mdwf_launch_count()
-    ctx.mdwf_profile(True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record()
@@ -189,72 +324,77 @@ def run_ours(args):
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.finish()
     launches = ctx.mdwf_launch_count() - l0
-    prof = {c: ctx.mdwf_profile_read(c) for c in (0, 1, 2)}
-    ctx.mdwf_profile(False)
     ms_total = max_over_ranks(ms_total, world, dev)
     ms_step = ms_total / args.steps
     sec_per_rhs = ms_step * 1e-3 / nrhs          # per replica; N replicas solve N*nrhs in the same time
 
-    # ---- roofline of the dominant kernel: the hop (Dslash stencil) launches inside the timed solves ------
+    # ---- roofline of the dominant kernel: the inner-precision hop (Dslash stencil incl. fused epilogue) launches of one
+    # more, UNTIMED solve, each timed with CUDA events on the launching stream (the per-launch events would otherwise sit
+    # inside the timed region) ----------------------------------------------------------------------------------
+    ctx.mdwf_profile(True)
+    res_p = step()
+    torch.cuda.synchronize()
+    prof = {c: ctx.mdwf_profile_read(c) for c in range(8)}
+    ctx.mdwf_profile(False)
     cls = {16: 0, 32: 1, 64: 2}[inner]
     pms, pby, pfl, pn = prof[cls]
-    roof = {"bound": "hbm", "kernel": "hop_kernel<%s,%d> (inner-precision Dslash stencil incl. fused Ls epilogue)"
-            % ({16: "__half", 32: "float", 64: "double"}[inner], recon),
+    kname = ("hop16_kernel (tensor-core fp16 Dslash stencil incl. fused Ls epilogue, mma.sync f16->f32)" if inner == 16 else
+             "hop_kernel<%s,%d> (Dslash stencil incl. fused Ls epilogue)" % ("float" if inner == 32 else "double", recon))
+    roof = {"bound": "hbm", "kernel": kname,
             "achieved": pby / pms / 1e6 if pms > 0 else None, "peak": hbm_peak, "unit": "GB/s",
-            "frac": (pby / pms / 1e6) / hbm_peak if pms > 0 else None, "traffic": None, "peak_source": peak_src,
-            "launches": pn, "avg_launch_ms": pms / pn if pn else None, "gflops": pfl / pms / 1e6 if pms > 0 else None,
-            "share_of_step": pms / (ms_total if world == 1 else ms_step * args.steps)}
-    # the 16-bit kernel is co-bound by FP32 issue: report it against the plain-FP32 FMA peak
-    # 148 SMs x 128 lanes x 2 flop x max SM clock, with the 1320 flop/site convention
-    fp32_peak = 148 * 128 * 2 * (clocks.get("sm_max_mhz") or 1965) * 1e-6
-    if roof["gflops"]:
-        roof["co_bound"] = {"bound": "alu", "achieved": roof["gflops"] * 1e-3, "peak": fp32_peak, "unit": "TFLOP/s",
-                            "frac": roof["gflops"] * 1e-3 / fp32_peak,
-                            "note": "convention flops (1320 per 5D site) / FP32 FMA peak; ncu: issue slots 68-70 % busy"}
-    try:
-        import csv
-        with open(os.path.join(ROOT, "profiles", "traffic_r1.csv")) as f:
-            rows = {r["key"]: r for r in csv.DictReader(f)}
-        tr = rows.get("%s|inner%d|recon%d" % (cfg.name, inner, recon))
-        if tr:
-            roof["traffic"] = float(tr["dram_bytes_per_launch"])
-            roof["traffic_source"] = tr["source"]
-            roof["algorithmic_bytes_per_launch"] = pby / pn if pn else None
-    except Exception:
-        pass
+            "frac": (pby / pms / 1e6) / hbm_peak if pms > 0 else None, "traffic": None,
+            "traffic_note": "not measured in this run; ncu dram bytes per launch of the same kernel are in profiles/ (per capture, with its commit)",
+            "peak_source": peak_src, "launches": pn, "avg_launch_ms": pms / pn if pn else None,
+            "algorithmic_bytes_per_launch": pby / pn if pn else None, "rhs_in_flight": res.batch,
+            "gflops": pfl / pms / 1e6 if pms > 0 else None,
+            "share_of_step": pms / (res_p.seconds * 1e3) if res_p.seconds > 0 else None,
+            "timing": "per-launch CUDA events on the launching stream, over one extra solve after the timed region"}
+    names = {0: "hop fp16 (tensor cores)", 1: "hop fp32", 2: "hop fp64 (reliable updates)", 3: "s-direction kernel", 4: "cg x/r update",
+             5: "cg p update (+ A p)", 6: "reduction finish", 7: "axpby / convert"}
+    roof["step_breakdown_ms"] = {names[c]: {"ms": prof[c][0], "launches": prof[c][3]} for c in range(8) if prof[c][3]}
+    roof["step_breakdown_ms"]["whole solve (4 rhs)" if nrhs == 4 else "whole solve"] = res_p.seconds * 1e3
     h64 = prof[2]
     dsl = {"inner_hop_GBps": roof["achieved"], "inner_hop_GFLOPs": roof["gflops"],
            "fp64_hop_GBps": h64[1] / h64[0] / 1e6 if h64[0] > 0 else None,
            "fp64_hop_GFLOPs": h64[2] / h64[0] / 1e6 if h64[0] > 0 else None, "fp64_hop_launches": h64[3]}
-    return dict(ctx=ctx, cfg=cfg, nrhs=nrhs, b=b, x=x, kw=kw, res=res, ms_step=ms_step, sec_per_rhs=sec_per_rhs,
-                clocks=clocks, launches=launches, roof=roof, dsl=dsl, rank=rank, world=world, dev=dev)
+    return dict(ctx=ctx, cfg=cfg, nrhs=nrhs, psi=psi, scratch=scratch, ws=ws, kw=kw, res=res, ms_step=ms_step,
+                sec_per_rhs=sec_per_rhs, clocks=clocks, launches=launches, roof=roof, dsl=dsl, rank=rank, world=world, dev=dev,
+                hbm_peak=hbm_peak)
 
 
 def run_e2e(st, args):
     """Same metric through the C-ABI call with HOST buffers (mdwf_solve_host): every step copies the step's
-    right-hand sides host->device and the solutions device->host inside the timed region."""
+    right-hand sides host->device and the solutions device->host inside the timed region (canonical fp64 5D fields;
+    the library batches the rhs and overlaps the copies of neighbouring batches with the solves)."""
     import torch
     import torch.distributed as dist
-    ctx, b, x, nrhs = st["ctx"], st["b"], st["x"], st["nrhs"]
+    import synth
+    ctx, cfg, nrhs, dev = st["ctx"], st["cfg"], st["nrhs"], st["dev"]
+    # the packed fields and the torch-owned workspace of the device-resident leg are released first
+    for f in st["psi"]:
+        f.mdwf_field_destroy()
+    ctx.mdwf_set_workspace(None)
+    st["psi"] = st["ws"] = st["scratch"] = None
+    torch.cuda.empty_cache()
     if st["world"] > 1 and nrhs > 1:
-        # N ranks share one host: bound the pinned staging memory per rank (2 x 13.6 GB instead of 2 x 54 GB);
-        # seconds per rhs is the same metric, the solver handles one rhs at a time at this size anyway
-        nrhs = 1
-        b = b[:1].contiguous()
-    nbytes = b.numel() * b.element_size()
+        nrhs = 1          # N ranks share one host: bound the pinned staging memory per rank
+    shape = (nrhs, cfg.Ls, cfg.V4, 4, 3)
     try:
-        bh = torch.empty(b.shape, dtype=b.dtype, pin_memory=True)
-        xh = torch.empty(b.shape, dtype=b.dtype, pin_memory=True)
+        bh = torch.empty(shape, dtype=torch.complex128, pin_memory=True)
+        xh = torch.empty(shape, dtype=torch.complex128, pin_memory=True)
         pinned = True
     except Exception:
-        bh = torch.empty(b.shape, dtype=b.dtype)
-        xh = torch.empty(b.shape, dtype=b.dtype)
+        bh = torch.empty(shape, dtype=torch.complex128)
+        xh = torch.empty(shape, dtype=torch.complex128)
         pinned = False
-    bh.copy_(b)
+    one = torch.empty((1,) + shape[1:], dtype=torch.complex128, device=dev)
+    for r in range(nrhs):                       # device-drawn (seeded), copied to the host buffer column by column
+        synth.gaussian_spinor_device(cfg.dims, cfg.Ls, 1, synth.seed_for(cfg.index, 2) + 7 * st["rank"] + 100 * r, device=dev, out=one)
+        bh[r].copy_(one[0])
+    del one
     torch.cuda.synchronize()
-    st["b"] = st["x"] = None
-    del b, x
     torch.cuda.empty_cache()
+    nbytes = bh.numel() * bh.element_size()
     kw = dict(st["kw"])
 
     def step():
@@ -271,14 +411,21 @@ def run_e2e(st, args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(args.e2e_steps):
-        step()
+        res = step()
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1)
     ms = max_over_ranks(ms, st["world"], st["dev"])
     return {"value": ms * 1e-3 / args.e2e_steps / nrhs, "unit": "s/RHS", "h2d_bytes_per_step": nbytes,
             "d2h_bytes_per_step": nbytes, "steps": args.e2e_steps, "warmup": args.e2e_warmup, "pinned_host": pinned,
-            "api": "mdwf_solve_host", "nrhs": nrhs}
+            "api": "mdwf_solve_host", "nrhs": nrhs, "rhs_in_flight": res.batch}
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a launcher: start the N ranks ourselves (one process per GPU, torchrun)."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(29500 + os.getpid() % 2000), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
 
 
 def main():
@@ -291,45 +438,64 @@ def main():
     ap.add_argument("--nrhs", type=int, default=0)
     ap.add_argument("--inner", type=int, default=16)
     ap.add_argument("--recon", type=int, default=12)
-    ap.add_argument("--batch", type=int, default=0)
-    ap.add_argument("--check-every", type=int, default=1)
     ap.add_argument("--asym", action="store_true", help="solve with Dhat instead of Mhat = M5^-1 Dhat")
     ap.add_argument("--delta", type=float, default=0.0, help="reliable-update threshold (0 = library default)")
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--e2e-warmup", type=int, default=1)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-dslash", action="store_true", help="skip the Dslash-only legs (bench lattice and config-2 sweep)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
         return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args)
     st = run_ours(args)
     cfg, nrhs, res, world = st["cfg"], st["nrhs"], st["res"], st["world"]
     e2e = None if args.no_e2e else run_e2e(st, args)
     if st["rank"] != 0:
         return
+    import torch
+    if args.no_e2e:
+        for f in st["psi"]:
+            f.mdwf_field_destroy()
+        st["ctx"].mdwf_set_workspace(None)
+        st["psi"] = st["ws"] = st["scratch"] = None
+        torch.cuda.empty_cache()
+    dsl = st["dsl"]
+    if not args.no_dslash and world == 1:
+        import synth
+        U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(cfg.index, 1), device=st["dev"])
+        st["ctx"].mdwf_load_gauge(U, 32, 12)
+        del U
+        torch.cuda.empty_cache()
+        fmts = [(16, args.recon), (32, 12)] if args.inner == 16 else [(args.inner, args.recon)]
+        dsl["bench_lattice"] = dslash_legs(st["ctx"], cfg, nrhs, fmts, st["dev"], st["hbm_peak"])
+        if nrhs > 1:
+            dsl["bench_lattice"] += dslash_legs(st["ctx"], cfg, 1, fmts, st["dev"], st["hbm_peak"])
+        dsl["config2_sweep"] = config2_sweep(st["dev"], st["hbm_peak"])
     line = {"metric": METRIC, "value": aggregate(st["sec_per_rhs"], world), "unit": "s/RHS", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": st["ms_step"], "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": {16: "f32", 32: "f32", 64: "f64"}[args.inner],
             "data": "synthetic",
-            "config": {"workload": cfg.name, "lattice": list(cfg.dims), "Ls": cfg.Ls, "nrhs_per_gpu": nrhs, "tol": cfg.tol,
-                       "mf": cfg.mf, "inner_prec": args.inner, "recon": args.recon,
-                       "arithmetic": {16: "inner CG: fp16 storage (+fp32 scale per site), fp32 arithmetic, fp64 reductions; outer: fp64 reliable updates",
+            "config": {"workload": cfg.name, "lattice": list(cfg.dims), "Ls": cfg.Ls, "nrhs_per_gpu": nrhs,
+                       "rhs_in_flight": res.batch, "tol": cfg.tol, "mf": cfg.mf, "inner_prec": args.inner, "recon": args.recon,
+                       "arithmetic": {16: "inner CG: IEEE fp16 storage (one power-of-two scale per field and rhs), fp16 x fp16 products accumulated in fp32 on the tensor cores, fp32 epilogues, fp64 reductions; outer: fp64 reliable updates",
                                       32: "inner CG: fp32 storage and arithmetic, fp64 reductions; outer: fp64 reliable updates",
                                       64: "fp64 throughout"}[args.inner], "links": "reunit(exp(i*%.3f*H))" % cfg.eps,
-                       "rhs": "Gaussian complex 5D, device-drawn, seeded", "parallelism": "replicas only",
-                       "l2": "inputs larger than L2 (half-lattice 16-bit spinor %.0f MB per rhs)" % (cfg.V4 / 2 * cfg.Ls * 52 / 1e6)},
+                       "rhs": "Gaussian complex 5D, device-drawn, seeded, restored inside every step (in-place packed solve)",
+                       "api": "mdwf_solve_packed (device-resident); mdwf_solve_host (e2e)", "parallelism": "replicas only",
+                       "l2": "inputs larger than L2 (half-lattice 16-bit spinor %.0f MB per rhs)" % (cfg.V4 / 2 * cfg.Ls * 48 / 1e6)},
             "cg": {"seconds_per_rhs_per_replica": st["sec_per_rhs"], "iters": res.iters, "reliable_updates": res.reliable_updates,
-                   "true_resid": res.true_resid, "seconds_inner_last_step": res.seconds_inner, "seconds_last_step": res.seconds},
-            "dslash": st["dsl"], "roofline": st["roof"], "gpu_launches": st["launches"], "clocks": st["clocks"]}
+                   "true_resid": res.true_resid, "seconds_inner_last_step": res.seconds_inner, "seconds_last_step": res.seconds,
+                   "kernel_launches_last_step": res.kernel_launches},
+            "dslash": dsl, "roofline": st["roof"], "gpu_launches": st["launches"], "clocks": st["clocks"]}
     if e2e is not None:
         e2e["value"] = aggregate(e2e["value"], world)
         line["e2e"] = e2e
     if world == 1 and not args.no_cpu_baseline:
-        base, per = oracle_baseline(cfg)
-        it = max(res.iters) if res.iters else 0
-        base["extrapolated_s_per_rhs_on_workload"] = per * cfg.V4 * cfg.Ls * max(1, base["iterations"])
-        base["note"] = "value is the measured sample; the extrapolation multiplies the measured s/(5D site x iteration) by the workload's 5D volume and the sample's iteration count (GPU needed %d inner iterations)" % it
+        base, _ = oracle_baseline(cfg, workload_iters=max(res.iters) if res.iters else None)
         line["cpu_baseline"] = base
     print(json.dumps(line), flush=True)
 

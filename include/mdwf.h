@@ -179,8 +179,9 @@ int mdwf_wall_project(mdwf_ctx* ctx, void* q4, const void* psi5, int ncol, void*
 int64_t mdwf_launch_count(const mdwf_ctx* ctx);
 /* Per-launch timing of the hop (Dslash stencil) kernel with CUDA events on the launching stream.
  * mdwf_profile(ctx, 1) clears the counters and starts recording, mdwf_profile(ctx, 0) stops.
- * mdwf_profile_read synchronises the recorded events and returns, for class cls (0: fp16 storage, 1: fp32,
- * 2: fp64), the summed device time [ms], algorithmic bytes and flops (DESIGN.md cost convention: per 5D
+ * mdwf_profile_read synchronises the recorded events and returns, for class cls (hop kernel by storage class 0: fp16,
+ * 1: fp32, 2: fp64; time only for the site-local kernels 3: s-direction, 4: CG x/r update, 5: CG p update, 6: reduction
+ * finish, 7: axpby/convert), the summed device time [ms], algorithmic bytes and flops (DESIGN.md cost convention: per 5D
  * site 24*w bytes per spinor pass, 2 passes (+1 with an xpay input), links once per launch; 1320 flop)
  * and the launch count. */
 int mdwf_profile(mdwf_ctx* ctx, int enable);

@@ -207,7 +207,7 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     c->ws = nullptr; c->ws_bytes = 0; c->ws_external = false;
     c->dctl = nullptr; c->hctl_stage = nullptr; c->hctl = nullptr;
     for (int i = 0; i < 4; ++i) c->tile16_forced[i] = 0;
-    for (int i = 0; i < 3; ++i) { c->prof_ms[i] = c->prof_bytes[i] = c->prof_flops[i] = 0.0; c->prof_n[i] = 0; }
+    for (int i = 0; i < 8; ++i) { c->prof_ms[i] = c->prof_bytes[i] = c->prof_flops[i] = 0.0; c->prof_n[i] = 0; }
     *out = c;   // returned even on failure so that mdwf_last_error can be read; caller destroys it
     long long v4 = 1;
     for (int m = 0; m < 4; ++m) {
@@ -288,12 +288,12 @@ int64_t mdwf_launch_count(const mdwf_ctx* c) { return c ? c->launches : 0; }
 int mdwf_profile(mdwf_ctx* c, int enable) {
     if (!c) return MDWF_EINVAL;
     prof_drain(c);
-    if (enable) for (int i = 0; i < 3; ++i) { c->prof_ms[i] = c->prof_bytes[i] = c->prof_flops[i] = 0.0; c->prof_n[i] = 0; }
+    if (enable) for (int i = 0; i < 8; ++i) { c->prof_ms[i] = c->prof_bytes[i] = c->prof_flops[i] = 0.0; c->prof_n[i] = 0; }
     c->prof_on = enable ? 1 : 0;
     return MDWF_OK;
 }
 int mdwf_profile_read(mdwf_ctx* c, int cls, double* ms, double* bytes, double* flops, int64_t* launches) {
-    if (!c || cls < 0 || cls > 2 || !ms || !bytes || !flops || !launches) return MDWF_EINVAL;
+    if (!c || cls < 0 || cls > 7 || !ms || !bytes || !flops || !launches) return MDWF_EINVAL;
     prof_drain(c);
     *ms = c->prof_ms[cls]; *bytes = c->prof_bytes[cls]; *flops = c->prof_flops[cls]; *launches = c->prof_n[cls];
     return MDWF_OK;

@@ -94,6 +94,31 @@ ScaleRule rule_lin(const mdwf_field* out, const mdwf_field* a, double ca, const 
     return r;
 }
 
+// Grouped mode of a launch whose fields are fp16 with the rhs interleaved in groups of 1 << ril (mdwf_blas.cuh RhsList):
+// the groups that hold an active rhs, their masks, and the blocks per group.
+static int group_rhs(const Geom& g, RhsList& rl, int ril, int blk) {
+    rl.ril = ril;
+    rl.ng = 0;
+    if (ril == 0) return -1;
+    for (int k = 0; k < rl.nact; ++k) {
+        const int gr = rl.rhs[k] >> ril;
+        int j = 0;
+        while (j < rl.ng && rl.grp[j] != gr) ++j;
+        if (j == rl.ng) { rl.grp[j] = (unsigned char)gr; rl.gmask[j] = 0; ++rl.ng; }
+        rl.gmask[j] |= (unsigned char)(1 << (rl.rhs[k] & ((1 << ril) - 1)));
+        rl.slot_of[rl.rhs[k]] = (unsigned char)k;
+    }
+    const long long rows = (long long)g.Vh * (g.Ls << ril);
+    return (int)((rows + blk - 1) / blk);      // blocks per group
+}
+// grid / partials per rhs of a site-local launch at storage precision `prec` whose fp16 fields have interleave ril
+static void site_grid(mdwf_ctx* c, int prec, RhsList& rl, int ril, int* grid, int* blk, int* nblk) {
+    *blk = c->blk_cls[cls_of(prec)];
+    const int per_group = prec == 16 || ril > 0 ? group_rhs(c->g, rl, ril, *blk) : -1;
+    if (per_group > 0) { *grid = per_group * rl.ng; *nblk = per_group; }
+    else { rl.ril = 0; rl.ng = 0; *grid = c->nblk_cls[cls_of(prec)] * rl.nact; *nblk = c->nblk_cls[cls_of(prec)]; }
+}
+
 #define LAUNCH(kern, grid, blk, smem, ...)                              \
     do {                                                                \
         kern<<<(grid), (blk), (smem), st>>>(__VA_ARGS__);               \
@@ -122,8 +147,10 @@ template <typename S> static size_t g_smem(mdwf_ctx* c, bool useG) {
 }
 
 int launch_ls(mdwf_ctx* c, int prec, LsArgs& a, cudaStream_t st) {
-    const int grid = c->nblk_cls[cls_of(prec)] * a.rl.nact, blk = c->blk_cls[cls_of(prec)];
-    if (a.partial) c->partial_nblk = c->nblk_cls[cls_of(prec)];
+    ProfScope ps(c, 3, st);
+    int grid, blk, nblk;
+    site_grid(c, prec, a.rl, prec == 16 ? a.in.ril : 0, &grid, &blk, &nblk);
+    if (a.partial) c->partial_nblk = nblk;
     switch (prec) {
         case 64: return launch_big_smem(c, ls_kernel<double>, grid, blk, g_smem<double>(c, a.op.kind != 0), st, a);
         case 32: return launch_big_smem(c, ls_kernel<float>, grid, blk, g_smem<float>(c, a.op.kind != 0), st, a);
@@ -161,12 +188,31 @@ int launch_hop(mdwf_ctx* c, int prec, int recon, int dagger, int fused, HopArgs&
     return rc;
 }
 
+ProfScope::ProfScope(mdwf_ctx* c_, int cls, cudaStream_t st_) : c(c_), st(st_), on(c_->prof_on != 0) {
+    if (!on) return;
+    for (int k = 0; k < 2; ++k) {
+        cudaEvent_t e;
+        if (!c->prof_pool.empty()) { e = c->prof_pool.back(); c->prof_pool.pop_back(); }
+        else if (cudaEventCreate(&e) != cudaSuccess) { on = false; return; }
+        (k ? r.e1 : r.e0) = e;
+    }
+    r.cls = cls; r.bytes = 0.0; r.flops = 0.0;
+    cudaEventRecord(r.e0, st);
+}
+ProfScope::~ProfScope() {
+    if (!on) return;
+    cudaEventRecord(r.e1, st);
+    c->prof_pending.push_back(r);
+}
+
 template <typename SO, typename SA>
 static int axpby_b(mdwf_ctx* c, int pb, AxpbyArgs& a, cudaStream_t st) {
-    const int cls = sizeof(SO) == 2 ? 0 : sizeof(SO) == 4 ? 1 : 2;      // blocked like the output's storage class
-    const int grid = c->nblk_cls[cls] * a.rl.nact, blk = c->blk_cls[cls];
+    // blocked like the output's storage class; grouped when any field is fp16 (they share one interleave)
+    const int ril = sizeof(SO) == 2 ? a.out.ril : sizeof(SA) == 2 && a.a.v ? a.a.ril : pb == 16 && a.b.v ? a.b.ril : 0;
+    int grid, blk, nblk;
+    site_grid(c, sizeof(SO) == 2 ? 16 : sizeof(SO) == 4 ? 32 : 64, a.rl, ril, &grid, &blk, &nblk);
     const size_t smem = (size_t)blk * sizeof(double);
-    if (a.partial) c->partial_nblk = c->nblk_cls[cls];
+    if (a.partial) c->partial_nblk = nblk;
     switch (pb) {
         case 64: LAUNCH((axpby_kernel<SO, SA, double>), grid, blk, smem, c->g, a); return MDWF_OK;
         case 32: LAUNCH((axpby_kernel<SO, SA, float>), grid, blk, smem, c->g, a); return MDWF_OK;
@@ -184,6 +230,7 @@ static int axpby_a(mdwf_ctx* c, int pa, int pb, AxpbyArgs& a, cudaStream_t st) {
     MDWF_FAIL(c, MDWF_EINVAL, "bad precision %d", pa);
 }
 int launch_axpby(mdwf_ctx* c, int po, int pa, int pb, AxpbyArgs& a, cudaStream_t st) {
+    ProfScope ps(c, 7, st);
     switch (po) {
         case 64: return axpby_a<double>(c, pa, pb, a, st);
         case 32: return axpby_a<float>(c, pa, pb, a, st);
@@ -193,9 +240,11 @@ int launch_axpby(mdwf_ctx* c, int po, int pa, int pb, AxpbyArgs& a, cudaStream_t
 }
 
 int launch_cg_xr(mdwf_ctx* c, int prec_x, int prec, CgXrArgs& a, cudaStream_t st) {
-    const int grid = c->nblk_cls[cls_of(prec)] * a.rl.nact, blk = c->blk_cls[cls_of(prec)];
+    ProfScope ps(c, 4, st);
+    int grid, blk, nblk;
+    site_grid(c, prec, a.rl, prec == 16 ? a.r.ril : 0, &grid, &blk, &nblk);
     const size_t smem = (size_t)blk * sizeof(double);
-    c->partial_nblk = c->nblk_cls[cls_of(prec)];
+    c->partial_nblk = nblk;
     if (prec == 64 && prec_x == 64) { LAUNCH((cg_update_xr_kernel<double, double>), grid, blk, smem, c->g, a); return MDWF_OK; }
     if (prec == 32 && prec_x == 32) { LAUNCH((cg_update_xr_kernel<float, float>), grid, blk, smem, c->g, a); return MDWF_OK; }
     if (prec == 16 && prec_x == 32) { LAUNCH((cg_update_xr_kernel<float, __half>), grid, blk, smem, c->g, a); return MDWF_OK; }
@@ -203,8 +252,10 @@ int launch_cg_xr(mdwf_ctx* c, int prec_x, int prec, CgXrArgs& a, cudaStream_t st
 }
 
 int launch_cg_p(mdwf_ctx* c, int prec, CgPArgs& a, cudaStream_t st) {
-    const int grid = c->nblk_cls[cls_of(prec)] * a.rl.nact, blk = c->blk_cls[cls_of(prec)];
-    if (a.partial) c->partial_nblk = c->nblk_cls[cls_of(prec)];
+    ProfScope ps(c, 5, st);
+    int grid, blk, nblk;
+    site_grid(c, prec, a.rl, prec == 16 ? a.p.ril : 0, &grid, &blk, &nblk);
+    if (a.partial) c->partial_nblk = nblk;
     switch (prec) {
         case 64: return launch_big_smem(c, cg_update_p_kernel<double>, grid, blk, g_smem<double>(c, a.op.kind != 0), st, a);
         case 32: return launch_big_smem(c, cg_update_p_kernel<float>, grid, blk, g_smem<float>(c, a.op.kind != 0), st, a);
@@ -214,6 +265,7 @@ int launch_cg_p(mdwf_ctx* c, int prec, CgPArgs& a, cudaStream_t st) {
 }
 
 int launch_finish(mdwf_ctx* c, const RhsList& rl, double* out, double* out2, cudaStream_t st, double* nb, const FinishCtl* fc) {
+    ProfScope ps(c, 6, st);
     FinishArgs f;
     memset(&f, 0, sizeof(f));
     if (fc) { f.stop = fc->stop; f.ctl = fc->ctl; f.hctl = fc->hctl; f.pap = fc->pap; f.seq = fc->seq; }

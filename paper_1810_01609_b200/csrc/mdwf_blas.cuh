@@ -8,10 +8,69 @@
 
 namespace mdwf {
 
+// The rhs a launch works on.  Plain mode (ril == 0): one rhs per block, blockIdx.x = tile*nact + slot.  Grouped mode
+// (launches whose fields are fp16: the rhs are interleaved in groups of 1 << ril inside a 4D site, mdwf_device.cuh):
+// blockIdx.x = tile*ng + group, and consecutive threads walk the (rhs in group, s) rows of consecutive 4D sites, i.e.
+// consecutive 16-byte pieces of memory; the Ls threads of one (site, rhs) are still consecutive.
 struct RhsList {
     int nact;
     int rhs[64];
+    int ril, ng;
+    unsigned char grp[64], gmask[64], slot_of[64];
 };
+struct RowWork {
+    int rhs, idx, slot, tile, nblk, ri, grp;
+    bool live;
+};
+__device__ __forceinline__ RowWork map_work(const Geom& g, const RhsList& rl) {
+    RowWork w;
+    if (rl.ril == 0 && rl.ng == 0) {
+        w.slot = blockIdx.x % rl.nact; w.tile = blockIdx.x / rl.nact; w.rhs = rl.rhs[w.slot];
+        w.idx = w.tile * blockDim.x + threadIdx.x; w.live = w.idx < g.N5h; w.nblk = gridDim.x / rl.nact; w.ri = 0; w.grp = w.rhs;
+    } else {
+        const int gi = blockIdx.x % rl.ng;
+        w.tile = blockIdx.x / rl.ng; w.nblk = gridDim.x / rl.ng; w.grp = rl.grp[gi];
+        const uint32_t v = (uint32_t)w.tile * blockDim.x + threadIdx.x;
+        const uint32_t q = g.dLs.div(v);                 // = xh * RI + ri
+        const int xh = (int)(q >> rl.ril);
+        w.ri = (int)(q & ((1u << rl.ril) - 1u));
+        w.rhs = (w.grp << rl.ril) + w.ri;
+        w.idx = xh * g.Ls + (int)(v - q * g.Ls);
+        w.live = xh < g.Vh && ((rl.gmask[gi] >> w.ri) & 1);
+        w.slot = rl.slot_of[w.rhs & 63];
+    }
+    return w;
+}
+// fixed-order block sums per rhs of the block: plain mode one sum, grouped mode one per active rhs of the group
+__device__ __forceinline__ void block_sum_rhs(double v, const RowWork& w, const RhsList& rl, unsigned char* smem_raw, double* partial) {
+    if (rl.ril == 0 && rl.ng == 0) {
+        block_sum_store(v, smem_raw, partial + (long long)w.slot * w.nblk + w.tile);
+        return;
+    }
+    const int gm = rl.gmask[blockIdx.x % rl.ng];
+    for (int j = 0; j < (1 << rl.ril); ++j) {
+        if (!((gm >> j) & 1)) continue;
+        block_sum_store(w.ri == j && w.live ? v : 0.0, smem_raw, partial + (long long)rl.slot_of[((w.grp << rl.ril) + j) & 63] * w.nblk + w.tile);
+        __syncthreads();
+    }
+}
+// 1 / scale of an fp16 output for this thread's rhs (see block_out_scale); grouped mode evaluates the rule once per rhs
+// of the group
+template <typename S>
+__device__ __forceinline__ typename Store<S>::real work_out_scale(const ScaleRule& sr, const RowWork& w, const RhsList& rl) {
+    if constexpr (!Store<S>::HALF) return 1;
+    else {
+        if (rl.ril == 0 && rl.ng == 0) return block_out_scale<S>(sr, w.rhs, w.tile == 0);
+        __shared__ float s_oinv4[4];
+        __syncthreads();
+        if (threadIdx.x < (1u << rl.ril)) {
+            const int gm = rl.gmask[blockIdx.x % rl.ng];
+            s_oinv4[threadIdx.x] = (gm >> threadIdx.x) & 1 ? 1.0f / eval_scale(sr, (w.grp << rl.ril) + (int)threadIdx.x, w.tile == 0) : 1.0f;
+        }
+        __syncthreads();
+        return s_oinv4[w.ri];
+    }
+}
 
 // out = cx*xin + ch * G in   (G == nullptr: identity), optional sum |out|^2, optional no store
 struct LsArgs {
@@ -29,9 +88,9 @@ __global__ void __launch_bounds__(256) ls_kernel(const Geom g, const LsArgs a) {
     typedef typename Store<S>::real T;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (a.stop != nullptr && *a.stop != 0) return;
-    const int slot = blockIdx.x % a.rl.nact, tile = blockIdx.x / a.rl.nact, rhs = a.rl.rhs[slot];
-    const int idx = tile * blockDim.x + threadIdx.x;
-    const bool live = idx < g.N5h;
+    const RowWork w = map_work(g, a.rl);
+    const int rhs = w.rhs, idx = w.idx;
+    const bool live = w.live;
     T acc[24];
     if (live) load_spinor<S>(a.in, rhs, idx, g.N5h, acc);
     else {
@@ -50,7 +109,7 @@ __global__ void __launch_bounds__(256) ls_kernel(const Geom g, const LsArgs a) {
         for (int i = 0; i < 24; ++i) acc[i] *= ch;
     }
     if (a.write) {
-        const T oinv = block_out_scale<S>(a.sr, rhs, tile == 0);
+        const T oinv = work_out_scale<S>(a.sr, w, a.rl);
         if (live) store_spinor<S>(a.out, rhs, idx, g.N5h, acc, oinv);
     }
     if (a.partial != nullptr) {
@@ -59,7 +118,7 @@ __global__ void __launch_bounds__(256) ls_kernel(const Geom g, const LsArgs a) {
 #pragma unroll
             for (int i = 0; i < 24; ++i) s2 += (double)acc[i] * (double)acc[i];
         }
-        block_sum_store(s2, smem_raw, a.partial + (long long)slot * (gridDim.x / a.rl.nact) + tile);
+        block_sum_rhs(s2, w, a.rl, smem_raw, a.partial);
     }
 }
 
@@ -76,11 +135,11 @@ template <typename SO, typename SA, typename SB>
 __global__ void __launch_bounds__(256) axpby_kernel(const Geom g, const AxpbyArgs p) {
     typedef typename Store<SO>::real TO;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int slot = blockIdx.x % p.rl.nact, tile = blockIdx.x / p.rl.nact, rhs = p.rl.rhs[slot];
-    const int idx = tile * blockDim.x + threadIdx.x;
-    const bool live = idx < g.N5h;
+    const RowWork w = map_work(g, p.rl);
+    const int rhs = w.rhs, idx = w.idx;
+    const bool live = w.live;
     double s2 = 0.0;
-    const TO oinv = block_out_scale<SO>(p.sr, rhs, tile == 0);
+    const TO oinv = work_out_scale<SO>(p.sr, w, p.rl);
     if (live) {
         double o[24];
 #pragma unroll
@@ -105,8 +164,7 @@ __global__ void __launch_bounds__(256) axpby_kernel(const Geom g, const AxpbyArg
         }
         store_spinor<SO>(p.out, rhs, idx, g.N5h, w, oinv);
     }
-    if (p.partial != nullptr)
-        block_sum_store(s2, smem_raw, p.partial + (long long)slot * (gridDim.x / p.rl.nact) + tile);
+    if (p.partial != nullptr) block_sum_rhs(s2, w, p.rl, smem_raw, p.partial);
 }
 
 // CG step, part 1:  alpha = rr/pAp ;  x += alpha p ;  r -= alpha Ap ;  partial |r|^2
@@ -125,11 +183,11 @@ __global__ void __launch_bounds__(256) cg_update_xr_kernel(const Geom g, const C
     typedef typename Store<SX>::real TX;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (a.stop != nullptr && *a.stop != 0) return;
-    const int slot = blockIdx.x % a.rl.nact, tile = blockIdx.x / a.rl.nact, rhs = a.rl.rhs[slot];
-    const int idx = tile * blockDim.x + threadIdx.x;
-    const bool live = idx < g.N5h;
+    const RowWork w = map_work(g, a.rl);
+    const int rhs = w.rhs, idx = w.idx;
+    const bool live = w.live;
     double s2 = 0.0;
-    const T oinv = block_out_scale<S>(a.sr, rhs, tile == 0);
+    const T oinv = work_out_scale<S>(a.sr, w, a.rl);
     if (live) {
         const double alpha_d = a.rr[rhs] / a.pAp[rhs];
         T pv[24], rv[24], av[24];
@@ -149,7 +207,7 @@ __global__ void __launch_bounds__(256) cg_update_xr_kernel(const Geom g, const C
         store_spinor<SX>(a.x, rhs, idx, g.N5h, xv);
         store_spinor<S>(a.r, rhs, idx, g.N5h, rv, oinv);
     }
-    block_sum_store(s2, smem_raw, a.partial + (long long)slot * (gridDim.x / a.rl.nact) + tile);
+    block_sum_rhs(s2, w, a.rl, smem_raw, a.partial);
 }
 
 // CG step, part 2:  beta = rr_new/rr_old ;  p = r + beta p ;  optionally also q = G p (G = A or M5^-dag:
@@ -169,13 +227,13 @@ __global__ void __launch_bounds__(256) cg_update_p_kernel(const Geom g, const Cg
     typedef typename Store<S>::real T;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (a.stop != nullptr && *a.stop != 0) return;
-    const int slot = blockIdx.x % a.rl.nact, tile = blockIdx.x / a.rl.nact, rhs = a.rl.rhs[slot];
-    const int idx = tile * blockDim.x + threadIdx.x;
-    const bool live = idx < g.N5h;
+    const RowWork w = map_work(g, a.rl);
+    const int rhs = w.rhs, idx = w.idx;
+    const bool live = w.live;
     T pv[24];
 #pragma unroll
     for (int i = 0; i < 24; ++i) pv[i] = 0;
-    const T oinv_p = block_out_scale<S>(a.sr_p, rhs, tile == 0);
+    const T oinv_p = work_out_scale<S>(a.sr_p, w, a.rl);
     if (live) {
         const T beta = (T)(a.rr_new[rhs] / a.rr_old[rhs]);
         T rv[24];
@@ -189,12 +247,12 @@ __global__ void __launch_bounds__(256) cg_update_p_kernel(const Geom g, const Cg
         double s2 = 0.0;
 #pragma unroll
         for (int i = 0; i < 24; ++i) s2 += (double)pv[i] * (double)pv[i];
-        block_sum_store(s2, smem_raw, a.partial + (long long)slot * (gridDim.x / a.rl.nact) + tile);
+        block_sum_rhs(s2, w, a.rl, smem_raw, a.partial);
         __syncthreads();
     }
     if (a.op.kind != 0) {
         apply_ls<T>(pv, a.op, g.Ls, smem_raw);
-        const T oinv_q = block_out_scale<S>(a.sr_q, rhs, tile == 0);
+        const T oinv_q = work_out_scale<S>(a.sr_q, w, a.rl);
         if (live) store_spinor<S>(a.q, rhs, idx, g.N5h, pv, oinv_q);
     }
 }

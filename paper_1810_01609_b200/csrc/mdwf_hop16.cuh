@@ -131,8 +131,7 @@ __global__ void __launch_bounds__(PF ? 32 * MDWF_H16_MAXW : 256, MINB) hop16_ker
 #pragma unroll
     for (int l = 0; l < 8; ++l) cl[l] = (uint32_t)l * MDWF_H16_LREC + ((vc >> (4 * l)) & 7u) * 48u;
     // A-fragment addressing inside a site: row block rb at rb*384, chunk c at + c*128, this lane at + gq*16 + tq*4.
-    // Row blocks 2*mt and 2*mt + 1 are read at compile-time offsets; when the site has an odd number of row blocks the
-    // last read runs into the next site (fields carry that much slack at their end) and feeds rows that are discarded.
+    // Row blocks 2*mt and 2*mt + 1 are read at compile-time offsets; rows beyond the site's last row block are zeros.
     const uint32_t lane_off = (uint32_t)gq * 16u + (uint32_t)tq * 4u;
     constexpr int NQ = (MT * 48 + 31) / 32;
     // epilogue work items of this lane: 16-byte piece q = lane + 32 qi of the site in memory order (row block q / 24,
@@ -237,9 +236,12 @@ __global__ void __launch_bounds__(PF ? 32 * MDWF_H16_MAXW : 256, MINB) hop16_ker
                 const uint32_t* np = reinterpret_cast<const uint32_t*>(ibase + ((long long)nxh[l] * sb + lane_off));
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) {
-                    dst[mt][0] = __ldg(np + mt * 192); dst[mt][1] = __ldg(np + mt * 192 + 96);
-                    dst[mt][2] = __ldg(np + mt * 192 + 32); dst[mt][3] = __ldg(np + mt * 192 + 128);
-                    dst[mt][4] = __ldg(np + mt * 192 + 64); dst[mt][5] = __ldg(np + mt * 192 + 160);
+                    dst[mt][0] = __ldg(np + mt * 192); dst[mt][2] = __ldg(np + mt * 192 + 32); dst[mt][4] = __ldg(np + mt * 192 + 64);
+                    if (2 * mt + 1 < nrb) {      // rows 8-15 of the tile exist (the site has an odd number of row blocks otherwise)
+                        dst[mt][1] = __ldg(np + mt * 192 + 96); dst[mt][3] = __ldg(np + mt * 192 + 128); dst[mt][5] = __ldg(np + mt * 192 + 160);
+                    } else {
+                        dst[mt][1] = 0u; dst[mt][3] = 0u; dst[mt][5] = 0u;
+                    }
                 }
             };
             if (PF) load_A(0, A[0]);

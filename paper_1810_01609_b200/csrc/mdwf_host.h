@@ -6,6 +6,7 @@
 #include <set>
 #include <cstdio>
 #include <cstddef>
+#include <cstring>
 #include "../../include/mdwf.h"
 #include "mdwf_blas.cuh"
 
@@ -66,8 +67,9 @@ struct mdwf_ctx {
     struct ProfRec { cudaEvent_t e0, e1; int cls; double bytes, flops; };
     std::vector<ProfRec> prof_pending;
     std::vector<cudaEvent_t> prof_pool;
-    double prof_ms[3], prof_bytes[3], prof_flops[3];
-    long long prof_n[3];
+    // classes 0..2: hop by storage class; 3: s-direction kernel, 4: x/r update, 5: p update, 6: reduction finish, 7: axpby/convert
+    double prof_ms[8], prof_bytes[8], prof_flops[8];
+    long long prof_n[8];
     int sm_count;
     double lsop_norm[MAT_COUNT];   // 2-norm bounds of the s-direction operators (fp16 scale rules)
     mdwf::Tile16Host* tile16[3];   // tile tables of the fp16 tensor-core stencil per rhs interleave (built on first use)
@@ -106,6 +108,7 @@ namespace mdwf {
 
 inline RhsList all_rhs(int n) {
     RhsList r;
+    memset(&r, 0, sizeof(r));
     r.nact = n;
     for (int i = 0; i < 64; ++i) r.rhs[i] = i < n ? i : 0;
     return r;
@@ -134,6 +137,12 @@ struct FinishCtl { const int* stop; CgCtl* ctl; CgCtlHost* hctl; const double* p
 int launch_finish(mdwf_ctx* c, const RhsList& rl, double* out, double* out2, cudaStream_t st, double* nb = nullptr,
                   const FinishCtl* fc = nullptr);
 inline int cls_of(int prec) { return prec == 16 ? 0 : prec == 32 ? 1 : 2; }
+// per-launch event timing of a site-local kernel while mdwf_profile is on (classes 3..7)
+struct ProfScope {
+    mdwf_ctx* c; cudaStream_t st; mdwf_ctx::ProfRec r; bool on;
+    ProfScope(mdwf_ctx* c_, int cls, cudaStream_t st_);
+    ~ProfScope();
+};
 int launch_pack(mdwf_ctx* c, int prec, bool unpack, PackArgs& a, cudaStream_t st);
 int pack_field(mdwf_field* f, const double* canon, int full, int par, cudaStream_t st);
 int unpack_field(const mdwf_field* f, double* canon, int full, int par, cudaStream_t st);

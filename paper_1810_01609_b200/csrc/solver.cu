@@ -137,8 +137,7 @@ int make_work(Solver& S, Work& W, mdwf_field* ext_rhs, mdwf_field* ext_opar) {
 // the rhs ids of `act` that fall into [c0, c0 + n)
 RhsList chunk_of(const RhsList& act, int c0, int n) {
     RhsList r;
-    r.nact = 0;
-    for (int k = 0; k < 64; ++k) r.rhs[k] = 0;
+    memset(&r, 0, sizeof(r));
     for (int k = 0; k < act.nact; ++k)
         if (act.rhs[k] >= c0 && act.rhs[k] < c0 + n) r.rhs[r.nact++] = act.rhs[k];
     return r;
@@ -248,8 +247,7 @@ static int solve_core(Solver& S, Work& W, mdwf_solve_info* info, int r0, double*
         r->flip();
         if ((rc2 = S.sync())) return rc2;
         RhsList na;
-        na.nact = 0;
-        for (int k = 0; k < 64; ++k) na.rhs[k] = 0;
+        memset(&na, 0, sizeof(na));
         for (int k = 0; k < act.nact; ++k) {
             const int i = act.rhs[k];
             const double tn = std::sqrt(S.hsc(SC_TMP)[i]);
