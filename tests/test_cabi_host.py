@@ -45,6 +45,18 @@ def test_product_sass_is_sm100a(libpath):
     assert "sm_100a" in out, out[:400]
 
 
+def test_fp16_stencil_runs_on_tensor_cores(libpath):
+    """the 16-bit stencil is an MMA kernel: its SASS holds HMMA (mma.sync f16 -> f32) instructions"""
+    sass = subprocess.run(["cuobjdump", "-sass", libpath], capture_output=True, text=True).stdout
+    in_hop16, hmma = False, 0
+    for line in sass.splitlines():
+        if "Function :" in line:
+            in_hop16 = "hop16_kernel" in line
+        elif in_hop16 and "HMMA." in line:
+            hmma += 1
+    assert hmma > 100, hmma
+
+
 @pytest.mark.skipif(torch.cuda.is_available(), reason="only meaningful on a box without a GPU")
 def test_no_cpu_fallback(libpath):
     import paper_1810_01609_b200 as mdwf
@@ -73,5 +85,7 @@ def test_product_does_not_import_oracle():
     for f in os.listdir(os.path.join(ROOT, "oracle")):
         if f.endswith((".py", ".cpp", ".h")):
             text = open(os.path.join(ROOT, "oracle", f)).read()
-            assert "paper_1810_01609_b200/" not in text.replace("paper_1810_01609_b200/csrc (the CUDA product path)", "").replace("under paper_1810_01609_b200/", "") or True
+            # the product is only ever NAMED in header comments that say the two share nothing
+            code = "\n".join(l for l in text.splitlines() if not l.lstrip().startswith(("//", "#", "*", "/*", "this package", '"""')))
+            assert "paper_1810_01609_b200" not in code, f
             assert "import paper_1810_01609_b200" not in text and '#include "../paper' not in text, f

@@ -1,11 +1,12 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
 
-The oracle cannot run whole 48^3x64x10 solves, so outputs are SAMPLED: (i) the hop acts on each s-slice
-independently, so two s-slices of a full-size field are compared with the oracle hop of those slices; (ii) D is a
-radius-one stencil, so a 4^4 core inside an 8^4 patch cut out of the big lattice (links + field copied onto a small
-periodic lattice) reproduces (D psi)(x) on the core exactly -- the oracle evaluates the residual b - D x there; (iii)
-the global residual is evaluated by the library's fp64 FULL operator, itself checked against the oracle in
-test_gpu_dslash.py and on the patches here."""
+Acceptance is "solver true residual <= tol" with the ORACLE's full operator (north_star): for configs 3
+and 4 the oracle evaluates |b - D x| / |b| of sampled columns on the whole lattice on the host; for config 5 it does so
+for one of the four right-hand sides (70 M 5D sites) and, for every right-hand side, on 8^4 patches: D is a radius-one
+stencil, so a 4^4 core inside an 8^4 patch cut out of the big lattice (links + field copied onto a small periodic
+lattice) reproduces (D psi)(x) on the core exactly.  The oracle cannot run whole 48^3x64x10 SOLVES, so the solutions
+themselves are checked through these residuals; the hop acts on each s-slice independently, so two s-slices of a
+full-size field are compared with the oracle hop of those slices."""
 import numpy as np
 import pytest
 import torch
@@ -48,8 +49,14 @@ def patch_residual(cfg, p_big, U, x, b, origin, P=8):
     return rn, bn
 
 
+def oracle_residual(cfg, U, x5, b5):
+    """|b - D x| / |b| per column with the oracle's full fp64 operator on the host"""
+    p = oracle.Params(dims=cfg.dims, Ls=cfg.Ls, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=cfg.mf, bc=cfg.bc)
+    return oracle.true_residual(p, U.cpu().numpy(), x5.cpu().numpy(), b5.cpu().numpy())
+
+
 def test_c3_point_source_propagator_full_size():
-    """config 3: 24^3x64, Ls=8, 12 point sources, 16-bit inner CG to 1e-8, 4D in / 4D out (batched multi-rhs)."""
+    """config 3: 24^3x64, Ls=8, 12 point sources, 16-bit inner CG to 1e-8, 4D in / 5D out (batched multi-rhs)."""
     import paper_1810_01609_b200 as mdwf
     cfg = synth.CONFIGS[3]
     ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
@@ -59,32 +66,26 @@ def test_c3_point_source_propagator_full_size():
     eta = synth.point_sources_4d(cfg.dims).cuda()
     x5, res = ctx.mdwf_solve(eta, tol=cfg.tol, inner_prec=16, recon=12, src_kind=1, out_kind=0)
     assert res.status == mdwf.OK, res
+    assert res.batch == 12                      # all twelve columns in flight together
     assert max(res.true_resid) <= cfg.tol
     cols = [0, 5, 11]
     b5 = ctx.mdwf_wall_inject(eta[cols].contiguous())
-    Dx = ctx.mdwf_dslash(mdwf.OP_FULL, x5[cols].contiguous(), prec=64, recon=18)
-    for r in range(3):
-        assert float(torch.linalg.vector_norm(b5[r] - Dx[r]) / torch.linalg.vector_norm(b5[r])) <= cfg.tol
-    # oracle check of D on a patch around the source-free region and of the 4D projection rule on it
-    origin = (4, 6, 8, 10)
-    idx = torch.from_numpy(patch_indices(cfg.dims, origin)).cuda()
-    pp = oracle.Params(dims=(8,) * 4, Ls=cfg.Ls, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=cfg.mf, bc=(1, 1, 1, 1))
-    Do = oracle.D(pp, U[:, idx].cpu().numpy(), x5[cols][:, :, idx].cpu().numpy()).reshape(3, cfg.Ls, 8, 8, 8, 8, 12)
-    Dg = Dx[:, :, idx].cpu().numpy().reshape(3, cfg.Ls, 8, 8, 8, 8, 12)
-    c = slice(2, 6)
-    # away from the source D x = 0 up to the residual, so the difference is measured against |x| on the core
-    xc = x5[cols][:, :, idx].cpu().numpy().reshape(3, cfg.Ls, 8, 8, 8, 8, 12)[:, :, c, c, c, c]
-    assert np.linalg.norm((Dg - Do)[:, :, c, c, c, c]) <= 1e-12 * np.linalg.norm(xc)
+    # the oracle's wall injection and the oracle's full operator decide
+    pfull = oracle.Params(dims=cfg.dims, Ls=cfg.Ls, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=cfg.mf, bc=cfg.bc)
+    bo = oracle.wall_inject(pfull, U.cpu().numpy(), eta[cols].cpu().numpy())
+    assert rel(b5.cpu().numpy(), bo) <= 1e-12
+    tr = oracle.true_residual(pfull, U.cpu().numpy(), x5[cols].cpu().numpy(), bo)
+    assert tr.max() <= cfg.tol, tr
     q = ctx.mdwf_wall_project(x5)
-    qo = oracle.wall_project(pp, x5[cols][:, :, idx].cpu().numpy())
-    assert np.array_equal(q[cols][:, idx].cpu().numpy(), qo)
+    qo = oracle.wall_project(pfull, x5[cols].cpu().numpy())
+    assert np.array_equal(q[cols].cpu().numpy(), qo)
     ctx.mdwf_destroy()
 
 
 def test_c4_fh_chain_full_size():
     """config 4: 32^3x48, Ls=12: smeared 12-column source -> S ; gamma_z gamma_5 S on all t ; S_FH ; C(t) with and
-    without the insertion.  Solves are checked through the fp64 residual of the 5D systems (sampled columns), the
-    sequential source and one timeslice of each contraction against the oracle's literal sums."""
+    without the insertion.  Solves are checked through the ORACLE's fp64 residual of the 5D systems (two columns of each
+    solve), the sequential source and one timeslice of each contraction against the oracle's literal sums."""
     import paper_1810_01609_b200 as mdwf
     cfg = synth.CONFIGS[4]
     ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
@@ -102,13 +103,17 @@ def test_c4_fh_chain_full_size():
     # sequential source: exact signed permutation of the input, all columns
     Sn = S[:2].cpu().numpy()
     assert rel(seq[:2].cpu().numpy(), oracle.seq_source(cfg.dims, Sn, G)) <= 1e-15
-    # 5D residual of two columns of the second solve, by the fp64 FULL operator
-    x5, r3 = ctx.mdwf_solve(seq[3:5].contiguous(), tol=cfg.tol, inner_prec=16, recon=12, src_kind=1, out_kind=0)
-    b5 = ctx.mdwf_wall_inject(seq[3:5].contiguous())
-    Dx = ctx.mdwf_dslash(mdwf.OP_FULL, x5, prec=64, recon=18)
-    for r in range(2):
-        assert float(torch.linalg.vector_norm(b5[r] - Dx[r]) / torch.linalg.vector_norm(b5[r])) <= cfg.tol
-    assert rel(ctx.mdwf_wall_project(x5).cpu().numpy(), SFH[3:5].cpu().numpy()) <= 1e-6
+    # 5D residual of two columns of each solve by the oracle's operator (the 5D solutions are solved again, 5D out)
+    pfull = oracle.Params(dims=cfg.dims, Ls=cfg.Ls, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=cfg.mf, bc=cfg.bc)
+    Un = U.cpu().numpy()
+    for src4, prop4 in ((eta[1:3].contiguous(), S[1:3]), (seq[3:5].contiguous(), SFH[3:5])):
+        x5, r3 = ctx.mdwf_solve(src4, tol=cfg.tol, inner_prec=16, recon=12, src_kind=1, out_kind=0)
+        assert r3.status == mdwf.OK
+        bo = oracle.wall_inject(pfull, Un, src4.cpu().numpy())
+        tr = oracle.true_residual(pfull, Un, x5.cpu().numpy(), bo)
+        assert tr.max() <= cfg.tol, tr
+        assert rel(ctx.mdwf_wall_project(x5).cpu().numpy(), prop4.cpu().numpy()) <= 1e-6
+        del x5
     # contractions: one timeslice by the oracle's literal loops
     P = 0.5 * (np.eye(4) + oracle.gamma(3))
     c0 = ctx.mdwf_nucleon_2pt(S, S, S, P).cpu().numpy()
@@ -123,13 +128,15 @@ def test_c4_fh_chain_full_size():
     ctx.mdwf_destroy()
 
 
-@pytest.fixture(scope="module")
-def c5():
+@pytest.fixture
+def c5(request):
+    """a fresh context per test (a module-wide one would keep its cached work fields alive: the four-rhs solve needs
+    nearly the whole device)"""
     import paper_1810_01609_b200 as mdwf
     cfg = synth.CONFIGS[5]
     ctx = mdwf.Context(cfg.dims, cfg.Ls, cfg.M5, cfg.b5, cfg.c5, cfg.mf, bc=cfg.bc)
     U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(5, 1), device="cuda")
-    for prec, recon in [(64, 18), (32, 12), (16, 12)]:
+    for prec, recon in getattr(request, "param", [(64, 18), (16, 12)]):
         ctx.mdwf_load_gauge(U, prec, recon)
     yield mdwf, cfg, ctx, U
     ctx.mdwf_destroy()
@@ -137,6 +144,7 @@ def c5():
     torch.cuda.empty_cache()
 
 
+@pytest.mark.parametrize("c5", [[(64, 18), (32, 12), (16, 12)]], indirect=True)
 def test_c5_hop_two_slices_vs_oracle(c5):
     """48^3x64, Ls=10: packed hop in fp64/fp32/fp16 storage; slices s = 0 and 7 against the oracle."""
     mdwf, cfg, ctx, U = c5
@@ -154,28 +162,48 @@ def test_c5_hop_two_slices_vs_oracle(c5):
         del out
 
 
-def test_c5_solve_sampled_residual(c5):
-    """config 5 as bench.py runs it (16-bit inner, 12-real links, tol 1e-10; bench.py's automatic batching also
-    solves one rhs at a time at this size), 1 of the 4 rhs to bound time and memory."""
+def test_c5_solve_all_four_rhs(c5):
+    """config 5 exactly as bench.py runs it: the four Gaussian right-hand sides IN FLIGHT TOGETHER through the packed
+    in-place solve (16-bit inner, 12-real links, tol 1e-10).  Every rhs: oracle residual on two 8^4 patches; rhs 0: the
+    oracle's residual on the whole lattice."""
+    import bench
     mdwf, cfg, ctx, U = c5
     torch.cuda.empty_cache()
-    b = synth.gaussian_spinor_device(cfg.dims, cfg.Ls, 1, synth.seed_for(5, 2), device="cuda")
-    x, res = ctx.mdwf_solve(b, tol=cfg.tol, inner_prec=16, recon=12, symmetric=True)
+    nrhs, Vh, dev = cfg.nrhs, cfg.V4 // 2, torch.device("cuda", 0)
+    psi = [ctx.mdwf_field_create(64, nrhs), ctx.mdwf_field_create(64, nrhs)]
+    scratch = torch.empty((1, cfg.Ls, Vh, 4, 3), dtype=torch.complex128, device=dev)
+    seed = synth.seed_for(5, 2)
+    bench.fill_packed_rhs(psi, cfg, nrhs, seed, dev, scratch)
+    ws = torch.empty(ctx.mdwf_workspace_bytes(nrhs, 16, packed=True), dtype=torch.uint8, device=dev)   # as bench.py does
+    ctx.mdwf_set_workspace(ws)
+    res = ctx.mdwf_solve_packed(psi[0], psi[1], tol=cfg.tol, inner_prec=16, recon=12, symmetric=True)
     assert res.status == mdwf.OK, res
-    # (iii) global true residual with the library's fp64 full operator
-    Dx = ctx.mdwf_dslash(mdwf.OP_FULL, x, prec=64, recon=18)
-    for r in range(1):
-        tr = float(torch.linalg.vector_norm(b[r] - Dx[r]) / torch.linalg.vector_norm(b[r]))
-        assert tr <= cfg.tol, (r, tr)
-        assert abs(tr - res.true_resid[r]) <= 0.05 * tr + 1e-14
-    # (ii) the oracle's D on patches: the fp64 FULL operator agrees with it, and the residual is small there
-    p_big = None
-    for origin in [(2, 4, 6, 8), (30, 20, 10, 40)]:
-        idx = torch.from_numpy(patch_indices(cfg.dims, origin)).cuda()
-        pp = oracle.Params(dims=(8,) * 4, Ls=cfg.Ls, M5=cfg.M5, b5=cfg.b5, c5=cfg.c5, mf=cfg.mf, bc=(1, 1, 1, 1))
-        Do = oracle.D(pp, U[:, idx].cpu().numpy(), x[:, :, idx].cpu().numpy()).reshape(1, cfg.Ls, 8, 8, 8, 8, 12)
-        Dg = Dx[:, :, idx].cpu().numpy().reshape(1, cfg.Ls, 8, 8, 8, 8, 12)
-        c = slice(2, 6)
-        assert rel(Dg[:, :, c, c, c, c], Do[:, :, c, c, c, c]) <= 1e-12
-        rn, bn = patch_residual(cfg, p_big, U, x, b, origin)
-        assert (rn / bn <= 20 * cfg.tol).all(), (origin, rn / bn)
+    assert res.batch == nrhs                    # all four in flight
+    assert max(res.true_resid) <= cfg.tol
+    ctx.mdwf_set_workspace(None)
+    del ws
+    torch.cuda.empty_cache()
+    # site lists of the two parities (full-lattice index of the k-th half-lattice site), from the oracle's own map
+    par_idx = [torch.from_numpy(oracle.sites_of_parity(cfg.dims, par).astype(np.int64)).cuda() for par in (0, 1)]
+    g = torch.Generator(device=dev)
+    x = torch.empty((1, cfg.Ls, cfg.V4, 4, 3), dtype=torch.complex128, device=dev)
+    b = torch.empty_like(x)
+    for r in range(nrhs):
+        for par in (0, 1):
+            psi[par].mdwf_field_unpack_rhs(r, scratch)
+            x[:, :, par_idx[par]] = scratch
+            g.manual_seed(int(seed) * 1000 + 2 * r + par)            # the same draw as bench.fill_packed_rhs
+            torch.view_as_real(scratch).normal_(0.0, 1.0, generator=g)
+            b[:, :, par_idx[par]] = scratch
+        # the residual energy of a converged CG is spread over the lattice like the source's; a patch core holding a
+        # fraction f of the sites then carries |r_core| ~ sqrt(f) |r| against |b_core| ~ sqrt(f) |b|: ratio ~ the global
+        # residual.  Allow a factor 3 for the variation between patches (the global residual itself is <= tol).
+        for origin in [(2, 4, 6, 8), (30, 20, 10, 40)]:
+            rn, bn = patch_residual(cfg, None, U, x, b, origin)
+            assert (rn / bn <= 3 * cfg.tol).all(), (r, origin, rn / bn)
+        if r == 0:
+            tr = oracle_residual(cfg, U, x, b)
+            assert tr.max() <= cfg.tol, tr
+            assert abs(tr[0] - res.true_resid[0]) <= 0.05 * tr[0] + 1e-14
+    for f in psi:
+        f.mdwf_field_destroy()
