@@ -76,7 +76,9 @@ static void build_lsops(int Ls, double M5, double b5, double c5, double mf, LsOp
         o.kind = 1; o.c0 = b5; o.c1 = c5; ops[MAT_A + 4 * dag] = o;
         o.kind = 1; o.c0 = a; o.c1 = d; ops[MAT_M5 + 4 * dag] = o;
         o.kind = 2; o.c0 = 0.0; o.c1 = 1.0; ops[MAT_M5INV + 4 * dag] = o;
-        if (d != 0.0) { o.kind = 2; o.c0 = c5 / d; o.c1 = b5 - c5 * a / d; }     // (b5 + c5 L)/(a + d L)
+        // (b5 + c5 L)/(a + d L) = c5/d + (b5 - c5 a/d) M5^-1 (d != 0; mdwf_create refuses 0 < |d| < 1e-4 |a|, where the two
+        // coefficients would cancel to fewer digits than the fp32 epilogues carry);  d == 0: M5 = a, so A M5^-1 = A / a
+        if (d != 0.0) { o.kind = 2; o.c0 = c5 / d; o.c1 = b5 - c5 * a / d; }
         else { o.kind = 1; o.c0 = b5 / a; o.c1 = c5 / a; }
         ops[MAT_AM5INV + 4 * dag] = o;
     }
@@ -217,8 +219,12 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     }
     if (geo->Ls < 1 || geo->Ls > 32) MDWF_FAIL(c, MDWF_EINVAL, "Ls must be in 1..32 (got %d)", geo->Ls);
     if (v4 / 2 * geo->Ls >= (1ll << 31) / 2) MDWF_FAIL(c, MDWF_EINVAL, "lattice too large for 32-bit 5D site indices");
-    const double a = b5 * (4.0 - M5) + 1.0;
+    const double a = b5 * (4.0 - M5) + 1.0, dd = c5 * (4.0 - M5) - 1.0;
     if (a == 0.0) MDWF_FAIL(c, MDWF_EINVAL, "b5(4-M5)+1 must be non-zero");
+    // M5 = a + d L is inverted through its closed form: kappa = -d/a must contract and 1 + mf kappa^Ls must not vanish
+    if (!(std::fabs(dd / a) < 1.0)) MDWF_FAIL(c, MDWF_EINVAL, "|c5(4-M5)-1| must be smaller than |b5(4-M5)+1| (kappa = %.4g)", -dd / a);
+    if (!(std::fabs(1.0 + mf * std::pow(-dd / a, geo->Ls)) > 1e-8)) MDWF_FAIL(c, MDWF_EINVAL, "1 + mf kappa^Ls vanishes: M5 is singular");
+    if (dd != 0.0 && std::fabs(dd) < 1e-4 * std::fabs(a)) MDWF_FAIL(c, MDWF_EINVAL, "c5(4-M5)-1 = %.3g is too close to (but not) zero for the fused A M5^-1 epilogue", dd);
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
         cudaGetLastError();
@@ -286,14 +292,15 @@ const char* mdwf_last_error(const mdwf_ctx* c) { return c ? c->err.c_str() : "nu
 int64_t mdwf_launch_count(const mdwf_ctx* c) { return c ? c->launches : 0; }
 
 int mdwf_profile(mdwf_ctx* c, int enable) {
-    if (!c) return MDWF_EINVAL;
+    MDWF_ENTER(c);
     prof_drain(c);
     if (enable) for (int i = 0; i < 8; ++i) { c->prof_ms[i] = c->prof_bytes[i] = c->prof_flops[i] = 0.0; c->prof_n[i] = 0; }
     c->prof_on = enable ? 1 : 0;
     return MDWF_OK;
 }
 int mdwf_profile_read(mdwf_ctx* c, int cls, double* ms, double* bytes, double* flops, int64_t* launches) {
-    if (!c || cls < 0 || cls > 7 || !ms || !bytes || !flops || !launches) return MDWF_EINVAL;
+    MDWF_ENTER(c);
+    if (cls < 0 || cls > 7 || !ms || !bytes || !flops || !launches) return MDWF_EINVAL;
     prof_drain(c);
     *ms = c->prof_ms[cls]; *bytes = c->prof_bytes[cls]; *flops = c->prof_flops[cls]; *launches = c->prof_n[cls];
     return MDWF_OK;
@@ -345,7 +352,7 @@ int mdwf_selftest_host(double M5, double b5, double c5, double mf) {
 }
 
 int mdwf_set_tiling(mdwf_ctx* c, int zc) {
-    if (!c) return MDWF_EINVAL;
+    MDWF_ENTER(c);
     if (zc < 0 || (zc > 0 && (c->g.Z % zc != 0 || zc % c->ghop[1].tz != 0 || zc % c->ghop[2].tz != 0)))
         MDWF_FAIL(c, MDWF_EINVAL, "zc = %d must divide Z = %d and be a multiple of the tile depth %d", zc, c->g.Z, c->g.tz);
     set_zc(c, zc);
@@ -353,7 +360,7 @@ int mdwf_set_tiling(mdwf_ctx* c, int zc) {
 }
 
 int mdwf_load_gauge(mdwf_ctx* c, const void* U, int store_prec, int recon, void* stream) {
-    if (!c) return MDWF_EINVAL;
+    MDWF_ENTER(c);
     if (!U) MDWF_FAIL(c, MDWF_EINVAL, "null gauge pointer");
     GaugeSet gs;
     int rc = pack_gauge(c, U, store_prec, recon, &gs, (cudaStream_t)stream);
@@ -505,7 +512,7 @@ int unpack_field(const mdwf_field* f, double* canon, int full, int par, cudaStre
 extern "C" {
 
 int mdwf_set_hop16_tile(mdwf_ctx* c, int lx, int ly, int lz, int lt, int warps) {
-    if (!c) return MDWF_EINVAL;
+    MDWF_ENTER(c);
     if (warps < 0 || warps > MDWF_H16_MAXW) MDWF_FAIL(c, MDWF_EINVAL, "warps must be in 0..%d", MDWF_H16_MAXW);
     for (int i = 0; i < 3; ++i) if (c->tile16[i]) { free_tile16(c->tile16[i]); delete c->tile16[i]; c->tile16[i] = nullptr; }
     c->tile16_forced[0] = lx; c->tile16_forced[1] = ly; c->tile16_forced[2] = lz; c->tile16_forced[3] = lt;
@@ -514,7 +521,8 @@ int mdwf_set_hop16_tile(mdwf_ctx* c, int lx, int ly, int lz, int lt, int warps) 
 }
 
 int mdwf_field_create(mdwf_ctx* c, int prec, int nrhs, mdwf_field** out) {
-    if (!c || !out) return MDWF_EINVAL;
+    MDWF_ENTER(c);
+    if (!out) return MDWF_EINVAL;
     return alloc_field(c, prec, nrhs, out);
 }
 int mdwf_field_destroy(mdwf_field* f) {
@@ -550,13 +558,13 @@ int mdwf_field_unpack_rhs(const mdwf_field* f, int rhs, void* canonical, void* s
 
 int mdwf_dslash_packed(mdwf_ctx* c, int op, int parity, int dagger, int recon, mdwf_field* out,
                        const mdwf_field* in, void* stream) {
-    if (!c) return MDWF_EINVAL;
+    MDWF_ENTER(c);
     return dslash_packed_impl(c, op, parity, dagger, recon, out, in, (cudaStream_t)stream);
 }
 
 int mdwf_dslash(mdwf_ctx* c, int op, int parity, int dagger, int prec, int recon, void* out, const void* in,
                 int nrhs, void* stream) {
-    if (!c) return MDWF_EINVAL;
+    MDWF_ENTER(c);
     if (!out || !in) MDWF_FAIL(c, MDWF_EINVAL, "null field pointer");
     if (nrhs < 1 || nrhs > MDWF_MAX_RHS) MDWF_FAIL(c, MDWF_EINVAL, "nrhs must be in 1..%d", MDWF_MAX_RHS);
     cudaStream_t st = (cudaStream_t)stream;

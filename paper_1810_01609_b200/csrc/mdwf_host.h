@@ -97,6 +97,12 @@ struct mdwf_ctx {
         (ctx)->err = _b;                                   \
         return (code);                                     \
     } while (0)
+// every entry point runs on the context's device, whatever the caller's current device is
+#define MDWF_ENTER(ctx)                                                                                   \
+    do {                                                                                                  \
+        if (!(ctx)) return MDWF_EINVAL;                                                                   \
+        if (cudaSetDevice((ctx)->geo.device) != cudaSuccess) { cudaGetLastError(); (ctx)->err = "cudaSetDevice failed"; return MDWF_ECUDA; } \
+    } while (0)
 #define MDWF_CUDA(ctx, expr)                                                                             \
     do {                                                                                                 \
         cudaError_t _e = (expr);                                                                         \

@@ -258,7 +258,7 @@ using namespace mdwf;
 extern "C" {
 
 int mdwf_wall_inject(mdwf_ctx* c, void* b5, const void* eta4, int ncol, int recon, void* stream) {
-    if (!c) return MDWF_EINVAL;
+    MDWF_ENTER(c);
     if (!b5 || !eta4) MDWF_FAIL(c, MDWF_EINVAL, "null pointer");
     if (ncol < 1 || ncol > MDWF_MAX_RHS) MDWF_FAIL(c, MDWF_EINVAL, "ncol must be in 1..%d", MDWF_MAX_RHS);
     cudaStream_t st = (cudaStream_t)stream;
@@ -280,7 +280,7 @@ int mdwf_wall_inject(mdwf_ctx* c, void* b5, const void* eta4, int ncol, int reco
 }
 
 int mdwf_wall_project(mdwf_ctx* c, void* q4, const void* psi5, int ncol, void* stream) {
-    if (!c) return MDWF_EINVAL;
+    MDWF_ENTER(c);
     if (!q4 || !psi5 || ncol < 1) MDWF_FAIL(c, MDWF_EINVAL, "bad argument");
     const long long V4 = 2ll * c->g.Vh, n = (long long)ncol * V4 * 12;
     wall_project_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>((double2*)q4, (const double2*)psi5, V4, c->g.Ls, ncol);
@@ -291,7 +291,7 @@ int mdwf_wall_project(mdwf_ctx* c, void* q4, const void* psi5, int ncol, void* s
 
 int mdwf_seq_source(mdwf_ctx* c, void* out4d, const void* prop4d, int ncol, const double* Gamma_host, int t_min,
                     int t_max, void* stream) {
-    if (!c) return MDWF_EINVAL;
+    MDWF_ENTER(c);
     if (!out4d || !prop4d || !Gamma_host || ncol < 1) MDWF_FAIL(c, MDWF_EINVAL, "bad argument");
     SeqArgs a;
     a.out = (double2*)out4d; a.in = (const double2*)prop4d;
@@ -306,7 +306,7 @@ int mdwf_seq_source(mdwf_ctx* c, void* out4d, const void* prop4d, int ncol, cons
 
 int mdwf_nucleon_2pt(mdwf_ctx* c, double* corr, const void* S_u1, const void* S_d, const void* S_u2,
                      const double* proj_host, int t0, void* stream) {
-    if (!c) return MDWF_EINVAL;
+    MDWF_ENTER(c);
     if (!corr || !S_u1 || !S_d || !S_u2 || !proj_host) MDWF_FAIL(c, MDWF_EINVAL, "null pointer");
     cudaStream_t st = (cudaStream_t)stream;
     NucArgs a;
