@@ -246,7 +246,7 @@ int mdwf_create(mdwf_ctx** out, const mdwf_geometry* geo, double M5, double b5, 
     int max_nblk = 0;
     for (int cls = 0; cls < 3; ++cls) {
         c->ghop[cls] = g;
-        if (cls == 0) pick_tile(c->ghop[cls], std::min(128 / g.Ls, 32));
+        if (cls == 0) pick_tile(c->ghop[cls], std::min(128 / g.Ls, 32));   // blocks of the site-local fp16 kernels (measured: ~128 threads)
         c->blk_cls[cls] = c->ghop[cls].nsite * g.Ls;
         c->nblk_cls[cls] = g.Vh / c->ghop[cls].nsite;
         max_nblk = std::max(max_nblk, c->nblk_cls[cls]);

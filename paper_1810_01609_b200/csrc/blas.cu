@@ -275,7 +275,7 @@ int launch_finish(mdwf_ctx* c, const RhsList& rl, double* out, double* out2, cud
     f.out2 = out2;
     f.nb = nb;
     f.rl = rl;
-    finish_sum_kernel<<<rl.nact, 256, 0, st>>>(f);
+    finish_sum_kernel<<<rl.nact, 1024, 0, st>>>(f);
     MDWF_CUDA(c, cudaGetLastError());
     c->launches++;
     return MDWF_OK;

@@ -94,10 +94,11 @@ void free_tile16(Tile16Host* th) {
     for (int i = 0; i < 2; ++i) if (th->dev[i]) { cudaFree(th->dev[i]); th->dev[i] = nullptr; }
 }
 
-// Tile choice.  The block's tile decides how often an input site is found again in L1 by another leg: a 2^4 box has 8
-// output sites and 40 distinct inputs (5 fetches per output instead of 8), 4x2x2x2 has 16 and 72 (4.5).  Default: the
-// largest box of at most 16 sites built from extents <= 4 (x) and <= 2 (y, z, t) that divides the lattice, one site
-// per warp.  mdwf_set_hop16_tile forces a box / warp count (tuning).
+// Tile choice.  The block's tile decides how often an input site is found again in L1 by another leg (a 2^4 box has 8
+// output sites and 40 distinct inputs: 5 fetches per output instead of 8; 4x4x2x2 has 32 and 128: 4), and with several
+// sites per warp all 32 lanes share the link staging of a tile.  Measured on B200 (48^3x64x10, 4 rhs; profiles/README.md):
+// 4x4x2x2 with 8 warps (4 sites per warp, two blocks per SM) is ~10 % faster than one site per warp.  Default: extents
+// (4, 4, 2, 2) reduced to divisors of the lattice, 8 warps.  mdwf_set_hop16_tile forces a box / warp count (tuning).
 static int choose_tile16(mdwf_ctx* c, int rows, int L[4], int* nw_out) {
     const Geom& g = c->g;
     const int dims[4] = {g.X, g.Y, g.Z, g.T};
@@ -112,13 +113,25 @@ static int choose_tile16(mdwf_ctx* c, int rows, int L[4], int* nw_out) {
         *nw_out = nw;
         return MDWF_OK;
     }
-    const int want[4] = {2, 2, 2, 2};
-    for (int d = 0; d < 4; ++d) L[d] = dims[d] % want[d] == 0 ? want[d] : 1;
+    const int want[4] = {4, 4, 2, 2};
+    for (int d = 0; d < 4; ++d) {
+        L[d] = want[d];
+        while (dims[d] % L[d]) L[d] >>= 1;
+    }
     if (L[0] < 2) L[0] = 2;
-    *nw_out = std::min(L[0] * L[1] * L[2] * L[3] / 2, MDWF_H16_MAXW);
-    const Plan16 p = plan_tile16(L, rows, *nw_out);
-    if (p.smem > cap) MDWF_FAIL(c, MDWF_EINVAL, "fp16 stencil tile does not fit in shared memory (%d rows per site)", rows);
-    return MDWF_OK;
+    for (;;) {
+        const int ns = L[0] * L[1] * L[2] * L[3] / 2;
+        *nw_out = std::min(std::max(ns / 4, std::min(ns, 8)), MDWF_H16_MAXW);
+        const Plan16 p = plan_tile16(L, rows, *nw_out);
+        if (p.smem <= cap / 2 && p.spw <= 4) return MDWF_OK;          // two blocks per SM
+        int d = 3;
+        while (d >= 0 && L[d] <= (d == 0 ? 2 : 1)) --d;
+        if (d < 0) {
+            if (p.smem <= cap && p.spw <= 4) return MDWF_OK;
+            MDWF_FAIL(c, MDWF_EINVAL, "fp16 stencil tile does not fit in shared memory (%d rows per site)", rows);
+        }
+        L[d] >>= 1;
+    }
 }
 
 // tiles are cached per rhs interleave (the epilogue tile holds RI * Ls rows per site)

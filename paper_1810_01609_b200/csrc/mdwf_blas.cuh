@@ -42,17 +42,31 @@ __device__ __forceinline__ RowWork map_work(const Geom& g, const RhsList& rl) {
     return w;
 }
 // fixed-order block sums per rhs of the block: plain mode one sum, grouped mode one per active rhs of the group
-__device__ __forceinline__ void block_sum_rhs(double v, const RowWork& w, const RhsList& rl, unsigned char* smem_raw, double* partial) {
+__device__ __forceinline__ void block_sum_rhs(double v, const RowWork& w, const RhsList& rl, unsigned char* smem_raw, double* partial, int g_Ls) {
     if (rl.ril == 0 && rl.ng == 0) {
         block_sum_store(v, smem_raw, partial + (long long)w.slot * w.nblk + w.tile);
         return;
     }
-    const int gm = rl.gmask[blockIdx.x % rl.ng];
-    for (int j = 0; j < (1 << rl.ril); ++j) {
-        if (!((gm >> j) & 1)) continue;
-        block_sum_store(w.ri == j && w.live ? v : 0.0, smem_raw, partial + (long long)rl.slot_of[((w.grp << rl.ril) + j) & 63] * w.nblk + w.tile);
-        __syncthreads();
+    // grouped mode: one pass through shared memory, then thread j < RI sums the entries of rhs j in thread order (the
+    // Ls threads of a (site, rhs) are consecutive and the rhs of a site follow each other, so thread t belongs to rhs
+    // (first + t / Ls) mod RI): two barriers instead of 4 RI
+    double* red = reinterpret_cast<double*>(smem_raw);
+    __syncthreads();
+    red[threadIdx.x] = w.live ? v : 0.0;
+    __syncthreads();
+    const int RI = 1 << rl.ril;
+    if ((int)threadIdx.x < RI) {
+        const int gm = rl.gmask[blockIdx.x % rl.ng], j = threadIdx.x;
+        if ((gm >> j) & 1) {
+            const int Ls = (int)g_Ls, ngrp = (int)blockDim.x / Ls;          // (site, rhs) groups of Ls threads in the block
+            const int first = (int)(((unsigned)w.tile * blockDim.x / (unsigned)Ls) & (unsigned)(RI - 1));   // rhs-in-group of thread 0
+            double tot = 0.0;
+            for (int q = (j - first) & (RI - 1); q < ngrp; q += RI)
+                for (int t = q * Ls; t < q * Ls + Ls; ++t) tot += red[t];
+            partial[(long long)rl.slot_of[((w.grp << rl.ril) + j) & 63] * w.nblk + w.tile] = tot;
+        }
     }
+    __syncthreads();
 }
 // 1 / scale of an fp16 output for this thread's rhs (see block_out_scale); grouped mode evaluates the rule once per rhs
 // of the group
@@ -118,7 +132,7 @@ __global__ void __launch_bounds__(256) ls_kernel(const Geom g, const LsArgs a) {
 #pragma unroll
             for (int i = 0; i < 24; ++i) s2 += (double)acc[i] * (double)acc[i];
         }
-        block_sum_rhs(s2, w, a.rl, smem_raw, a.partial);
+        block_sum_rhs(s2, w, a.rl, smem_raw, a.partial, g.Ls);
     }
 }
 
@@ -164,7 +178,7 @@ __global__ void __launch_bounds__(256) axpby_kernel(const Geom g, const AxpbyArg
         }
         store_spinor<SO>(p.out, rhs, idx, g.N5h, w, oinv);
     }
-    if (p.partial != nullptr) block_sum_rhs(s2, w, p.rl, smem_raw, p.partial);
+    if (p.partial != nullptr) block_sum_rhs(s2, w, p.rl, smem_raw, p.partial, g.Ls);
 }
 
 // CG step, part 1:  alpha = rr/pAp ;  x += alpha p ;  r -= alpha Ap ;  partial |r|^2
@@ -207,7 +221,7 @@ __global__ void __launch_bounds__(256) cg_update_xr_kernel(const Geom g, const C
         store_spinor<SX>(a.x, rhs, idx, g.N5h, xv);
         store_spinor<S>(a.r, rhs, idx, g.N5h, rv, oinv);
     }
-    block_sum_rhs(s2, w, a.rl, smem_raw, a.partial);
+    block_sum_rhs(s2, w, a.rl, smem_raw, a.partial, g.Ls);
 }
 
 // CG step, part 2:  beta = rr_new/rr_old ;  p = r + beta p ;  optionally also q = G p (G = A or M5^-dag:
@@ -247,7 +261,7 @@ __global__ void __launch_bounds__(256) cg_update_p_kernel(const Geom g, const Cg
         double s2 = 0.0;
 #pragma unroll
         for (int i = 0; i < 24; ++i) s2 += (double)pv[i] * (double)pv[i];
-        block_sum_rhs(s2, w, a.rl, smem_raw, a.partial);
+        block_sum_rhs(s2, w, a.rl, smem_raw, a.partial, g.Ls);
         __syncthreads();
     }
     if (a.op.kind != 0) {
@@ -289,18 +303,18 @@ struct FinishArgs {
     const double* pap;  // loop control: <p, A p> of the iteration (breakdown check)
     int seq;
 };
-static __global__ void __launch_bounds__(256) finish_sum_kernel(const FinishArgs a) {
-    __shared__ double red[256];
+static __global__ void __launch_bounds__(1024) finish_sum_kernel(const FinishArgs a) {
+    __shared__ double red[1024];
     const int slot = blockIdx.x, rhs = a.rl.rhs[slot];
     const bool skip = a.stop != nullptr && *a.stop != 0;
     bool want_stop = false;
     if (!skip) {
         const double* p = a.partial + (long long)slot * a.nblk;
         double s = 0.0;
-        for (int i = threadIdx.x; i < a.nblk; i += 256) s += p[i];
+        for (int i = threadIdx.x; i < a.nblk; i += 1024) s += p[i];
         red[threadIdx.x] = s;
         __syncthreads();
-        for (int o = 128; o > 0; o >>= 1) {
+        for (int o = 512; o > 0; o >>= 1) {
             if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
             __syncthreads();
         }

@@ -277,15 +277,25 @@ __global__ void __launch_bounds__(PF ? 32 * MDWF_H16_MAXW : 256, MINB) hop16_ker
             if (op.kind == 2) {
                 // closed form of M5^-1 as a first-order recurrence along s (mdwf_hop.cuh, LsOp), one lane per column of a rhs:
                 // P_s = v_s + kappa P_{s-1} in place (forward for one chirality, backward for the other)
-                for (int j = lane; j < RI * 24; j += 32) {
-                    const int rj = j / 24, col = j - rj * 24;
-                    const bool fwd = ((col & 7) < 4) != (op.dag != 0);
-                    float run = 0.f;
-                    float* base = E + rj * Ls * 24 + col;
-                    for (int kk = 0; kk < Ls; ++kk) {
-                        float* p = base + (fwd ? kk : Ls - 1 - kk) * 24;
-                        run = *p + kap * run;
-                        *p = run;
+                // (up to three columns per lane, advanced together so that their dependent load-fma-store chains overlap)
+                float* cb[3];
+                bool cf[3], cv[3];
+                float run[3] = {0.f, 0.f, 0.f};
+#pragma unroll
+                for (int u = 0; u < 3; ++u) {
+                    const int j = lane + 32 * u, rj = j / 24, col = j - rj * 24;
+                    cv[u] = j < RI * 24;
+                    cf[u] = ((col & 7) < 4) != (op.dag != 0);
+                    cb[u] = E + rj * Ls * 24 + col;
+                }
+                for (int kk = 0; kk < Ls; ++kk) {
+#pragma unroll
+                    for (int u = 0; u < 3; ++u) {
+                        if (cv[u]) {
+                            float* p = cb[u] + (cf[u] ? kk : Ls - 1 - kk) * 24;
+                            run[u] = *p + kap * run[u];
+                            *p = run[u];
+                        }
                     }
                 }
                 __syncwarp();
