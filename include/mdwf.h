@@ -186,12 +186,31 @@ int64_t mdwf_launch_count(const mdwf_ctx* ctx);
  * and the launch count. */
 int mdwf_profile(mdwf_ctx* ctx, int enable);
 int mdwf_profile_read(mdwf_ctx* ctx, int cls, double* ms, double* bytes, double* flops, int64_t* launches);
-/* set the z-slab depth of the hop kernel's site traversal (L2 tiling); 0 = automatic */
+/* force the z-slab depth of the fp32 / fp64 hop kernel's site traversal (L2 tiling); 0 = back to the tuned
+ * (mdwf_autotune) or heuristic value.  zc must divide Z and be a multiple of the block's z extent (else EINVAL). */
 int mdwf_set_tiling(mdwf_ctx* ctx, int zc);
 
+/* Run-time autotuner ("GPU kernel autotuning ... brute-force search ... stored in a std::map", PAPER.md:92-94 IV).
+ * mdwf_autotune times, on scratch fields of the real size (3 fields of `nrhs` columns in precision `prec` are allocated
+ * for the duration of the call; ENOMEM if they do not fit), the free launch parameters of the Dslash stencil for the
+ * loaded gauge format (prec, recon) (ESTATE if it is not loaded) with `nrhs` right-hand sides per launch -- prec 16: the
+ * 4D tile and warps per block of the tensor-core kernel; prec 32 / 64: the z-slab depth -- keeps the fastest in the
+ * context and uses it for every later launch of that (lattice, Ls, prec, rhs count).  Results never depend on these
+ * parameters beyond the order of fp32 partial sums.  The call synchronises the stream.  Forced values
+ * (mdwf_set_tiling, mdwf_set_hop16_tile) take precedence over tuned ones.
+ * mdwf_tune_save / mdwf_tune_load write / read all entries as a text file ("key v0 v1 ..." per line; entries of other
+ * lattices are kept and never match); EINVAL if the file cannot be opened or parsed.
+ * mdwf_tune_get copies the values of one entry (keys: "hop16/XxYxZxT/LsN/rowsR" -> lx ly lz lt warps;
+ * "hop32/.../rhsN", "hop64/.../rhsN" -> zc) into values[0..cap) and returns their number, 0 if there is no such entry,
+ * < 0 on a null argument. */
+int mdwf_autotune(mdwf_ctx* ctx, int prec, int recon, int nrhs, void* stream);
+int mdwf_tune_save(mdwf_ctx* ctx, const char* path);
+int mdwf_tune_load(mdwf_ctx* ctx, const char* path);
+int mdwf_tune_get(mdwf_ctx* ctx, const char* key, int* values, int cap);
+
 /* Tuning control of the fp16 tensor-core stencil (mdwf_hop16.cuh): the 4D box of output sites one block owns
- * (lx even; each extent divides the lattice) and the warps per block (0 = default).  lx = 0 returns to the automatic
- * choice.  Results do not depend on it beyond fp32 summation order.  EINVAL if the box does not fit in shared memory. */
+ * (lx even; each extent divides the lattice) and the warps per block (0 = default).  lx = 0 returns to the tuned (mdwf_autotune)
+ * or default choice.  Results do not depend on it beyond fp32 summation order.  EINVAL if the box does not fit in shared memory. */
 int mdwf_set_hop16_tile(mdwf_ctx* ctx, int lx, int ly, int lz, int lt, int warps);
 
 /* Host-only self-test (needs no GPU): the run-time-constant division used for site decoding (exhaustive over

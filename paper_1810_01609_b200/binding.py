@@ -26,6 +26,7 @@ EXPORTS = [
     "mdwf_solve", "mdwf_solve_host", "mdwf_seq_source", "mdwf_nucleon_2pt", "mdwf_wall_inject",
     "mdwf_wall_project", "mdwf_launch_count", "mdwf_set_tiling", "mdwf_profile", "mdwf_profile_read", "mdwf_selftest_host", "mdwf_solve_packed",
     "mdwf_workspace_bytes", "mdwf_set_workspace", "mdwf_set_hop16_tile", "mdwf_field_pack_rhs", "mdwf_field_unpack_rhs",
+    "mdwf_autotune", "mdwf_tune_save", "mdwf_tune_load", "mdwf_tune_get",
 ]
 
 
@@ -95,6 +96,10 @@ def lib():
         L.mdwf_workspace_bytes.argtypes = [vp, ci, ci, ci, ctypes.POINTER(ctypes.c_int64)]
         L.mdwf_set_workspace.argtypes = [vp, vp, ctypes.c_int64]
         L.mdwf_set_hop16_tile.argtypes = [vp, ci, ci, ci, ci, ci]
+        L.mdwf_autotune.argtypes = [vp, ci, ci, ci, vp]
+        L.mdwf_tune_save.argtypes = [vp, ctypes.c_char_p]
+        L.mdwf_tune_load.argtypes = [vp, ctypes.c_char_p]
+        L.mdwf_tune_get.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(ctypes.c_int), ci]
         L.mdwf_field_pack_rhs.argtypes = [vp, ci, vp, vp]
         L.mdwf_field_unpack_rhs.argtypes = [vp, ci, vp, vp]
         _lib = L
@@ -299,6 +304,22 @@ class Context:
 
     def mdwf_set_hop16_tile(self, lx, ly, lz, lt, warps=0):
         self._chk(lib().mdwf_set_hop16_tile(self._h, lx, ly, lz, lt, warps))
+
+    def mdwf_autotune(self, prec, recon, nrhs=1):
+        self._chk(lib().mdwf_autotune(self._h, prec, recon, nrhs, _stream()))
+
+    def mdwf_tune_save(self, path):
+        self._chk(lib().mdwf_tune_save(self._h, str(path).encode()))
+
+    def mdwf_tune_load(self, path):
+        self._chk(lib().mdwf_tune_load(self._h, str(path).encode()))
+
+    def mdwf_tune_get(self, key):
+        buf = (ctypes.c_int * 8)()
+        n = lib().mdwf_tune_get(self._h, key.encode(), buf, 8)
+        if n < 0:
+            raise MdwfError(n, "mdwf_tune_get")
+        return [buf[i] for i in range(min(n, 8))]
 
     def mdwf_seq_source(self, prop4d: torch.Tensor, Gamma, t_min=0, t_max=None, out=None):
         ncol = prop4d.shape[0]

@@ -140,22 +140,25 @@ static void fill_zc(mdwf_ctx* c, Geom& g, int zc) {
     (void)c;
 }
 static const double kSiteBytes[3] = {48.0, 96.0, 192.0};
-static void set_zc(mdwf_ctx* c, int want) {
+namespace mdwf {
+void set_zc(mdwf_ctx* c, int want) {
     c->zc_forced = want > 0 ? want : 0;
     c->ghop_multi.clear();
     for (int cls = 0; cls < 3; ++cls) fill_zc(c, c->ghop[cls], pick_zc(c, c->ghop[cls], want, kSiteBytes[cls]));
     c->g = c->ghop[1];
 }
-namespace mdwf {
-// Geometry of a hop launch: with nact rhs in flight the slab working set is nact times larger, so the slab depth is
-// chosen for nact * (bytes per site)
+// Geometry of a hop launch.  Slab depth: forced (mdwf_set_tiling) > tuned (mdwf_autotune) > heuristic; with nact rhs in
+// flight the slab working set is nact times larger, so the heuristic is evaluated for nact * (bytes per site)
 const Geom& hop_geom(mdwf_ctx* c, int cls, int nact) {
-    if (nact <= 1 || c->zc_forced > 0) return c->ghop[cls];
+    if (c->zc_forced > 0) return c->ghop[cls];
     const int key = cls * 100 + nact;
     auto it = c->ghop_multi.find(key);
     if (it != c->ghop_multi.end()) return it->second;
+    auto tu = c->tune.find(tune_key_zc(c, cls, nact));
+    if (tu == c->tune.end() && nact <= 1) return c->ghop[cls];
     Geom g = c->ghop[cls];
-    fill_zc(c, g, pick_zc(c, g, 0, kSiteBytes[cls] * nact));
+    const int want = tu != c->tune.end() && !tu->second.empty() ? tu->second[0] : 0;   // pick_zc ignores an inadmissible value
+    fill_zc(c, g, pick_zc(c, g, want, kSiteBytes[cls] * std::max(1, nact)));
     return c->ghop_multi.emplace(key, g).first->second;
 }
 }  // namespace mdwf
@@ -500,6 +503,16 @@ int pack_field(mdwf_field* f, const double* canon, int full, int par, cudaStream
     const int rc = launch_pack(f->ctx, f->prec, false, a, st);
     f->flip();
     return rc;
+}
+// one rhs column, s-slices [s0, s0 + ns) of one parity <-> a full-lattice canonical buffer [ns][V][4][3] (host-buffer solves
+// stream a right-hand side through a small staging buffer this way); fp64 / fp32 fields only
+int pack_slices(mdwf_field* f, int rhs, double* stage, int s0, int ns, int par, bool unpack, cudaStream_t st) {
+    mdwf_ctx* c = f->ctx;
+    if (f->prec == 16 || rhs < 0 || rhs >= f->nrhs || s0 < 0 || ns < 1 || s0 + ns > c->g.Ls) MDWF_FAIL(c, MDWF_EINVAL, "internal: bad slice pack");
+    PackArgs a;
+    memset(&a, 0, sizeof(a));
+    a.f = f->view(); a.canon = stage; a.Vc = 2ll * c->g.Vh; a.full = 1; a.par = par; a.nrhs = 1; a.rhs0 = rhs; a.s0 = s0; a.ns = ns;
+    return launch_pack(c, f->prec, unpack, a, st);
 }
 int unpack_field(const mdwf_field* f, double* canon, int full, int par, cudaStream_t st) {
     PackArgs a;

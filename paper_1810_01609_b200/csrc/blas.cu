@@ -43,11 +43,19 @@ static int make_field(mdwf_ctx* c, int prec, int nrhs, void* mem, void* meta_mem
     f->rs = rhs_bytes(c->g, prec, nrhs);
     if (!mem) {
         cudaError_t e = cudaMalloc(&f->v, f->bytes);
+        if (e == cudaErrorMemoryAllocation && c->ws && !c->ws_external) {
+            // the solver workspace the library keeps between solves is only a cache: give it back and try again
+            cudaGetLastError();
+            cudaFree(c->ws);
+            c->ws = nullptr; c->ws_bytes = 0;
+            e = cudaMalloc(&f->v, f->bytes);
+        }
         if (e == cudaSuccess && prec == 16) e = cudaMemset(f->v, 0, f->bytes);     // padding rhs of the last group
         if (e != cudaSuccess) {
+            const size_t want = f->bytes;
             delete f;
             cudaGetLastError();
-            MDWF_FAIL(c, MDWF_ENOMEM, "cudaMalloc of %zu bytes for a packed field failed: %s", f->bytes, cudaGetErrorString(e));
+            MDWF_FAIL(c, MDWF_ENOMEM, "cudaMalloc of %zu bytes for a packed field failed: %s", want, cudaGetErrorString(e));
         }
     }
     if (prec == 16 && meta_mem) f->meta = reinterpret_cast<FieldMeta*>(meta_mem);

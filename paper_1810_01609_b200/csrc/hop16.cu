@@ -113,6 +113,19 @@ static int choose_tile16(mdwf_ctx* c, int rows, int L[4], int* nw_out) {
         *nw_out = nw;
         return MDWF_OK;
     }
+    auto tu = c->tune.find(tune_key_tile16(c, rows));
+    if (tu != c->tune.end() && tu->second.size() == 5) {        // found by mdwf_autotune (or loaded): use it if it is admissible here
+        bool ok = true;
+        for (int d = 0; d < 4; ++d) {
+            L[d] = tu->second[d];
+            if (L[d] < 1 || L[d] > 16 || dims[d] % L[d] || (d == 0 && (L[d] & 1))) ok = false;
+        }
+        const int nw = tu->second[4];
+        if (ok && nw >= 1 && nw <= MDWF_H16_MAXW) {
+            const Plan16 pt = plan_tile16(L, rows, nw);
+            if (pt.smem <= cap && pt.spw <= 4) { *nw_out = nw; return MDWF_OK; }
+        }
+    }
     const int want[4] = {4, 4, 2, 2};
     for (int d = 0; d < 4; ++d) {
         L[d] = want[d];

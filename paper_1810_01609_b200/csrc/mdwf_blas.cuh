@@ -352,6 +352,7 @@ struct PackArgs {
     long long Vc;           // Vh or V4
     int full, par, nrhs;
     int rhs0;               // packed rhs index = rhs0 + r for canonical rhs r
+    int s0, ns;             // ns > 0: `canon` holds only the s-slices [s0, s0 + ns) of each rhs, [rhs][ns][Vc][24]
     double* partial;        // NORM pass only: [nrhs][gridDim.x] sums of squares of the canonical data
     ScaleRule sr;           // fp16 pack only
 };
@@ -393,8 +394,9 @@ __global__ void __launch_bounds__(256) pack_kernel(const Geom g, const PackArgs 
     if (idx >= g.N5h) return;
     uint32_t xh, s;
     g.dLs.divmod((uint32_t)idx, xh, s);
+    if (a.ns > 0 && ((int)s < a.s0 || (int)s >= a.s0 + a.ns)) return;
     const long long xs = canon_site(g, a.full, a.par, (int)xh);
-    double* c = a.canon + (((long long)rhs * g.Ls + s) * a.Vc + xs) * 24;
+    double* c = a.canon + ((a.ns > 0 ? (long long)rhs * a.ns + ((int)s - a.s0) : (long long)rhs * g.Ls + s) * a.Vc + xs) * 24;
     T v[24];
     if (UNPACK) {
         load_spinor<S>(a.f, a.rhs0 + rhs, idx, g.N5h, v);

@@ -216,6 +216,8 @@ __global__ void __launch_bounds__(PF ? 32 * MDWF_H16_MAXW : 256, MINB) hop16_ker
         const char* xbase = a.xin.v != nullptr ? reinterpret_cast<const char*>(a.xin.v) + (long long)grp * a.xin.rs : nullptr;
         char* obase = reinterpret_cast<char*>(a.out.v) + (long long)grp * a.out.rs;
         float s2r[4] = {0.f, 0.f, 0.f, 0.f};
+        uint32_t A[2][MT][6];
+        bool a0_ready = false;          // A[0] already holds leg 0 of this site (issued during the previous site's last leg)
         for (int il = 0; il < spw; ++il) {
             const int i = warp * spw + il;
             if (i >= ns) break;
@@ -230,10 +232,9 @@ __global__ void __launch_bounds__(PF ? 32 * MDWF_H16_MAXW : 256, MINB) hop16_ker
                 for (int n = 0; n < 3; ++n)
 #pragma unroll
                     for (int e = 0; e < 4; ++e) acc[mt][n][e] = 0.f;
-            uint32_t A[2][MT][6];
             // A fragments of one leg: per m16 tile six 128-byte lines (rows 0-7 / 8-15 x colour chunk 0, 1, 2)
-            auto load_A = [&](int l, uint32_t (&dst)[MT][6]) {
-                const uint32_t* np = reinterpret_cast<const uint32_t*>(ibase + ((long long)nxh[l] * sb + lane_off));
+            auto load_A = [&](int nx, uint32_t (&dst)[MT][6]) {
+                const uint32_t* np = reinterpret_cast<const uint32_t*>(ibase + ((long long)nx * sb + lane_off));
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) {
                     dst[mt][0] = __ldg(np + mt * 192); dst[mt][2] = __ldg(np + mt * 192 + 32); dst[mt][4] = __ldg(np + mt * 192 + 64);
@@ -244,11 +245,19 @@ __global__ void __launch_bounds__(PF ? 32 * MDWF_H16_MAXW : 256, MINB) hop16_ker
                     }
                 }
             };
-            if (PF) load_A(0, A[0]);
+            if (PF && !a0_ready) load_A(nxh[0], A[0]);
+            a0_ready = false;
+            const long long idx0 = (long long)smeta[0] * sb;
 #pragma unroll
             for (int l = 0; l < 8; ++l) {
-                if (PF) { if (l < 7) load_A(l + 1, A[(l + 1) & 1]); }
-                else load_A(l, A[l & 1]);
+                if (PF) {
+                    if (l < 7) load_A(nxh[l + 1], A[(l + 1) & 1]);
+                    else if (il + 1 < spw && i + 1 < ns) {
+                        // leg 0 of the warp's next site of this tile: in flight during this site's last MMAs and its epilogue
+                        load_A(reinterpret_cast<const int*>(wl + (il + 1) * MDWF_H16_SREC + 8 * MDWF_H16_LREC)[4], A[0]);
+                        a0_ready = true;
+                    }
+                } else load_A(nxh[l], A[l & 1]);
                 const uint4 b0 = *reinterpret_cast<const uint4*>(wl + il * MDWF_H16_SREC + cl[l]);
                 const uint4 b1 = *reinterpret_cast<const uint4*>(wl + il * MDWF_H16_SREC + cl[l] + 16);
                 const uint32_t b2 = *reinterpret_cast<const uint32_t*>(wl + il * MDWF_H16_SREC + cl[l] + 32);
@@ -300,7 +309,6 @@ __global__ void __launch_bounds__(PF ? 32 * MDWF_H16_MAXW : 256, MINB) hop16_ker
                 }
                 __syncwarp();
             }
-            const long long idx0 = (long long)smeta[0] * sb;
 #pragma unroll
             for (int qi = 0; qi < NQ; ++qi) {
                 const int q = lane + 32 * qi;
@@ -352,6 +360,7 @@ __global__ void __launch_bounds__(PF ? 32 * MDWF_H16_MAXW : 256, MINB) hop16_ker
                         const long long off = idx0 + q * 16;
                         if (xbase != nullptr) {
                             const float cxs = (float)a.cx * cf.y;                   // cx * e_x / e_out
+                            // (loading the xpay input ahead of the s-direction operator was tried: +5 registers' worth of spills, 30 % slower)
                             const uint4 xv = __ldcs(reinterpret_cast<const uint4*>(xbase + off));
                             const float2 x0 = h2f(xv.x), x1 = h2f(xv.y), x2 = h2f(xv.z), x3 = h2f(xv.w);
                             o8[0] = fmaf(cxs, x0.x, o8[0]); o8[1] = fmaf(cxs, x0.y, o8[1]);

@@ -80,6 +80,9 @@ struct mdwf_ctx {
     mdwf::CgCtl* dctl;             // device-side loop control of the inner CG (mdwf_blas.cuh) and its pinned staging copy / mirror
     mdwf::CgCtl* hctl_stage;
     mdwf::CgCtlHost* hctl;
+    // launch parameters found by mdwf_autotune (tune.cu), keyed by kernel / lattice / Ls / rows or rhs in flight:
+    // "hop16/..." -> {lx, ly, lz, lt, warps}; "hop32/..." and "hop64/..." -> {zc}
+    std::map<std::string, std::vector<int> > tune;
     void* ws;                      // solver workspace: library-owned (kept between calls) or caller-supplied
     size_t ws_bytes;
     bool ws_external;
@@ -152,7 +155,12 @@ struct ProfScope {
 int launch_pack(mdwf_ctx* c, int prec, bool unpack, PackArgs& a, cudaStream_t st);
 int pack_field(mdwf_field* f, const double* canon, int full, int par, cudaStream_t st);
 int unpack_field(const mdwf_field* f, double* canon, int full, int par, cudaStream_t st);
+int pack_slices(mdwf_field* f, int rhs, double* stage, int s0, int ns, int par, bool unpack, cudaStream_t st);
 const mdwf::Geom& hop_geom(mdwf_ctx* c, int cls, int nact);
+void set_zc(mdwf_ctx* c, int want);                       // force (want > 0) or release (0) the z-slab depth of hop_kernel
+std::string tune_key_tile16(const mdwf_ctx* c, int rows); // rows = (rhs per interleave group) * Ls
+std::string tune_key_zc(const mdwf_ctx* c, int cls, int nact);
+void tune_invalidate(mdwf_ctx* c);                        // drop the launch tables built from forced / tuned parameters
 int pack_gauge(mdwf_ctx* c, const void* U, int prec, int recon, GaugeSet* gs, cudaStream_t st);
 void free_gauge(GaugeSet* gs);
 

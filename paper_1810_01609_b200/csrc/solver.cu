@@ -290,7 +290,9 @@ static int solve_core(Solver& S, Work& W, mdwf_solve_info* info, int r0, double*
     // turns everything queued behind it into no-ops (gate `ctl->stop`).  One cycle = arm the control block, (pending
     // p-update), iterations until the gate closes, drain, fp64 reliable update.
     const int* gate = &c->dctl->stop;
-    const int kRunAhead = 6;
+    // iterations the host may be ahead: enough to hide the launch latency of tiny lattices; on large ones an iteration takes
+    // tens of milliseconds and every iteration queued behind a closed gate costs ~3 ms of empty million-block launches
+    const int kRunAhead = (double)c->g.N5h * nb > 2.0e7 ? 2 : 6;
     bool pending_p = false;
     auto p_update = [&](const int* stop) -> int {
         int rc2;
@@ -344,7 +346,9 @@ static int solve_core(Solver& S, Work& W, mdwf_solve_info* info, int r0, double*
         const int cur0[5] = {r->cur, p->cur, t->cur, wa->cur, wb->cur};
         const int rrOld0 = rrOld, rrNew0 = rrNew;
         int queued = 0;
+        std::vector<size_t> pmark;               // profile records at the start of each queued iteration
         while (rc == MDWF_OK) {
+            if (c->prof_on) pmark.push_back(c->prof_pending.size());
             // t = S p, pAp = |t|^2 ; Ap = S^dag t   (out may alias the first work field, see op_schur)
             FinishCtl fg;
             memset(&fg, 0, sizeof(fg));
@@ -389,6 +393,14 @@ static int solve_core(Solver& S, Work& W, mdwf_solve_info* info, int r0, double*
         wa->cur = cur0[3]; wb->cur = cur0[4];      // an even number of flips per iteration
         if ((done - 1) & 1) { rrOld = rrNew0; rrNew = rrOld0; } else { rrOld = rrOld0; rrNew = rrNew0; }
         for (int k = 0; k < act.nact; ++k) iters[act.rhs[k]] += done;
+        // launches queued behind the closed gate did no work: they are not part of the per-launch profile
+        if (c->prof_on && done < (int)pmark.size()) {
+            for (size_t k = pmark[done]; k < c->prof_pending.size(); ++k) {
+                c->prof_pool.push_back(c->prof_pending[k].e0);
+                c->prof_pool.push_back(c->prof_pending[k].e1);
+            }
+            c->prof_pending.resize(pmark[done]);
+        }
         if ((rc = reliable(false))) break;
         pending_p = true;
     }
@@ -438,6 +450,114 @@ static int solve_batch(Solver& S, double* x, const double* b, const mdwf_solve_o
     return S.sync();
 }
 
+// Host-buffer solves (mdwf_solve_host): the copies are part of the call.  A 5D right-hand side is never held in canonical
+// form on the device: it streams, a few s-slices at a time, through two staging chunks on a copy stream and is packed into
+// (unpacked from) the batch's fp64 half-lattice fields as it arrives, so the device holds the same fields as a packed
+// in-place solve and the same number of right-hand sides stays in flight.  True copy/pack overlap needs pinned host
+// memory; pageable memory still gives correct results.
+struct HostStage {
+    cudaStream_t cs = nullptr;
+    void* stage[2] = {nullptr, nullptr};
+    cudaEvent_t filled[2] = {nullptr, nullptr}, drained[2] = {nullptr, nullptr};
+    void *d4in = nullptr, *d4out = nullptr;     // whole-batch buffers of 4D sources / 4D solutions
+    size_t slice_bytes = 0;
+    int ns = 1, k = 0;
+    int acquire(mdwf_ctx* c, size_t chunk, size_t in4, size_t out4) {
+        cudaError_t e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
+        for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+            if (chunk) e = cudaMalloc(&stage[i], chunk);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&filled[i], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&drained[i], cudaEventDisableTiming);
+        }
+        if (e == cudaSuccess && in4) e = cudaMalloc(&d4in, in4);
+        if (e == cudaSuccess && out4) e = cudaMalloc(&d4out, out4);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            c->err = std::string("staging buffers for host-buffer solve: ") + cudaGetErrorString(e);
+            return MDWF_ENOMEM;
+        }
+        return MDWF_OK;
+    }
+    void release() {
+        for (int i = 0; i < 2; ++i) {
+            if (stage[i]) cudaFree(stage[i]);
+            if (filled[i]) cudaEventDestroy(filled[i]);
+            if (drained[i]) cudaEventDestroy(drained[i]);
+            stage[i] = nullptr; filled[i] = drained[i] = nullptr;
+        }
+        if (d4in) cudaFree(d4in);
+        if (d4out) cudaFree(d4out);
+        d4in = d4out = nullptr;
+        if (cs) cudaStreamDestroy(cs);
+        cs = nullptr;
+    }
+};
+
+// column `col` of the two half-lattice fields <-> one canonical 5D host field, chunk by chunk
+static int stream_rhs(Solver& S, HostStage& H, mdwf_field* fpar, mdwf_field* fopar, int col, char* host, bool download) {
+    mdwf_ctx* c = S.c;
+    int rc;
+    for (int s0 = 0; s0 < c->g.Ls; s0 += H.ns, ++H.k) {
+        const int n = std::min(H.ns, c->g.Ls - s0), set = H.k & 1;
+        const size_t bytes = (size_t)n * H.slice_bytes;
+        double* stg = (double*)H.stage[set];
+        if (!download) {
+            MDWF_CUDA(c, cudaStreamWaitEvent(H.cs, H.drained[set], 0));       // the pack that last read this chunk is done
+            MDWF_CUDA(c, cudaMemcpyAsync(stg, host + (size_t)s0 * H.slice_bytes, bytes, cudaMemcpyHostToDevice, H.cs));
+            MDWF_CUDA(c, cudaEventRecord(H.filled[set], H.cs));
+            MDWF_CUDA(c, cudaStreamWaitEvent(S.st, H.filled[set], 0));
+            if ((rc = pack_slices(fpar, col, stg, s0, n, S.par, false, S.st))) return rc;
+            if ((rc = pack_slices(fopar, col, stg, s0, n, 1 - S.par, false, S.st))) return rc;
+            MDWF_CUDA(c, cudaEventRecord(H.drained[set], S.st));
+        } else {
+            MDWF_CUDA(c, cudaStreamWaitEvent(S.st, H.drained[set], 0));       // the copy that last read this chunk is done
+            if ((rc = pack_slices(fpar, col, stg, s0, n, S.par, true, S.st))) return rc;
+            if ((rc = pack_slices(fopar, col, stg, s0, n, 1 - S.par, true, S.st))) return rc;
+            MDWF_CUDA(c, cudaEventRecord(H.filled[set], S.st));
+            MDWF_CUDA(c, cudaStreamWaitEvent(H.cs, H.filled[set], 0));
+            MDWF_CUDA(c, cudaMemcpyAsync(host + (size_t)s0 * H.slice_bytes, stg, bytes, cudaMemcpyDeviceToHost, H.cs));
+            MDWF_CUDA(c, cudaEventRecord(H.drained[set], H.cs));
+        }
+    }
+    return MDWF_OK;
+}
+
+// one batch from / to host buffers
+static int solve_batch_host(Solver& S, HostStage& H, char* x, const char* b, const mdwf_solve_opts* opts, mdwf_solve_info* info,
+                            int r0, double* t_inner_ms) {
+    mdwf_ctx* c = S.c;
+    const Geom& g = c->g;
+    Work W;
+    int rc = make_work(S, W, nullptr, nullptr);
+    if (rc) return rc;
+    const size_t x4d = (size_t)2 * g.Vh * 24 * 8, x5d = x4d * g.Ls;
+    if (opts->src_kind == 0) {
+        for (int i = 0; i < S.nb; ++i)
+            if ((rc = stream_rhs(S, H, W.rhs, W.opar, i, const_cast<char*>(b) + (size_t)(r0 + i) * x5d, false))) return rc;
+    } else {
+        MDWF_CUDA(c, cudaMemcpyAsync(H.d4in, b + (size_t)r0 * x4d, x4d * S.nb, cudaMemcpyHostToDevice, S.st));
+        if ((rc = make_source(S, W, (const double*)H.d4in, 1, S.par, W.rhs))) return rc;
+        if ((rc = make_source(S, W, (const double*)H.d4in, 1, 1 - S.par, W.opar))) return rc;
+    }
+    mdwf_solve_info tmp;
+    memset(&tmp, 0, sizeof(tmp));
+    if ((rc = solve_core(S, W, &tmp, 0, t_inner_ms))) return rc;
+    for (int i = 0; i < S.nb; ++i) {
+        info->iters[r0 + i] = tmp.iters[i]; info->reliable_updates[r0 + i] = tmp.reliable_updates[i];
+        info->status[r0 + i] = tmp.status[i]; info->true_resid[r0 + i] = tmp.true_resid[i];
+    }
+    if (opts->out_kind == 0) {
+        for (int i = 0; i < S.nb; ++i)
+            if ((rc = stream_rhs(S, H, W.xh, W.opar, i, x + (size_t)(r0 + i) * x5d, true))) return rc;
+        MDWF_CUDA(c, cudaStreamSynchronize(H.cs));
+    } else {
+        if ((rc = launch_wall_unpack(c, (double*)H.d4out, W.xh->view(), S.par, S.nb, S.st))) return rc;
+        if ((rc = launch_wall_unpack(c, (double*)H.d4out, W.opar->view(), 1 - S.par, S.nb, S.st))) return rc;
+        MDWF_CUDA(c, cudaMemcpyAsync(x + (size_t)r0 * x4d, H.d4out, x4d * S.nb, cudaMemcpyDeviceToHost, S.st));
+    }
+    return S.sync();
+}
+
 static int setup_solver(mdwf_ctx* c, Solver& S, const mdwf_solve_opts* opts, cudaStream_t st) {
     if (!(opts->tol > 0.0)) MDWF_FAIL(c, MDWF_EINVAL, "tol must be > 0");
     if (opts->parity != 0 && opts->parity != 1) MDWF_FAIL(c, MDWF_EINVAL, "parity must be 0 or 1");
@@ -445,6 +565,10 @@ static int setup_solver(mdwf_ctx* c, Solver& S, const mdwf_solve_opts* opts, cud
     if (prec != 64 && prec != 32 && prec != 16) MDWF_FAIL(c, MDWF_EINVAL, "inner_prec must be 64, 32 or 16");
     S.c = c; S.st = st;
     S.prec = prec;
+    // x_lo, the solution accumulated since the last reliable update, stays in fp32 under the fp16 inner solve: fp16 rounding
+    // of x (2^-11 per element and iteration) is noise in all directions, which A = Mhat^dag Mhat amplifies by its average
+    // eigenvalue while x itself sits in the low modes -- at the condition numbers of the production workload that noise
+    // floor is above the residual the cycle is supposed to reach and the solve stalls (tried, measured, reverted)
     S.px = prec == 16 ? 32 : prec;
     S.par = opts->parity; S.sym = opts->symmetric ? 1 : 0;
     S.tol = opts->tol;
@@ -497,8 +621,24 @@ int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_o
     const size_t in_per = (size_t)2 * g.Vh * 24 * 8 * (opts->src_kind ? 1 : g.Ls);
     const size_t out_per = (size_t)2 * g.Vh * 24 * 8 * (opts->out_kind ? 1 : g.Ls);
     int nb = 1, nhi = 1;
-    const int nset_guess = (host_buffers && (opts->batch <= 0 || opts->batch < nrhs)) ? 2 : 1;
-    if ((rc = plan_batch(c, S, nrhs, opts->batch, avail_bytes(c), host_buffers ? nset_guess * (in_per + out_per) : 0, true, &nb, &nhi))) return rc;
+    HostStage H;
+    size_t avail = avail_bytes(c), per_rhs = 0;
+    if (host_buffers) {
+        // 5D fields stream through two staging chunks of whole s-slices (<= ~1.5 GB each); 4D fields (wall sources, wall-projected
+        // solutions) are small and staged whole
+        const size_t slice = (size_t)2 * g.Vh * 24 * 8;
+        H.slice_bytes = slice;
+        H.ns = (int)std::max<size_t>(1, std::min<size_t>((size_t)g.Ls, ((size_t)3 << 29) / slice));
+        if (opts->src_kind == 0 || opts->out_kind == 0) avail = avail > 2 * H.ns * slice ? avail - 2 * H.ns * slice : 0;
+        per_rhs = (opts->src_kind ? in_per : 0) + (opts->out_kind ? out_per : 0);
+    }
+    if ((rc = plan_batch(c, S, nrhs, opts->batch, avail, per_rhs, true, &nb, &nhi))) return rc;
+    if (host_buffers) {
+        // the workspace first, so that the staging buffers cannot starve it
+        if ((rc = ensure_workspace(c, work_bytes(g, S.prec, S.px, nb, nhi, true)))) return rc;
+        if ((rc = H.acquire(c, (opts->src_kind == 0 || opts->out_kind == 0) ? H.ns * H.slice_bytes : 0,
+                            opts->src_kind ? in_per * nb : 0, opts->out_kind ? out_per * nb : 0))) { H.release(); return rc; }
+    }
     memset(info, 0, sizeof(*info));
     cudaEvent_t e0, e1;
     MDWF_CUDA(c, cudaEventCreate(&e0));
@@ -514,71 +654,12 @@ int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_o
             rc = solve_batch(S, (double*)x, (const double*)b, opts, info, r0, &inner_ms);
         }
     } else {
-        // Host buffers: every batch is staged through device buffers; the copies are part of the call (mdwf.h).
-        // Two buffer sets and a copy stream: the upload of batch k+1 and the download of batch k-1 overlap the
-        // solve of batch k (true overlap needs pinned host memory; pageable memory still gives correct results).
-        void *din[2] = {nullptr, nullptr}, *dout[2] = {nullptr, nullptr};
-        cudaStream_t cs = nullptr;
-        cudaEvent_t up[2] = {nullptr, nullptr}, down[2] = {nullptr, nullptr}, solved = nullptr;
-        const int nbatch = (nrhs + nb - 1) / nb, nset = nbatch > 1 ? 2 : 1;
-        // the workspace first, so that the staging buffers cannot starve it
-        rc = ensure_workspace(c, work_bytes(g, S.prec, S.px, nb, nhi, true));
-        cudaError_t e = cudaSuccess;
-        if (rc == MDWF_OK) e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
-        for (int k = 0; k < nset && e == cudaSuccess && rc == MDWF_OK; ++k) {
-            e = cudaMalloc(&din[k], in_per * nb);
-            if (e == cudaSuccess) e = cudaMalloc(&dout[k], out_per * nb);
-            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&up[k], cudaEventDisableTiming);
-            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&down[k], cudaEventDisableTiming);
-        }
-        if (e == cudaSuccess && rc == MDWF_OK) e = cudaEventCreateWithFlags(&solved, cudaEventDisableTiming);
-        if (e != cudaSuccess) {
-            cudaGetLastError();
-            c->err = std::string("staging buffers for host-buffer solve: ") + cudaGetErrorString(e);
-            rc = MDWF_ENOMEM;
-        }
-        auto upload = [&](int k) -> cudaError_t {     // batch k -> din[k % nset] on the copy stream
-            const int r0 = k * nb, n = std::min(nb, nrhs - r0);
-            cudaError_t ee = cudaMemcpyAsync(din[k % nset], (const char*)b + in_per * r0, in_per * n, cudaMemcpyHostToDevice, cs);
-            if (ee == cudaSuccess) ee = cudaEventRecord(up[k % nset], cs);
-            return ee;
-        };
-        if (rc == MDWF_OK && (e = upload(0)) != cudaSuccess) { c->err = cudaGetErrorString(e); rc = MDWF_ECUDA; }
-        for (int k = 0; k < nbatch && rc == MDWF_OK; ++k) {
-            const int r0 = k * nb, set = k % nset;
+        for (int r0 = 0; r0 < nrhs && rc == MDWF_OK; r0 += nb) {
             S.nb = std::min(nb, nrhs - r0);
             S.nhi = std::min(nhi, S.nb);
-            e = cudaStreamWaitEvent(st, up[set], 0);                           // batch k is on the device
-            if (e == cudaSuccess && k >= nset) e = cudaStreamWaitEvent(st, down[set], 0);   // dout[set] has been drained
-            // din[(k+1) % nset] was last read by batch k-1, which has completed (solve_batch returns synchronised)
-            if (e == cudaSuccess && k + 1 < nbatch) e = upload(k + 1);
-            if (e != cudaSuccess) { c->err = cudaGetErrorString(e); rc = MDWF_ECUDA; break; }
-            mdwf_solve_info tmp;
-            memset(&tmp, 0, sizeof(tmp));
-            rc = solve_batch(S, (double*)dout[set], (const double*)din[set], opts, &tmp, 0, &inner_ms);
-            if (rc) break;
-            for (int i = 0; i < S.nb; ++i) {
-                info->iters[r0 + i] = tmp.iters[i]; info->reliable_updates[r0 + i] = tmp.reliable_updates[i];
-                info->status[r0 + i] = tmp.status[i]; info->true_resid[r0 + i] = tmp.true_resid[i];
-            }
-            e = cudaEventRecord(solved, st);
-            if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, solved, 0);
-            if (e == cudaSuccess) e = cudaMemcpyAsync((char*)x + out_per * r0, dout[set], out_per * S.nb, cudaMemcpyDeviceToHost, cs);
-            if (e == cudaSuccess) e = cudaEventRecord(down[set], cs);
-            if (e != cudaSuccess) { c->err = cudaGetErrorString(e); rc = MDWF_ECUDA; break; }
+            rc = solve_batch_host(S, H, (char*)x, (const char*)b, opts, info, r0, &inner_ms);
         }
-        if (cs) {
-            e = cudaStreamSynchronize(cs);
-            if (e != cudaSuccess && rc == MDWF_OK) { c->err = cudaGetErrorString(e); rc = MDWF_ECUDA; }
-        }
-        for (int k = 0; k < 2; ++k) {
-            if (din[k]) cudaFree(din[k]);
-            if (dout[k]) cudaFree(dout[k]);
-            if (up[k]) cudaEventDestroy(up[k]);
-            if (down[k]) cudaEventDestroy(down[k]);
-        }
-        if (solved) cudaEventDestroy(solved);
-        if (cs) cudaStreamDestroy(cs);
+        H.release();
     }
     cudaEventRecord(e1, st);
     cudaEventSynchronize(e1);
