@@ -286,6 +286,20 @@ def run_ours(args):
     ctx.mdwf_load_gauge(U, inner, recon)
     del U
     torch.cuda.empty_cache()
+    # launch parameters: the library's run-time autotuner, before anything is timed
+    tuned = {}
+    if not args.no_autotune:
+        t0 = time.time()
+        ctx.mdwf_autotune(inner, recon, nrhs)
+        ctx.mdwf_autotune(64, 18, 1)
+        lat = "%dx%dx%dx%d/Ls%d" % (tuple(cfg.dims) + (cfg.Ls,))
+        if inner == 16:
+            rows = cfg.Ls * max(r for r in (1, 2, 4) if r <= nrhs and r * cfg.Ls <= 48)
+            tuned["hop16 tile (lx, ly, lz, lt, warps)"] = ctx.mdwf_tune_get("hop16/%s/rows%d" % (lat, rows))
+        else:
+            tuned["hop%d zc" % inner] = ctx.mdwf_tune_get("hop%d/%s/rhs%d" % (inner, lat, nrhs))
+        tuned["hop64 zc"] = ctx.mdwf_tune_get("hop64/%s/rhs1" % lat)
+        tuned["seconds"] = time.time() - t0
     # the solver workspace comes from PyTorch's allocator (mdwf_set_workspace)
     ws = torch.empty(ctx.mdwf_workspace_bytes(nrhs, inner, packed=True) + (1 << 20), dtype=torch.uint8, device=dev)
     ctx.mdwf_set_workspace(ws)
@@ -357,7 +371,7 @@ def run_ours(args):
     dsl = {"inner_hop_GBps": roof["achieved"], "inner_hop_GFLOPs": roof["gflops"],
            "fp64_hop_GBps": h64[1] / h64[0] / 1e6 if h64[0] > 0 else None,
            "fp64_hop_GFLOPs": h64[2] / h64[0] / 1e6 if h64[0] > 0 else None, "fp64_hop_launches": h64[3]}
-    return dict(ctx=ctx, cfg=cfg, nrhs=nrhs, psi=psi, scratch=scratch, ws=ws, kw=kw, res=res, ms_step=ms_step,
+    return dict(tuned=tuned, ctx=ctx, cfg=cfg, nrhs=nrhs, psi=psi, scratch=scratch, ws=ws, kw=kw, res=res, ms_step=ms_step,
                 sec_per_rhs=sec_per_rhs, clocks=clocks, launches=launches, roof=roof, dsl=dsl, rank=rank, world=world, dev=dev,
                 hbm_peak=hbm_peak)
 
@@ -446,6 +460,7 @@ def main():
     ap.add_argument("--e2e-warmup", type=int, default=1)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-autotune", action="store_true", help="keep the library's default launch parameters")
     ap.add_argument("--no-dslash", action="store_true", help="skip the Dslash-only legs (bench lattice and config-2 sweep)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -492,7 +507,8 @@ def main():
             "cg": {"seconds_per_rhs_per_replica": st["sec_per_rhs"], "iters": res.iters, "reliable_updates": res.reliable_updates,
                    "true_resid": res.true_resid, "seconds_inner_last_step": res.seconds_inner, "seconds_last_step": res.seconds,
                    "kernel_launches_last_step": res.kernel_launches},
-            "dslash": dsl, "roofline": st["roof"], "gpu_launches": st["launches"], "clocks": st["clocks"]}
+            "dslash": dsl, "roofline": st["roof"], "gpu_launches": st["launches"], "clocks": st["clocks"],
+            "autotune": st["tuned"] or None}
     if e2e is not None:
         e2e["value"] = aggregate(e2e["value"], world)
         line["e2e"] = e2e

@@ -85,8 +85,11 @@ int autotune_impl(mdwf_ctx* c, int prec, int recon, int nrhs, cudaStream_t st) {
     MDWF_CUDA(c, cudaEventCreate(&S.e0));
     MDWF_CUDA(c, cudaEventCreate(&S.e1));
     const RhsList rl = all_rhs(nrhs);
-    const int reps = 3;
+    // repetitions per candidate: at least 3, and enough for ~20 ms per candidate on small lattices (first candidate's time)
+    int reps = 3;
     float best_ms = -1.f, ms = 0.f;
+    auto set_reps = [&](float one_ms) { if (one_ms > 0.f) reps = std::max(3, std::min(100, (int)(20.f / one_ms))); };
+    bool reps_set = false;
     std::vector<int> best;
 
     if (prec == 16) {
@@ -108,7 +111,9 @@ int autotune_impl(mdwf_ctx* c, int prec, int recon, int nrhs, cudaStream_t st) {
                 c->tile16_nw = nw;
                 tune_invalidate(c);
                 // a candidate that does not fit (shared memory) is refused by the launcher: skip it
-                if (time_hops(o, S, rl, 1, &ms) != MDWF_OK || time_hops(o, S, rl, reps, &ms) != MDWF_OK) { cudaGetLastError(); c->err.clear(); continue; }
+                if (time_hops(o, S, rl, 1, &ms) != MDWF_OK) { cudaGetLastError(); c->err.clear(); continue; }
+                if (!reps_set) { if (time_hops(o, S, rl, 1, &ms) == MDWF_OK) set_reps(ms); reps_set = true; }
+                if (time_hops(o, S, rl, reps, &ms) != MDWF_OK) { cudaGetLastError(); c->err.clear(); continue; }
                 if (best_ms < 0.f || ms < best_ms) { best_ms = ms; best = {t[0], t[1], t[2], t[3], nw}; }
             }
         for (int d = 0; d < 4; ++d) c->tile16_forced[d] = saved[d];
@@ -123,7 +128,9 @@ int autotune_impl(mdwf_ctx* c, int prec, int recon, int nrhs, cudaStream_t st) {
         for (int zc = tz; zc <= c->g.Z; zc += tz) {
             if (c->g.Z % zc || zc % c->ghop[1].tz || zc % c->ghop[2].tz) continue;
             set_zc(c, zc);
-            if ((rc = time_hops(o, S, rl, 1, &ms)) || (rc = time_hops(o, S, rl, reps, &ms))) { set_zc(c, saved); return rc; }
+            if ((rc = time_hops(o, S, rl, 1, &ms))) { set_zc(c, saved); return rc; }
+            if (!reps_set) { if ((rc = time_hops(o, S, rl, 1, &ms))) { set_zc(c, saved); return rc; } set_reps(ms); reps_set = true; }
+            if ((rc = time_hops(o, S, rl, reps, &ms))) { set_zc(c, saved); return rc; }
             if (best_ms < 0.f || ms < best_ms) { best_ms = ms; best = {zc}; }
         }
         set_zc(c, saved);

@@ -72,6 +72,7 @@ def main():
     ap.add_argument("--zc", type=int, default=0)
     ap.add_argument("--dagger", type=int, default=0)
     ap.add_argument("--tile", default="", help="fp16 stencil box and warps per block: lx,ly,lz,lt[,warps]")
+    ap.add_argument("--autotune", action="store_true", help="run mdwf_autotune for every format first and print what it chose")
     ap.add_argument("--meas", action="store_true", help="time the sequential-source and nucleon 2-pt kernels instead")
     a = ap.parse_args()
     cfg = synth.CONFIGS[a.config]
@@ -93,6 +94,13 @@ def main():
         ctx.mdwf_load_gauge(U, prec, recon)
     del U
     torch.cuda.empty_cache()
+    if a.autotune:
+        for prec, recon in fmts:
+            ctx.mdwf_autotune(prec, recon, a.nrhs)
+        tmp = "/tmp/mdwf_tune_%d.txt" % os.getpid()
+        ctx.mdwf_tune_save(tmp)
+        print(json.dumps({"autotune": [l.split() for l in open(tmp).read().splitlines() if l and l[0] != "#"]}), flush=True)
+        os.remove(tmp)
     Vh = cfg.V4 // 2
     g = torch.Generator(device="cuda").manual_seed(synth.seed_for(cfg.index, 2))
     for prec, recon in fmts:
