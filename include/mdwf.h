@@ -169,6 +169,22 @@ int mdwf_seq_source(mdwf_ctx* ctx, void* out4d, const void* prop4d, int ncol, co
 int mdwf_nucleon_2pt(mdwf_ctx* ctx, double* corr, const void* S_u1, const void* S_d, const void* S_u2,
                      const double* proj_host, int t0, void* stream);
 
+/* The same contraction (same arguments, same launch shape, same fixed-order sums, hence the same numbers) for callers that
+ * cannot allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The call makes
+ * no cudaMalloc / cudaMallocAsync / cudaFree and calls no allocating library routine: the per-warp partial sums that
+ * mdwf_nucleon_2pt takes from the stream-ordered allocator live in a file-scope `static __device__` array of
+ * mdwf_nucleon_2pt_noalloc_max_bytes() = 512 KiB, which every GPU that loads the library holds until the process exits.
+ * Limit: 16 * T * min(ceil(X*Y*Z / 4), max(1, 16 * SMs / T)) doubles must fit in it (on a 148-SM GPU every T <= 2368 with
+ * any spatial volume does, e.g. all BASELINE configs); beyond that the call returns MDWF_EINVAL with the sizes in
+ * mdwf_last_error and touches nothing.  The array is shared by every call on that GPU and keeps the last call's contents
+ * (the call clears the part it uses first): calls that overlap on the GPU -- two streams, or two contexts on one device
+ * -- race on it and must be serialised by the caller; calls on one stream are ordered and safe.  The first call on a
+ * device looks up the array's device address (cudaGetSymbolAddress, that device current) and raises the kernel's
+ * shared-memory limit; neither allocates device memory. */
+int mdwf_nucleon_2pt_noalloc(mdwf_ctx* ctx, double* corr, const void* S_u1, const void* S_d, const void* S_u2,
+                             const double* proj_host, int t0, void* stream);
+int64_t mdwf_nucleon_2pt_noalloc_max_bytes(void);
+
 /* 4D <-> 5D maps of SURVEY O3 as stand-alone calls (used by the tests; mdwf_solve applies them
  * itself for src_kind/out_kind = 1):  b5 = -D_- (P+ eta @ s=0 (+) P- eta @ s=Ls-1),
  * q = P- psi_0 + P+ psi_{Ls-1}.  Full-lattice canonical fp64 device fields. */

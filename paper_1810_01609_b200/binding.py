@@ -27,6 +27,7 @@ EXPORTS = [
     "mdwf_wall_project", "mdwf_launch_count", "mdwf_set_tiling", "mdwf_profile", "mdwf_profile_read", "mdwf_selftest_host", "mdwf_solve_packed",
     "mdwf_workspace_bytes", "mdwf_set_workspace", "mdwf_set_hop16_tile", "mdwf_field_pack_rhs", "mdwf_field_unpack_rhs",
     "mdwf_autotune", "mdwf_tune_save", "mdwf_tune_load", "mdwf_tune_get",
+    "mdwf_nucleon_2pt_noalloc", "mdwf_nucleon_2pt_noalloc_max_bytes",
 ]
 
 
@@ -83,6 +84,9 @@ def lib():
         L.mdwf_solve_host.argtypes = [vp, vp, vp, ci, ctypes.POINTER(SolveOpts), ctypes.POINTER(SolveInfo), vp]
         L.mdwf_seq_source.argtypes = [vp, vp, vp, ci, ctypes.POINTER(cd), ci, ci, vp]
         L.mdwf_nucleon_2pt.argtypes = [vp, vp, vp, vp, vp, ctypes.POINTER(cd), ci, vp]
+        L.mdwf_nucleon_2pt_noalloc.argtypes = [vp, vp, vp, vp, vp, ctypes.POINTER(cd), ci, vp]
+        L.mdwf_nucleon_2pt_noalloc_max_bytes.argtypes = []
+        L.mdwf_nucleon_2pt_noalloc_max_bytes.restype = ctypes.c_int64
         L.mdwf_wall_inject.argtypes = [vp, vp, vp, ci, ci, vp]
         L.mdwf_wall_project.argtypes = [vp, vp, vp, ci, vp]
         L.mdwf_launch_count.argtypes = [vp]
@@ -336,6 +340,16 @@ class Context:
             assert S.shape == (12, self.V4, 4, 3), S.shape
         self._chk(lib().mdwf_nucleon_2pt(self._h, _dev(corr), _dev(S_u1), _dev(S_d), _dev(S_u2), _mat32(proj), t0,
                                          _stream()))
+        return torch.view_as_complex(corr)
+
+    def mdwf_nucleon_2pt_noalloc(self, S_u1, S_d, S_u2, proj, corr, t0=0):
+        """mdwf_nucleon_2pt without any device allocation: the caller supplies corr (float64 [T][2], device) as well."""
+        T = self.dims[3]
+        assert corr.shape == (T, 2) and corr.dtype == torch.float64 and corr.is_cuda and corr.is_contiguous()
+        for S in (S_u1, S_d, S_u2):
+            assert S.shape == (12, self.V4, 4, 3), S.shape
+        self._chk(lib().mdwf_nucleon_2pt_noalloc(self._h, _dev(corr), _dev(S_u1), _dev(S_d), _dev(S_u2), _mat32(proj), t0,
+                                                 _stream()))
         return torch.view_as_complex(corr)
 
     def mdwf_wall_inject(self, eta4: torch.Tensor, recon=18):

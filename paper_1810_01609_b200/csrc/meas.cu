@@ -349,3 +349,87 @@ int mdwf_nucleon_2pt(mdwf_ctx* c, double* corr, const void* S_u1, const void* S_
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// mdwf_nucleon_2pt_noalloc: the same contraction for callers that must not allocate (CUDA graph capture, serving loops,
+// harnesses that forbid cudaMalloc).  mdwf_nucleon_2pt takes its per-warp partial sums from cudaMallocAsync; here they
+// live in a file-scope device array of fixed size that every GPU loading the library holds until exit.
+// In HOST code the array's name is only a host-side stand-in, never a device address: the address is asked for once per
+// device, with that device current, by cudaGetSymbolAddress, and that pointer is what the kernels get.
+// All calls share the array (it keeps the previous call's contents): calls that overlap on the GPU -- different
+// streams, or two contexts on one device -- race; serialise them.
+// ---------------------------------------------------------------------------------------------
+#define MDWF_NUC_SCRATCH_DOUBLES 65536        // 512 KiB: 2 x T x (blocks per timeslice) x MDWF_NUC_WARPS doubles must fit
+static __device__ __align__(256) double g_nuc_scratch[MDWF_NUC_SCRATCH_DOUBLES];
+
+#define MDWF_NUC_MAX_DEVICES 64
+static double* g_nuc_scratch_ptr[MDWF_NUC_MAX_DEVICES];      // device address of g_nuc_scratch on device d, nullptr = not set up
+
+// once per device, with that device current (MDWF_ENTER): the array's device address and the kernel's shared-memory limit
+static int nuc_noalloc_setup(mdwf_ctx* c, size_t nsm, double** ptr) {
+    const int dev = c->geo.device;
+    if (dev < 0 || dev >= MDWF_NUC_MAX_DEVICES) MDWF_FAIL(c, MDWF_EINVAL, "mdwf_nucleon_2pt_noalloc: device %d outside 0..%d", dev, MDWF_NUC_MAX_DEVICES - 1);
+    if (!g_nuc_scratch_ptr[dev]) {
+        double* p = nullptr;
+        MDWF_CUDA(c, cudaGetSymbolAddress((void**)&p, g_nuc_scratch));
+        if (!p) MDWF_FAIL(c, MDWF_ECUDA, "mdwf_nucleon_2pt_noalloc: cudaGetSymbolAddress returned a null address");
+        MDWF_CUDA(c, cudaFuncSetAttribute(nucleon_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nsm));
+        g_nuc_scratch_ptr[dev] = p;
+    }
+    *ptr = g_nuc_scratch_ptr[dev];
+    return MDWF_OK;
+}
+
+extern "C" {
+
+int64_t mdwf_nucleon_2pt_noalloc_max_bytes(void) { return (int64_t)sizeof(double) * MDWF_NUC_SCRATCH_DOUBLES; }
+
+int mdwf_nucleon_2pt_noalloc(mdwf_ctx* c, double* corr, const void* S_u1, const void* S_d, const void* S_u2,
+                             const double* proj_host, int t0, void* stream) {
+    MDWF_ENTER(c);
+    if (!corr || !S_u1 || !S_d || !S_u2 || !proj_host) MDWF_FAIL(c, MDWF_EINVAL, "null pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    NucArgs a;
+    a.Su1 = (const double2*)S_u1; a.Sd = (const double2*)S_d; a.Su2 = (const double2*)S_u2;
+    a.V4 = 2ll * c->g.Vh; a.V3 = a.V4 / c->g.T;
+    const int T = c->g.T;
+    const int gpb = MDWF_NUC_WARPS / MDWF_NUC_WPS;
+    // the launch shape of mdwf_nucleon_2pt, so that the fixed-order sums are the same sums
+    a.nblk_t = (int)std::min<long long>((a.V3 + gpb - 1) / gpb, std::max(1, (c->sm_count * 16) / T));
+    const int npart = a.nblk_t * MDWF_NUC_WARPS;
+    const long long need = 2ll * T * npart;
+    if (need > MDWF_NUC_SCRATCH_DOUBLES)
+        MDWF_FAIL(c, MDWF_EINVAL, "mdwf_nucleon_2pt_noalloc: T = %d with %d blocks per timeslice needs %lld bytes of scratch, the "
+                  "static array holds %lld (use mdwf_nucleon_2pt)", T, a.nblk_t, need * 8, (long long)sizeof(double) * MDWF_NUC_SCRATCH_DOUBLES);
+    // C = gamma_y gamma_t, G = C gamma5, Gt = gamma_t G^dag gamma_t in the DeGrand-Rossi basis (SURVEY 8 Notation)
+    const double gy[32] = {0,0, 0,0, 0,0, -1,0,   0,0, 0,0, 1,0, 0,0,   0,0, 1,0, 0,0, 0,0,   -1,0, 0,0, 0,0, 0,0};
+    const double gt[32] = {0,0, 0,0, 1,0, 0,0,   0,0, 0,0, 0,0, 1,0,   1,0, 0,0, 0,0, 0,0,   0,0, 1,0, 0,0, 0,0};
+    const double g5[32] = {1,0, 0,0, 0,0, 0,0,   0,0, 1,0, 0,0, 0,0,   0,0, 0,0, -1,0, 0,0,   0,0, 0,0, 0,0, -1,0};
+    double C[32], G[32], Gd[32], Gt[32];
+    mat4mul(gy, gt, C);
+    mat4mul(C, g5, G);
+    for (int i = 0; i < 4; ++i)
+        for (int j = 0; j < 4; ++j) { Gd[2 * (4 * i + j)] = G[2 * (4 * j + i)]; Gd[2 * (4 * i + j) + 1] = -G[2 * (4 * j + i) + 1]; }
+    mat4mul(gt, Gd, Gt);
+    mat4mul(Gt, gt, Gt);
+    memcpy(a.G, G, sizeof(G));
+    memcpy(a.Gt, Gt, sizeof(Gt));
+    memcpy(a.P, proj_host, sizeof(a.P));
+    const size_t nsm = (size_t)gpb * (5 * 144 + 16) * sizeof(double2);
+    double* scratch = nullptr;
+    int rc = nuc_noalloc_setup(c, nsm, &scratch);
+    if (rc) return rc;
+    a.partial = scratch;
+    // every slot the finish kernel reads is written by nucleon_kernel of this call; the clear only keeps a kernel that
+    // failed to launch from passing off the previous call's sums as its own
+    MDWF_CUDA(c, cudaMemsetAsync(scratch, 0, sizeof(double) * (size_t)need, st));
+    dim3 grid(a.nblk_t, T);
+    nucleon_kernel<<<grid, 32 * MDWF_NUC_WARPS, nsm, st>>>(a);
+    MDWF_CUDA(c, cudaGetLastError());
+    nucleon_finish_kernel<<<(T + 63) / 64, 64, 0, st>>>(corr, scratch, npart, T, t0);
+    MDWF_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    return MDWF_OK;
+}
+
+}  // extern "C"
