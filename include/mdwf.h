@@ -185,6 +185,21 @@ int mdwf_nucleon_2pt_noalloc(mdwf_ctx* ctx, double* corr, const void* S_u1, cons
                              const double* proj_host, int t0, void* stream);
 int64_t mdwf_nucleon_2pt_noalloc_max_bytes(void);
 
+/* Gauge-covariant Gaussian smearing of 4D spin-colour fields, for sources and sinks of the Feynman-Hellmann workload
+ * (PAPER.md:98-102 names smeared sources, no formula; R25):
+ *     out = (1 + width^2 / (4 n_iter) Lap)^n_iter in,
+ *     (Lap psi)(x) = sum_{j=x,y,z} [ U_j(x) psi(x+j) + U_j(x-j)^dag psi(x-j) - 2 psi(x) ]   (every timeslice on its own),
+ * hops that wrap multiplied by the geometry's bc_j.  in4d / out4d: ncol canonical 4D fields [col][x4][4][3][2] fp64
+ * (device); out4d must not alias in4d (EINVAL).  Needs the fp64 18-real links (mdwf_load_gauge(U, 64, 18); ESTATE
+ * otherwise).  n_iter = 0 copies; n_iter > 1 takes one temporary of the fields' size from the stream-ordered allocator
+ * for the duration of the call.  For a positive kernel keep 6 width^2 / (4 n_iter) < 1.  Stream-ordered, no host sync. */
+int mdwf_smear_gaussian(mdwf_ctx* ctx, void* out4d, const void* in4d, int ncol, double width, int n_iter, void* stream);
+
+/* Feynman-Hellmann effective derivative (Fig. 1; R25): with R(t) = C_FH(t) / C_2pt(t) (complex
+ * division), geff[t] = R(t+1) - R(t) for t = 0 .. T-2.  c2pt, cfh: device double [T][2] as written by mdwf_nucleon_2pt;
+ * geff: device double [T-1][2], overwritten. */
+int mdwf_fh_effective_derivative(mdwf_ctx* ctx, double* geff, const double* c2pt, const double* cfh, void* stream);
+
 /* 4D <-> 5D maps of SURVEY O3 as stand-alone calls (used by the tests; mdwf_solve applies them
  * itself for src_kind/out_kind = 1):  b5 = -D_- (P+ eta @ s=0 (+) P- eta @ s=Ls-1),
  * q = P- psi_0 + P+ psi_{Ls-1}.  Full-lattice canonical fp64 device fields. */

@@ -28,6 +28,7 @@ EXPORTS = [
     "mdwf_workspace_bytes", "mdwf_set_workspace", "mdwf_set_hop16_tile", "mdwf_field_pack_rhs", "mdwf_field_unpack_rhs",
     "mdwf_autotune", "mdwf_tune_save", "mdwf_tune_load", "mdwf_tune_get",
     "mdwf_nucleon_2pt_noalloc", "mdwf_nucleon_2pt_noalloc_max_bytes",
+    "mdwf_smear_gaussian", "mdwf_fh_effective_derivative",
 ]
 
 
@@ -86,6 +87,8 @@ def lib():
         L.mdwf_nucleon_2pt.argtypes = [vp, vp, vp, vp, vp, ctypes.POINTER(cd), ci, vp]
         L.mdwf_nucleon_2pt_noalloc.argtypes = [vp, vp, vp, vp, vp, ctypes.POINTER(cd), ci, vp]
         L.mdwf_nucleon_2pt_noalloc_max_bytes.argtypes = []
+        L.mdwf_smear_gaussian.argtypes = [vp, vp, vp, ci, cd, ci, vp]
+        L.mdwf_fh_effective_derivative.argtypes = [vp, vp, vp, vp, vp]
         L.mdwf_nucleon_2pt_noalloc_max_bytes.restype = ctypes.c_int64
         L.mdwf_wall_inject.argtypes = [vp, vp, vp, ci, ci, vp]
         L.mdwf_wall_project.argtypes = [vp, vp, vp, ci, vp]
@@ -351,6 +354,22 @@ class Context:
         self._chk(lib().mdwf_nucleon_2pt_noalloc(self._h, _dev(corr), _dev(S_u1), _dev(S_d), _dev(S_u2), _mat32(proj), t0,
                                                  _stream()))
         return torch.view_as_complex(corr)
+
+    def mdwf_smear_gaussian(self, psi4: torch.Tensor, width, n_iter, out=None):
+        ncol = psi4.shape[0]
+        assert psi4.shape == (ncol, self.V4, 4, 3) and psi4.dtype == torch.complex128 and psi4.is_contiguous()
+        if out is None:
+            out = torch.empty_like(psi4)
+        self._chk(lib().mdwf_smear_gaussian(self._h, _dev(out), _dev(psi4), ncol, float(width), int(n_iter), _stream()))
+        return out
+
+    def mdwf_fh_effective_derivative(self, c2pt: torch.Tensor, cfh: torch.Tensor):
+        T = self.dims[3]
+        c2, cf = torch.view_as_real(c2pt.contiguous()), torch.view_as_real(cfh.contiguous())
+        assert c2.shape == (T, 2) and cf.shape == (T, 2) and c2.dtype == torch.float64 and cf.dtype == torch.float64
+        geff = torch.empty((T - 1, 2), dtype=torch.float64, device=c2pt.device)
+        self._chk(lib().mdwf_fh_effective_derivative(self._h, _dev(geff), _dev(c2), _dev(cf), _stream()))
+        return torch.view_as_complex(geff)
 
     def mdwf_wall_inject(self, eta4: torch.Tensor, recon=18):
         ncol = eta4.shape[0]

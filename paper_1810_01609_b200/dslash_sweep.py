@@ -55,6 +55,16 @@ def measurement_kernels(ctx, cfg, iters, peak):
     ms = timed(lambda: ctx.mdwf_seq_source(props[0], G, out=out))
     print(json.dumps({"workload": cfg.name, "op": "seq_source", "ms": round(ms, 4), "GBps": round(2 * pbytes / ms / 1e6, 1),
                       "frac_of_measured_hbm": round(2 * pbytes / ms / 1e6 / peak, 4)}), flush=True)
+    # gauge-covariant Gaussian smearing (NEXT-3): needs links; one step reads and writes the propagator and reads 3 x 144 B
+    # of links per site
+    U = synth.gauge_field(cfg.dims, cfg.eps, synth.seed_for(cfg.index, 1), device="cuda")
+    ctx.mdwf_load_gauge(U, 64, 18)
+    del U
+    n_smear = 30
+    ms = timed(lambda: ctx.mdwf_smear_gaussian(props[0], 3.0, n_smear, out=out))
+    sbytes = n_smear * (2 * pbytes + 3 * 144 * cfg.V4)
+    print(json.dumps({"workload": cfg.name, "op": "smear_gaussian", "steps": n_smear, "ms": round(ms, 4), "ms_per_step": round(ms / n_smear, 4),
+                      "GBps": round(sbytes / ms / 1e6, 1), "frac_of_measured_hbm": round(sbytes / ms / 1e6 / peak, 4)}), flush=True)
     ms = timed(lambda: ctx.mdwf_nucleon_2pt(props[0], props[1], props[2], P))
     print(json.dumps({"workload": cfg.name, "op": "nucleon_2pt", "ms": round(ms, 4), "GBps": round(3 * pbytes / ms / 1e6, 1),
                       "GFLOPs": round(2.0e4 * cfg.V4 / ms / 1e6, 1),
