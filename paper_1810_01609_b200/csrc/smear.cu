@@ -7,9 +7,9 @@
 // mdwf_seq_source / mdwf_nucleon_2pt); links are the loaded fp64 18-real format.
 //
 // One step = one launch.  A block owns NS consecutive 4D sites: phase 0 parks their 6 spatial links in shared memory as
-// the 3x3 matrices the step multiplies (backward legs daggered, boundary sign folded) together with the 6 neighbour
-// indices; phase 1 runs over the (site, column) pairs -- a warp = 32 consecutive sites of one column, i.e. 6 KB of
-// contiguous reads per leg -- so the links are read from HBM once per step and shared by all columns (the same idea as
+// the 3x3 matrices the step multiplies (backward legs daggered, boundary sign and the step size folded) together with the 6 neighbour
+// indices; phase 1 runs over (column, site, spin) items -- a lane owns one colour 3-vector (48 contiguous bytes), a warp 8
+// consecutive sites of one column, all 6 neighbour vectors in flight at once -- so the links are read from HBM once per step and shared by all columns (the same idea as
 // the link staging of the Dslash stencil, north_star).  Algorithmic bytes per step: 2 x 192 B per site and column plus
 // 3 x 144 B of links per site; HBM-bound.
 #include "mdwf_host.h"
@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(MDWF_SMEAR_THREADS) smear_step_kernel(const Ge
         double U[18];
         if (!bwd) load_link<double, 18>(a.g.v[par], j, (int)(x4 >> 1), g.Vh, U);
         else load_link<double, 18>(a.g.v[1 - par], j, (int)(xn >> 1), g.Vh, U);
-        const double sg = wrap ? (double)(j == 0 ? g.bc[0] : j == 1 ? g.bc[1] : g.bc[2]) : 1.0;
+        const double sg = a.a * (wrap ? (double)(j == 0 ? g.bc[0] : j == 1 ? g.bc[1] : g.bc[2]) : 1.0);   // a = sigma^2/(4N) folded in
 #pragma unroll
         for (int r = 0; r < 3; ++r)
 #pragma unroll
@@ -65,49 +65,43 @@ __global__ void __launch_bounds__(MDWF_SMEAR_THREADS) smear_step_kernel(const Ge
             }
     }
     __syncthreads();
-    // ---- phase 1: (site, column) pairs ------------------------------------------------------------------------
+    // ---- phase 1: (column, site, spin) items: a lane owns one colour 3-vector, 4 lanes a site, a warp 8 consecutive sites -------
     const double diag = 1.0 - 6.0 * a.a;
-    for (int it = threadIdx.x; it < MDWF_SMEAR_NS * a.ncol; it += blockDim.x) {
-        const int col = it / MDWF_SMEAR_NS, s = it - col * MDWF_SMEAR_NS;
+    for (int it = threadIdx.x; it < MDWF_SMEAR_NS * 4 * a.ncol; it += blockDim.x) {
+        const int col = it / (MDWF_SMEAR_NS * 4), rem = it - col * (MDWF_SMEAR_NS * 4), s = rem >> 2, sp = rem & 3;
         const long long x4 = x0 + s;
         if (x4 >= a.V4) continue;
-        const double2* base = a.in + (long long)col * a.V4 * 12;
-        double2 acc[12];
+        const double2* base = a.in + (long long)col * a.V4 * 12 + 3 * sp;
+        double2 acc[3];
         {
             const double2* p = base + x4 * 12;
 #pragma unroll
-            for (int i = 0; i < 12; ++i) {
-                const double2 v = __ldg(p + i);
-                acc[i] = make_double2(diag * v.x, diag * v.y);
+            for (int c = 0; c < 3; ++c) {
+                const double2 v = __ldg(p + c);
+                acc[c] = make_double2(diag * v.x, diag * v.y);
             }
         }
-#pragma unroll 1
+        double2 v[6][3];
+#pragma unroll
         for (int l = 0; l < 6; ++l) {
             const double2* p = base + (long long)s_nb[s][l] * 12;
-            double2 v[12];
 #pragma unroll
-            for (int i = 0; i < 12; ++i) v[i] = __ldg(p + i);
+            for (int c = 0; c < 3; ++c) v[l][c] = __ldg(p + c);
+        }
 #pragma unroll
-            for (int r = 0; r < 3; ++r) {
-                double2 m[3];
+        for (int l = 0; l < 6; ++l)
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    const double2 t = s_link[s][l][r * 3 + c];
-                    m[c] = make_double2(a.a * t.x, a.a * t.y);
+                    const double2 m = s_link[s][l][r * 3 + c];
+                    const double2 w = v[l][c];
+                    acc[r].x = fma(m.x, w.x, fma(-m.y, w.y, acc[r].x));
+                    acc[r].y = fma(m.x, w.y, fma(m.y, w.x, acc[r].y));
                 }
+        double2* o = a.out + ((long long)col * a.V4 + x4) * 12 + 3 * sp;
 #pragma unroll
-                for (int sp = 0; sp < 4; ++sp)
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) {
-                        const double2 w = v[3 * sp + c];
-                        acc[3 * sp + r].x += m[c].x * w.x - m[c].y * w.y;
-                        acc[3 * sp + r].y += m[c].x * w.y + m[c].y * w.x;
-                    }
-            }
-        }
-        double2* o = a.out + ((long long)col * a.V4 + x4) * 12;
-#pragma unroll
-        for (int i = 0; i < 12; ++i) o[i] = acc[i];
+        for (int c = 0; c < 3; ++c) o[c] = acc[c];
     }
 }
 
