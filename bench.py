@@ -294,7 +294,7 @@ def run_ours(args):
         ctx.mdwf_autotune(64, 18, 1)
         lat = "%dx%dx%dx%d/Ls%d" % (tuple(cfg.dims) + (cfg.Ls,))
         if inner == 16:
-            rows = cfg.Ls * max(r for r in (1, 2, 4) if r <= nrhs and r * cfg.Ls <= 48)
+            rows = cfg.Ls * max(r for r in (1, 2, 4) if r < 2 * nrhs and r * cfg.Ls <= 48)     # rhs per interleave group
             tuned["hop16 tile (lx, ly, lz, lt, warps)"] = ctx.mdwf_tune_get("hop16/%s/rows%d" % (lat, rows))
         else:
             tuned["hop%d zc" % inner] = ctx.mdwf_tune_get("hop%d/%s/rhs%d" % (inner, lat, nrhs))

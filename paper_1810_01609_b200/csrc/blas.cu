@@ -4,11 +4,13 @@
 
 namespace mdwf {
 
-// fp16: rhs interleave of a field with nrhs columns (log2): groups of 4 when there are at least 4, else 2, else 1
-// (the RI * Ls rows of a site are at most 48 = three m16 tiles of the tensor-core stencil)
+// fp16: rhs interleave of a field with nrhs columns (log2): groups of RI = 4 when there are at least 3 rhs, of 2 for two,
+// else 1, as far as the RI * Ls rows of a site stay within 48 = three m16 tiles of the tensor-core stencil.  Three rhs
+// take a group of 4 with one padding slot: the stencil's cost per group grows much more slowly than its rows (measured at
+// 48^3x64x10: 3.8 / 6.3 / 9.4 ms for groups of 1 / 2 / 4), so one padded group beats two groups of 2.
 int half_ril(int nrhs, int Ls) {
     for (int ril = 2; ril > 0; --ril)
-        if ((1 << ril) <= nrhs && (Ls << ril) <= 48) return ril;
+        if ((1 << ril) < 2 * nrhs && (Ls << ril) <= 48) return ril;
     return 0;
 }
 int half_site_bytes(int nrhs, int Ls) { return (((Ls << half_ril(nrhs, Ls)) + 7) / 8) * 384; }
