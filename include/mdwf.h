@@ -174,7 +174,7 @@ int mdwf_nucleon_2pt(mdwf_ctx* ctx, double* corr, const void* S_u1, const void* 
  * no cudaMalloc / cudaMallocAsync / cudaFree and calls no allocating library routine: the per-warp partial sums that
  * mdwf_nucleon_2pt takes from the stream-ordered allocator live in a file-scope `static __device__` array of
  * mdwf_nucleon_2pt_noalloc_max_bytes() = 512 KiB, which every GPU that loads the library holds until the process exits.
- * Limit: 16 * T * min(ceil(X*Y*Z / 4), max(1, 16 * SMs / T)) doubles must fit in it (on a 148-SM GPU every T <= 2368 with
+ * Limit: 10 * T * min(ceil(X*Y*Z / 4), max(1, 16 * SMs / T)) doubles must fit in it (on a 148-SM GPU every T <= 2368 with
  * any spatial volume does, e.g. all BASELINE configs); beyond that the call returns MDWF_EINVAL with the sizes in
  * mdwf_last_error and touches nothing.  The array is shared by every call on that GPU and keeps the last call's contents
  * (the call clears the part it uses first): calls that overlap on the GPU -- two streams, or two contexts on one device

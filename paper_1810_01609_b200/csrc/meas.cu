@@ -108,13 +108,16 @@ __global__ void __launch_bounds__(256) seq_source_kernel(const SeqArgs a) {
 // Nucleon 2-pt (SURVEY O4 C-def), in the trace form
 //   C(t) = sum_x eps_{abc} eps_{a'b'c'} { tr[Q^{bb'} (Su1^{aa'})^T] tr[P Su2^{cc'}] - tr[(Q^{bb'})^T Su1^{ac'} P Su2^{ca'}] },
 //   Q^{bb'} = G Sd^{bb'} Gt,  G = C gamma5,  Gt = gamma_t G^dag gamma_t,  S^{ab}_{al be}(x) = S[3 be + b][x][al][a].
-// One warp per site; the 144 work items (colour-permutation pair e1,e2 ; spin index al') are spread over the lanes.
 struct NucArgs {
     const double2 *Su1, *Sd, *Su2;
     double* partial;       // [T][nblk_t][2]
     long long V4, V3;
     int nblk_t;            // blocks per timeslice
     double G[32], Gt[32], P[32];
+    // G = C gamma5 and Gt = gamma_t G^dag gamma_t are signed permutation matrices (one non-zero per row and column; checked
+    // on the host): Q_{al al'} = sum G[al][be] Sd_{be be'} Gt[be'][al'] = qc[al][al'] Sd_{gb[al] gtb[al']}
+    int gb[4], gtb[4];
+    double qc[32];         // qc[al][al'] = G[al][gb[al]] * Gt[gtb[al']][al'], complex
 };
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 __device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
@@ -122,94 +125,117 @@ __device__ __forceinline__ double2 cfma(double2 a, double2 b, double2 c) {
     return make_double2(c.x + a.x * b.x - a.y * b.y, c.y + a.x * b.y + a.y * b.x);
 }
 
-#define MDWF_NUC_WARPS 8      // warps per block
-#define MDWF_NUC_WPS 2        // warps per site (they meet at a named barrier)
+#define MDWF_NUC_SPB 4        // sites per block and pass
+#define MDWF_NUC_WARPS 5      // warps per block: 36 lanes per site (one per pair of colour permutations) = 144 of the 160 threads
+#define MDWF_NUC_BLK 17       // stride of a 4x4 spin block in shared memory (double2): 8 consecutive blocks cover all banks once
+#define MDWF_NUC_SITE (5 * 9 * MDWF_NUC_BLK)                 // per site: Su1, Sd, Su2, Q, W as 9 colour-pair blocks each
+#define MDWF_NUC_SMEM ((MDWF_NUC_SPB * MDWF_NUC_SITE + 32) * sizeof(double2))   // + qc, P
 __constant__ int c_perm[6][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}, {0, 2, 1}, {2, 1, 0}, {1, 0, 2}};
 __constant__ double c_psign[6] = {1, 1, 1, -1, -1, -1};
-__global__ void __launch_bounds__(32 * MDWF_NUC_WARPS) nucleon_kernel(const NucArgs a) {
-    // MDWF_NUC_WPS warps per site (named barriers only); 144 work items per phase are spread over their lanes.
-    // prop element (sink spin al, sink colour ca, source spin be, source colour cb) at S[(3*be+cb)*12 + 3*al+ca]
+// A block handles MDWF_NUC_SPB sites per pass in three phases separated by block barriers (three blocks per SM overlap
+// each other's phases):
+//  1. the three propagators of the sites -> shared memory as 4x4 spin blocks per colour pair,
+//     B^{xy}[al*4 + be] = S^{xy}_{al be} = S[col 3 be + y][site][3 al + x]   (x sink colour, y source colour);
+//  2. Q^{bb'} = G Sd^{bb'} Gt and W^{ca'} = P Su2^{ca'} for the 9 colour pairs (tr[P Su2^{cc'}] is the trace of W^{cc'});
+//  3. one lane per (site, e1, e2), e1 = (a b c), e2 = (a' b' c') colour permutations: W^{ca'} stays in registers while the
+//     rows of Q^{bb'}, Su1^{ac'} and Su1^{aa'} stream through: 96 complex multiply-adds for 68 16-byte loads.
+__global__ void __launch_bounds__(32 * MDWF_NUC_WARPS, 3) nucleon_kernel(const NucArgs a) {
     extern __shared__ __align__(16) unsigned char nuc_smem[];
-    constexpr int GT = 32 * MDWF_NUC_WPS;                     // threads per site group
-    const int grp = threadIdx.x / GT, lane = threadIdx.x % GT;
-    double2* base = reinterpret_cast<double2*>(nuc_smem) + grp * (5 * 144 + 16);
-#define NUC_SYNC() asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "r"(GT) : "memory")
-    double2 *s1 = base, *sd = base + 144, *s2 = base + 288, *Q = base + 432, *W = base + 576, *trP = base + 720;
+    double2* sm = reinterpret_cast<double2*>(nuc_smem);
+    double2* sC = sm + MDWF_NUC_SPB * MDWF_NUC_SITE;          // qc[16], P[16]
+    const int tid = threadIdx.x, NT = 32 * MDWF_NUC_WARPS;
+    int gb_me = 0, gtb_me = 0;                                // phase 2: this thread's element is (al, al') = ((tid >> 2) & 3, tid & 3)
+    if (tid < 32) {
+        const double* src = tid < 16 ? a.qc : a.P;
+        const int k = tid & 15;
+        double re = 0.0, im = 0.0;
+#pragma unroll
+        for (int q = 0; q < 16; ++q)
+            if (q == k) { re = src[2 * q]; im = src[2 * q + 1]; }      // (no dynamic indexing of the kernel parameters)
+        sC[tid] = make_double2(re, im);
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        if (q == ((tid >> 2) & 3)) gb_me = a.gb[q];
+        if (q == (tid & 3)) gtb_me = a.gtb[q];
+    }
     const int t = blockIdx.y;
     double accr = 0.0, acci = 0.0;
-    constexpr int GPB = MDWF_NUC_WARPS / MDWF_NUC_WPS;         // site groups per block
-    const int gid = blockIdx.x * GPB + grp, ng = a.nblk_t * GPB;
-    for (long long xs = gid; xs < a.V3; xs += ng) {
-        const long long x = (long long)t * a.V3 + xs;
-        for (int i = lane; i < 144; i += GT) {
-            const int col = i / 12, k = i - col * 12;
-            const long long off = ((long long)col * a.V4 + x) * 12 + k;
-            s1[i] = __ldg(a.Su1 + off);
-            sd[i] = __ldg(a.Sd + off);
-            s2[i] = __ldg(a.Su2 + off);
+    const int my_site = tid / 36, item = tid - 36 * my_site, e1 = (item / 6) % 6, e2 = item % 6;
+    const int ca = c_perm[e1][0], cb = c_perm[e1][1], cc = c_perm[e1][2];
+    const int cap = c_perm[e2][0], cbp = c_perm[e2][1], ccp = c_perm[e2][2];
+    const double sg = c_psign[e1] * c_psign[e2];
+    constexpr int NEL = 3 * 12 * MDWF_NUC_SPB * 12;            // propagator elements per pass
+    constexpr int NLD = (NEL + 32 * MDWF_NUC_WARPS - 1) / (32 * MDWF_NUC_WARPS);
+    for (long long xs0 = (long long)blockIdx.x * MDWF_NUC_SPB; xs0 < a.V3; xs0 += (long long)a.nblk_t * MDWF_NUC_SPB) {
+        const int nsite = (int)min((long long)MDWF_NUC_SPB, a.V3 - xs0);
+        const long long x0 = (long long)t * a.V3 + xs0;
+        // ---- phase 1: element i -> (prop, col, site, k): runs of SPB * 192 contiguous bytes per (prop, col); all loads of a
+        // thread are issued before the first store
+        double2 v[NLD];
+#pragma unroll
+        for (int n = 0; n < NLD; ++n) {
+            const int i = tid + NT * n;
+            const int k = i % 12, r = i / 12, site = r % MDWF_NUC_SPB, pc = r / MDWF_NUC_SPB, col = pc % 12, prop = pc / 12;
+            const double2* src = prop == 0 ? a.Su1 : prop == 1 ? a.Sd : a.Su2;
+            v[n] = (i < NEL && site < nsite) ? __ldg(src + ((long long)col * a.V4 + x0 + site) * 12 + k) : make_double2(0.0, 0.0);
         }
-        NUC_SYNC();
-        for (int e = lane; e < 144; e += GT) {
-            // e -> (b, b', al, al'):  Q^{bb'}_{al al'} = sum_{be,be'} G[al][be] Sd^{bb'}_{be be'} Gt[be'][al']
-            const int b = e / 48, bp = (e / 16) % 3, al = (e / 4) % 4, alp = e % 4;
-            double2 q = make_double2(0.0, 0.0);
+        __syncthreads();                                       // the previous pass is through with the blocks
 #pragma unroll
-            for (int be = 0; be < 4; ++be) {
-                const double2 g1 = make_double2(a.G[2 * (4 * al + be)], a.G[2 * (4 * al + be) + 1]);
-                if (g1.x == 0.0 && g1.y == 0.0) continue;
+        for (int n = 0; n < NLD; ++n) {
+            const int i = tid + NT * n;
+            const int k = i % 12, r = i / 12, site = r % MDWF_NUC_SPB, pc = r / MDWF_NUC_SPB, col = pc % 12, prop = pc / 12;
+            const int be = col / 3, y = col - 3 * be, al = k / 3, x = k - 3 * al;
+            if (i < NEL) sm[site * MDWF_NUC_SITE + (prop * 9 + x * 3 + y) * MDWF_NUC_BLK + al * 4 + be] = v[n];
+        }
+        __syncthreads();
+        // ---- phase 2: Q (array 3) and W (array 4): element j -> (site, Q|W, colour pair, al, al'), (al, al') = j & 15 is the
+        // same for every element of a thread (NT is a multiple of 16)
+        for (int j = tid; j < MDWF_NUC_SPB * 288; j += NT) {
+            const int site = j / 288, e = j - 288 * site, isW = e >= 144, blk = (e - 144 * isW) >> 4, al = (j >> 2) & 3, alp = j & 3;
+            double2* S = sm + site * MDWF_NUC_SITE;
+            if (!isW) {
+                S[(27 + blk) * MDWF_NUC_BLK + al * 4 + alp] = cmul(sC[al * 4 + alp], S[(9 + blk) * MDWF_NUC_BLK + gb_me * 4 + gtb_me]);
+            } else {
+                const double2* B = S + (18 + blk) * MDWF_NUC_BLK;                   // Su2^{ca'}
+                double2 r = make_double2(0.0, 0.0);
 #pragma unroll
-                for (int bep = 0; bep < 4; ++bep) {
-                    const double2 g2 = make_double2(a.Gt[2 * (4 * bep + alp)], a.Gt[2 * (4 * bep + alp) + 1]);
-                    if (g2.x == 0.0 && g2.y == 0.0) continue;
-                    q = cfma(cmul(g1, g2), sd[(3 * bep + bp) * 12 + 3 * be + b], q);
-                }
+                for (int ga = 0; ga < 4; ++ga) r = cfma(sC[16 + al * 4 + ga], B[ga * 4 + alp], r);
+                S[(36 + blk) * MDWF_NUC_BLK + al * 4 + alp] = r;
             }
-            Q[e] = q;     // index ((b*3+bp)*4+al)*4+alp
-            // W^{c a'}_{ga' al'} = sum_ga P[ga'][ga] Su2^{c a'}_{ga al'}   (same index pattern: c, a', ga', al')
-            double2 w = make_double2(0.0, 0.0);
-#pragma unroll
-            for (int ga = 0; ga < 4; ++ga) {
-                const double2 pp = make_double2(a.P[2 * (4 * al + ga)], a.P[2 * (4 * al + ga) + 1]);
-                if (pp.x == 0.0 && pp.y == 0.0) continue;
-                w = cfma(pp, s2[(3 * alp + bp) * 12 + 3 * ga + b], w);
-            }
-            W[e] = w;     // index ((c*3+a')*4+ga')*4+al'
         }
-        if (lane < 9) {
-            const int c = lane / 3, cp = lane % 3;
-            double2 tr = make_double2(0.0, 0.0);
-            for (int gap = 0; gap < 4; ++gap)
-                for (int ga = 0; ga < 4; ++ga)
-                    tr = cfma(make_double2(a.P[2 * (4 * gap + ga)], a.P[2 * (4 * gap + ga) + 1]),
-                              s2[(3 * gap + cp) * 12 + 3 * ga + c], tr);
-            trP[lane] = tr;
-        }
-        NUC_SYNC();
-        for (int wi = lane; wi < 144; wi += GT) {
-            const int e = wi / 4, alp = wi % 4, e1 = e / 6, e2 = e % 6;
-            const int ca = c_perm[e1][0], cb = c_perm[e1][1], cc = c_perm[e1][2];
-            const int cap = c_perm[e2][0], cbp = c_perm[e2][1], ccp = c_perm[e2][2];
-            const double sg = c_psign[e1] * c_psign[e2];
-            const double2* q = Q + (cb * 3 + cbp) * 16;
-            // direct: sum_al Q_{al al'} Su1^{aa'}_{al al'}  * tr[P Su2^{cc'}]
-            double2 d = make_double2(0.0, 0.0);
+        __syncthreads();
+        // ---- phase 3
+        if (my_site < nsite) {
+            const double2* S = sm + my_site * MDWF_NUC_SITE;
+            const double2* Wb = S + (36 + cc * 3 + cap) * MDWF_NUC_BLK;
+            const double2* Wt = S + (36 + cc * 3 + ccp) * MDWF_NUC_BLK;
+            const double2* Qb = S + (27 + cb * 3 + cbp) * MDWF_NUC_BLK;
+            const double2* Sx = S + (ca * 3 + ccp) * MDWF_NUC_BLK;                  // Su1^{ac'}
+            const double2* Sdr = S + (ca * 3 + cap) * MDWF_NUC_BLK;                 // Su1^{aa'}
+            double2 w[16];
 #pragma unroll
-            for (int al = 0; al < 4; ++al) d = cfma(q[al * 4 + alp], s1[(3 * alp + cap) * 12 + 3 * al + ca], d);
-            d = cmul(d, trP[cc * 3 + ccp]);
-            // exchange: sum_{al, ga'} Q_{al al'} Su1^{ac'}_{al ga'} W^{ca'}_{ga' al'}
-            const double2* w = W + (cc * 3 + cap) * 16;
-            double2 ex = make_double2(0.0, 0.0);
+            for (int i = 0; i < 16; ++i) w[i] = Wb[i];
+            const double2 trp = cadd(cadd(Wt[0], Wt[5]), cadd(Wt[10], Wt[15]));
+            double2 d = make_double2(0.0, 0.0), ex = make_double2(0.0, 0.0);
 #pragma unroll
             for (int al = 0; al < 4; ++al) {
-                double2 u = make_double2(0.0, 0.0);
+                double2 q[4], sx[4], sd[4];
 #pragma unroll
-                for (int gap = 0; gap < 4; ++gap) u = cfma(s1[(3 * gap + ccp) * 12 + 3 * al + ca], w[gap * 4 + alp], u);
-                ex = cfma(q[al * 4 + alp], u, ex);
+                for (int i = 0; i < 4; ++i) { q[i] = Qb[al * 4 + i]; sx[i] = Sx[al * 4 + i]; sd[i] = Sdr[al * 4 + i]; }
+#pragma unroll
+                for (int alp = 0; alp < 4; ++alp) {
+                    double2 u = make_double2(0.0, 0.0);
+#pragma unroll
+                    for (int gap = 0; gap < 4; ++gap) u = cfma(sx[gap], w[gap * 4 + alp], u);
+                    ex = cfma(q[alp], u, ex);
+                    d = cfma(q[alp], sd[alp], d);
+                }
             }
+            d = cmul(d, trp);
             accr += sg * (d.x - ex.x);
             acci += sg * (d.y - ex.y);
         }
-        NUC_SYNC();
     }
     // fixed-order warp sum, one partial per warp
 #pragma unroll
@@ -222,7 +248,6 @@ __global__ void __launch_bounds__(32 * MDWF_NUC_WARPS) nucleon_kernel(const NucA
         a.partial[((long long)t * nw + wid) * 2] = accr;
         a.partial[((long long)t * nw + wid) * 2 + 1] = acci;
     }
-#undef NUC_SYNC
 }
 
 __global__ void nucleon_finish_kernel(double* corr, const double* partial, int nblk_t, int T, int t0) {
@@ -250,6 +275,41 @@ static void mat4mul(const double* A, const double* B, double* C) {   // complex 
         }
     memcpy(C, T, sizeof(T));
 }
+
+// C = gamma_y gamma_t, G = C gamma5, Gt = gamma_t G^dag gamma_t in the DeGrand-Rossi basis (SURVEY 8 Notation), the projector,
+// and the signed-permutation form of G and Gt that the kernel's phase 2 uses
+static int nuc_fill_args(mdwf_ctx* c, NucArgs& a, const double* proj_host) {
+    const double gy[32] = {0,0, 0,0, 0,0, -1,0,   0,0, 0,0, 1,0, 0,0,   0,0, 1,0, 0,0, 0,0,   -1,0, 0,0, 0,0, 0,0};
+    const double gt[32] = {0,0, 0,0, 1,0, 0,0,   0,0, 0,0, 0,0, 1,0,   1,0, 0,0, 0,0, 0,0,   0,0, 1,0, 0,0, 0,0};
+    const double g5[32] = {1,0, 0,0, 0,0, 0,0,   0,0, 1,0, 0,0, 0,0,   0,0, 0,0, -1,0, 0,0,   0,0, 0,0, 0,0, -1,0};
+    double C[32], G[32], Gd[32], Gt[32];
+    mat4mul(gy, gt, C);
+    mat4mul(C, g5, G);
+    for (int i = 0; i < 4; ++i)
+        for (int j = 0; j < 4; ++j) { Gd[2 * (4 * i + j)] = G[2 * (4 * j + i)]; Gd[2 * (4 * i + j) + 1] = -G[2 * (4 * j + i) + 1]; }
+    mat4mul(gt, Gd, Gt);
+    mat4mul(Gt, gt, Gt);
+    memcpy(a.G, G, sizeof(G));
+    memcpy(a.Gt, Gt, sizeof(Gt));
+    memcpy(a.P, proj_host, sizeof(a.P));
+    for (int i = 0; i < 4; ++i) {
+        int nr = 0, ncol = 0;
+        for (int j = 0; j < 4; ++j) {
+            if (G[2 * (4 * i + j)] != 0.0 || G[2 * (4 * i + j) + 1] != 0.0) { a.gb[i] = j; ++nr; }          // row i of G
+            if (Gt[2 * (4 * j + i)] != 0.0 || Gt[2 * (4 * j + i) + 1] != 0.0) { a.gtb[i] = j; ++ncol; }     // column i of Gt
+        }
+        if (nr != 1 || ncol != 1) MDWF_FAIL(c, MDWF_ECUDA, "internal: C gamma5 is not a signed permutation in this basis");
+    }
+    for (int al = 0; al < 4; ++al)
+        for (int alp = 0; alp < 4; ++alp) {
+            const double gr = G[2 * (4 * al + a.gb[al])], gi = G[2 * (4 * al + a.gb[al]) + 1];
+            const double hr = Gt[2 * (4 * a.gtb[alp] + alp)], hi = Gt[2 * (4 * a.gtb[alp] + alp) + 1];
+            a.qc[2 * (4 * al + alp)] = gr * hr - gi * hi;
+            a.qc[2 * (4 * al + alp) + 1] = gr * hi + gi * hr;
+        }
+    return MDWF_OK;
+}
+
 
 }  // namespace mdwf
 
@@ -313,28 +373,15 @@ int mdwf_nucleon_2pt(mdwf_ctx* c, double* corr, const void* S_u1, const void* S_
     a.Su1 = (const double2*)S_u1; a.Sd = (const double2*)S_d; a.Su2 = (const double2*)S_u2;
     a.V4 = 2ll * c->g.Vh; a.V3 = a.V4 / c->g.T;
     const int T = c->g.T;
-    const int gpb = MDWF_NUC_WARPS / MDWF_NUC_WPS;
+    const int gpb = MDWF_NUC_SPB;
     a.nblk_t = (int)std::min<long long>((a.V3 + gpb - 1) / gpb, std::max(1, (c->sm_count * 16) / T));
-    // C = gamma_y gamma_t, G = C gamma5, Gt = gamma_t G^dag gamma_t in the DeGrand-Rossi basis (SURVEY 8 Notation)
-    const double gy[32] = {0,0, 0,0, 0,0, -1,0,   0,0, 0,0, 1,0, 0,0,   0,0, 1,0, 0,0, 0,0,   -1,0, 0,0, 0,0, 0,0};
-    const double gt[32] = {0,0, 0,0, 1,0, 0,0,   0,0, 0,0, 0,0, 1,0,   1,0, 0,0, 0,0, 0,0,   0,0, 1,0, 0,0, 0,0};
-    const double g5[32] = {1,0, 0,0, 0,0, 0,0,   0,0, 1,0, 0,0, 0,0,   0,0, 0,0, -1,0, 0,0,   0,0, 0,0, 0,0, -1,0};
-    double C[32], G[32], Gd[32], Gt[32];
-    mat4mul(gy, gt, C);
-    mat4mul(C, g5, G);
-    for (int i = 0; i < 4; ++i)
-        for (int j = 0; j < 4; ++j) { Gd[2 * (4 * i + j)] = G[2 * (4 * j + i)]; Gd[2 * (4 * i + j) + 1] = -G[2 * (4 * j + i) + 1]; }
-    mat4mul(gt, Gd, Gt);
-    mat4mul(Gt, gt, Gt);
-    memcpy(a.G, G, sizeof(G));
-    memcpy(a.Gt, Gt, sizeof(Gt));
-    memcpy(a.P, proj_host, sizeof(a.P));
+    { const int rcf = nuc_fill_args(c, a, proj_host); if (rcf) return rcf; }
     double* partial = nullptr;
     const int npart = a.nblk_t * MDWF_NUC_WARPS;
     MDWF_CUDA(c, cudaMallocAsync(&partial, sizeof(double) * 2 * T * npart, st));
     a.partial = partial;
     dim3 grid(a.nblk_t, T);
-    const size_t nsm = (size_t)gpb * (5 * 144 + 16) * sizeof(double2);
+    const size_t nsm = MDWF_NUC_SMEM;
     if (!c->attr_raised.count((const void*)nucleon_kernel)) {
         MDWF_CUDA(c, cudaFuncSetAttribute(nucleon_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nsm));
         c->attr_raised.insert((const void*)nucleon_kernel);
@@ -393,7 +440,7 @@ int mdwf_nucleon_2pt_noalloc(mdwf_ctx* c, double* corr, const void* S_u1, const 
     a.Su1 = (const double2*)S_u1; a.Sd = (const double2*)S_d; a.Su2 = (const double2*)S_u2;
     a.V4 = 2ll * c->g.Vh; a.V3 = a.V4 / c->g.T;
     const int T = c->g.T;
-    const int gpb = MDWF_NUC_WARPS / MDWF_NUC_WPS;
+    const int gpb = MDWF_NUC_SPB;
     // the launch shape of mdwf_nucleon_2pt, so that the fixed-order sums are the same sums
     a.nblk_t = (int)std::min<long long>((a.V3 + gpb - 1) / gpb, std::max(1, (c->sm_count * 16) / T));
     const int npart = a.nblk_t * MDWF_NUC_WARPS;
@@ -401,21 +448,8 @@ int mdwf_nucleon_2pt_noalloc(mdwf_ctx* c, double* corr, const void* S_u1, const 
     if (need > MDWF_NUC_SCRATCH_DOUBLES)
         MDWF_FAIL(c, MDWF_EINVAL, "mdwf_nucleon_2pt_noalloc: T = %d with %d blocks per timeslice needs %lld bytes of scratch, the "
                   "static array holds %lld (use mdwf_nucleon_2pt)", T, a.nblk_t, need * 8, (long long)sizeof(double) * MDWF_NUC_SCRATCH_DOUBLES);
-    // C = gamma_y gamma_t, G = C gamma5, Gt = gamma_t G^dag gamma_t in the DeGrand-Rossi basis (SURVEY 8 Notation)
-    const double gy[32] = {0,0, 0,0, 0,0, -1,0,   0,0, 0,0, 1,0, 0,0,   0,0, 1,0, 0,0, 0,0,   -1,0, 0,0, 0,0, 0,0};
-    const double gt[32] = {0,0, 0,0, 1,0, 0,0,   0,0, 0,0, 0,0, 1,0,   1,0, 0,0, 0,0, 0,0,   0,0, 1,0, 0,0, 0,0};
-    const double g5[32] = {1,0, 0,0, 0,0, 0,0,   0,0, 1,0, 0,0, 0,0,   0,0, 0,0, -1,0, 0,0,   0,0, 0,0, 0,0, -1,0};
-    double C[32], G[32], Gd[32], Gt[32];
-    mat4mul(gy, gt, C);
-    mat4mul(C, g5, G);
-    for (int i = 0; i < 4; ++i)
-        for (int j = 0; j < 4; ++j) { Gd[2 * (4 * i + j)] = G[2 * (4 * j + i)]; Gd[2 * (4 * i + j) + 1] = -G[2 * (4 * j + i) + 1]; }
-    mat4mul(gt, Gd, Gt);
-    mat4mul(Gt, gt, Gt);
-    memcpy(a.G, G, sizeof(G));
-    memcpy(a.Gt, Gt, sizeof(Gt));
-    memcpy(a.P, proj_host, sizeof(a.P));
-    const size_t nsm = (size_t)gpb * (5 * 144 + 16) * sizeof(double2);
+    { const int rcf = nuc_fill_args(c, a, proj_host); if (rcf) return rcf; }
+    const size_t nsm = MDWF_NUC_SMEM;
     double* scratch = nullptr;
     int rc = nuc_noalloc_setup(c, nsm, &scratch);
     if (rc) return rc;

@@ -586,15 +586,25 @@ static int setup_solver(mdwf_ctx* c, Solver& S, const mdwf_solve_opts* opts, cud
     return MDWF_OK;
 }
 
-// batch size and number of rhs served by the fp64 temporaries that fit in `avail` bytes (beyond `extra_per_rhs`)
+// Batch size nb and number of rhs served by the fp64 temporaries (nhi) for `avail` bytes (beyond `extra_per_rhs` each).
+// As many rhs in flight as fit (that is what the kernels gain from); the temporaries only save a few chunked passes at
+// the reliable updates, so they may grow only while the workspace stays within half of `avail` -- a library-owned
+// workspace is cached between calls and must not starve the caller's own allocations.
 static int plan_batch(mdwf_ctx* c, const Solver& S, int nrhs, int want, size_t avail, size_t extra_per_rhs, bool own_src,
                       int* nb_out, int* nhi_out) {
     const Geom& g = c->g;
     int nb = want > 0 ? std::min(want, nrhs) : nrhs;
     for (; nb >= 1; --nb) {
-        for (int nhi = nb; nhi >= 1; nhi = nhi > 1 ? (nhi + 1) / 2 : 0) {
-            if (work_bytes(g, S.prec, S.px, nb, nhi, own_src) + extra_per_rhs * nb <= avail) { *nb_out = nb; *nhi_out = nhi; return MDWF_OK; }
-            if (nhi == 1) break;
+        if (work_bytes(g, S.prec, S.px, nb, 1, own_src) + extra_per_rhs * nb <= avail) {
+            int nhi = 1;
+            while (nhi < nb) {
+                const int next = std::min(nb, nhi * 2);
+                const size_t need = work_bytes(g, S.prec, S.px, nb, next, own_src) + extra_per_rhs * nb;
+                if (need > avail || (!c->ws_external && need > avail / 2)) break;
+                nhi = next;
+            }
+            *nb_out = nb; *nhi_out = nhi;
+            return MDWF_OK;
         }
         if (want > 0) break;    // an explicit batch is honoured or refused
     }

@@ -66,7 +66,7 @@ def test_noalloc_refuses_what_does_not_fit():
     from paper_1810_01609_b200.binding import lib
     cap = lib().mdwf_nucleon_2pt_noalloc_max_bytes()
     assert cap == 512 * 1024
-    dims = (2, 2, 2, 4098)          # one block per timeslice: 16 * T doubles = 524544 bytes > 512 KiB
+    dims = (2, 2, 2, 6556)          # one block per timeslice: 10 * T doubles = 524480 bytes > 512 KiB
     ctx = mdwf.Context(dims, 1, 1.3, 1.5, 0.5, 0.1)
     V4 = int(np.prod(dims))
     S = crandn((12, V4, 4, 3), 9200).cuda()
