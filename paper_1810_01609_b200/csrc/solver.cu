@@ -23,6 +23,7 @@
 #include <cmath>
 #include <algorithm>
 #include <cstring>
+#include <cstdlib>
 #include <string>
 
 namespace mdwf {
@@ -639,6 +640,11 @@ int solve_impl(mdwf_ctx* c, void* x, const void* b, int nrhs, const mdwf_solve_o
         const size_t slice = (size_t)2 * g.Vh * 24 * 8;
         H.slice_bytes = slice;
         H.ns = (int)std::max<size_t>(1, std::min<size_t>((size_t)g.Ls, ((size_t)3 << 29) / slice));
+        // test hook: MDWF_STAGE_SLICES=n forces chunks of n s-slices, so that small lattices exercise the chunked, double-buffered path
+        if (const char* ev = getenv("MDWF_STAGE_SLICES")) {
+            const int n = atoi(ev);
+            if (n >= 1) H.ns = std::min(n, g.Ls);
+        }
         if (opts->src_kind == 0 || opts->out_kind == 0) avail = avail > 2 * H.ns * slice ? avail - 2 * H.ns * slice : 0;
         per_rhs = (opts->src_kind ? in_per : 0) + (opts->out_kind ? out_per : 0);
     }

@@ -98,6 +98,30 @@ def test_host_buffer_solve_matches_device_solve():
     assert oracle.true_residual(p, U.numpy(), xh.numpy(), b.numpy()).max() <= 1e-10
 
 
+@pytest.mark.parametrize("slices", [1, 3])
+def test_host_buffer_solve_streams_in_chunks(slices, monkeypatch):
+    """mdwf_solve_host streams every right-hand side through two staging chunks of whole s-slices.  At test
+    sizes one chunk would hold all of Ls, so MDWF_STAGE_SLICES forces chunks of 1 and of 3 slices (Ls = 8: ragged last
+    chunk), with 3 rhs in batches of 2 (the chunk buffers are re-used across right-hand sides, batches, upload and
+    download).  Same packed fields, same solve: the result must equal the device-buffer solve bit for bit."""
+    import paper_1810_01609_b200 as mdwf
+    dims, Ls, mf = (4, 4, 4, 6), 8, 0.08
+    p = oracle.Params(dims=dims, Ls=Ls, M5=1.3, b5=1.5, c5=0.5, mf=mf, bc=(1, 1, 1, -1))
+    U = synth.gauge_field(dims, 0.3, 6101)
+    ctx = mdwf.Context(dims, Ls, 1.3, 1.5, 0.5, mf)
+    ctx.mdwf_load_gauge(U.cuda(), 64, 18)
+    ctx.mdwf_load_gauge(U.cuda(), 16, 12)
+    b = synth.gaussian_spinor(dims, Ls, 3, 6102)
+    kw = dict(tol=1e-9, inner_prec=16, recon=12, batch=2)
+    xd, rd = ctx.mdwf_solve(b.cuda(), **kw)
+    monkeypatch.setenv("MDWF_STAGE_SLICES", str(slices))
+    xh = torch.full(b.shape, float("nan"), dtype=b.dtype).pin_memory()
+    _, rh = ctx.mdwf_solve_host(b.pin_memory(), xh, **kw)
+    assert rd.status == mdwf.OK and rh.status == mdwf.OK and rh.iters == rd.iters
+    assert torch.equal(torch.view_as_real(xh), torch.view_as_real(xd.cpu()))
+    assert oracle.true_residual(p, U.numpy(), xh.numpy(), b.numpy()).max() <= 1e-9
+
+
 def test_not_converged_is_reported():
     mdwf, cfg, p, U, ctx, Ud = make(1)
     b = synth.gaussian_spinor(cfg.dims, cfg.Ls, 1, synth.seed_for(1, 2))
