@@ -205,7 +205,13 @@ int launch_hop_f16(mdwf_ctx* c, int recon, int dagger, int fused, HopArgs& a, cu
     const int regs = 128;
     const int per_sm = std::max(1, std::min(2048 / block, (int)((227 * 1024) / (tl.smem_total + 1024))));
     const int grid = (int)std::min<long long>((long long)tl.ntiles * tl.ngrp, (long long)c->sm_count * std::min(per_sm, 65536 / (regs * block)) );
-    auto kern = rows <= 16 ? hop16_kernel<1, 1, 1> : rows <= 32 ? hop16_kernel<2, 1, 1> : hop16_kernel<3, 1, 1>;
+    typedef void (*Kern16)(const Geom, const Tile16, const HopArgs, const int);
+    // (templating on the xpay input / the norm output as well was measured: no gain)
+    static const Kern16 kerns[3][3] = {{hop16_kernel<1, 1, 1, 0>, hop16_kernel<1, 1, 1, 1>, hop16_kernel<1, 1, 1, 2>},
+                                       {hop16_kernel<2, 1, 1, 0>, hop16_kernel<2, 1, 1, 1>, hop16_kernel<2, 1, 1, 2>},
+                                       {hop16_kernel<3, 1, 1, 0>, hop16_kernel<3, 1, 1, 1>, hop16_kernel<3, 1, 1, 2>}};
+    if (a.op.kind < 0 || a.op.kind > 2) MDWF_FAIL(c, MDWF_EINVAL, "internal: bad epilogue kind %d", a.op.kind);
+    const Kern16 kern = kerns[rows <= 16 ? 0 : rows <= 32 ? 1 : 2][a.op.kind];
     if (!c->attr_raised.count((const void*)kern)) {
         MDWF_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         c->attr_raised.insert((const void*)kern);

@@ -86,7 +86,9 @@ __device__ __forceinline__ void tile16_origin(const Tile16& tl, int tile, int o[
 //   so that the k16 operand pairs of the three n-tiles (= output colours) are aligned register pairs of two 16-byte
 //   loads; the five blocks sit in disjoint banks, so the 32 lanes of a fragment load never conflict.
 // MT = m16 tiles per site: ceil(RI * Ls / 16) <= 3
-template <int MT, int PF, int MINB>
+// KIND = LsOp kind of the fused epilogue (0: none, 1: c0 + c1 L, 2: c0 + c1 M5^-1), a template parameter so that each
+// instantiation carries only its own epilogue (registers, code size)
+template <int MT, int PF, int MINB, int KIND>
 __global__ void __launch_bounds__(PF ? 32 * MDWF_H16_MAXW : 256, MINB) hop16_kernel(const Geom g, const Tile16 tl, const HopArgs a, const int dag) {
     extern __shared__ __align__(128) unsigned char sm[];
     if (a.stop != nullptr && *a.stop != 0) return;
@@ -283,7 +285,7 @@ __global__ void __launch_bounds__(PF ? 32 * MDWF_H16_MAXW : 256, MINB) hop16_ker
                     *reinterpret_cast<float2*>(e0 + 8 * 24) = make_float2(acc[mt][n][2], acc[mt][n][3]);
                 }
             __syncwarp();
-            if (op.kind == 2) {
+            if (KIND == 2) {
                 // closed form of M5^-1 as a first-order recurrence along s (mdwf_hop.cuh, LsOp), one lane per column of a rhs:
                 // P_s = v_s + kappa P_{s-1} in place (forward for one chirality, backward for the other)
                 // (up to three columns per lane, advanced together so that their dependent load-fma-store chains overlap)
@@ -319,12 +321,12 @@ __global__ void __launch_bounds__(PF ? 32 * MDWF_H16_MAXW : 256, MINB) hop16_ker
                         const float chc = (float)a.ch * cf.x;                       // ch * e_in / e_out
                         const float* Er = E + (qd[qi] & 0xffff);                    // this rhs, this colour chunk, row s at + s*24
                         float o8[8];
-                        if (op.kind == 0) {
+                        if (KIND == 0) {
                             const float4 lo = *reinterpret_cast<const float4*>(Er + s * 24);
                             const float4 hi = *reinterpret_cast<const float4*>(Er + s * 24 + 4);
                             o8[0] = chc * lo.x; o8[1] = chc * lo.y; o8[2] = chc * lo.z; o8[3] = chc * lo.w;
                             o8[4] = chc * hi.x; o8[5] = chc * hi.y; o8[6] = chc * hi.z; o8[7] = chc * hi.w;
-                        } else if (op.kind == 1) {
+                        } else if (KIND == 1) {
                             const float c0f = (float)op.c0 * chc, c1f = (float)op.c1 * chc;
                             const int sm1 = s == 0 ? Ls - 1 : s - 1, sp1 = s == Ls - 1 ? 0 : s + 1;
                             const float fm = c1f * (s == 0 ? -mf : 1.f), fp = c1f * (s == Ls - 1 ? -mf : 1.f);
