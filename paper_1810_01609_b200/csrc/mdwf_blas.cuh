@@ -50,8 +50,9 @@ __device__ __forceinline__ void block_sum_rhs(double v, const RowWork& w, const 
     // grouped mode: one pass through shared memory, then thread j < RI sums the entries of rhs j in thread order (the
     // Ls threads of a (site, rhs) are consecutive and the rhs of a site follow each other, so thread t belongs to rhs
     // (first + t / Ls) mod RI): two barriers instead of 4 RI
+    // (no barrier before the first write: every earlier user of smem_raw in these kernels ends with one -- apply_ls -- or
+    // there is none; and none after the sums: the callers either end here or synchronise themselves)
     double* red = reinterpret_cast<double*>(smem_raw);
-    __syncthreads();
     red[threadIdx.x] = w.live ? v : 0.0;
     __syncthreads();
     const int RI = 1 << rl.ril;
@@ -66,17 +67,16 @@ __device__ __forceinline__ void block_sum_rhs(double v, const RowWork& w, const 
             partial[(long long)rl.slot_of[((w.grp << rl.ril) + j) & 63] * w.nblk + w.tile] = tot;
         }
     }
-    __syncthreads();
 }
 // 1 / scale of an fp16 output for this thread's rhs (see block_out_scale); grouped mode evaluates the rule once per rhs
 // of the group
-template <typename S>
+// (SLOT: a kernel that evaluates two rules uses a different slot for each, so that no barrier is needed before the write)
+template <typename S, int SLOT = 0>
 __device__ __forceinline__ typename Store<S>::real work_out_scale(const ScaleRule& sr, const RowWork& w, const RhsList& rl) {
     if constexpr (!Store<S>::HALF) return 1;
     else {
         if (rl.ril == 0 && rl.ng == 0) return block_out_scale<S>(sr, w.rhs, w.tile == 0);
         __shared__ float s_oinv4[4];
-        __syncthreads();
         if (threadIdx.x < (1u << rl.ril)) {
             const int gm = rl.gmask[blockIdx.x % rl.ng];
             s_oinv4[threadIdx.x] = (gm >> threadIdx.x) & 1 ? 1.0f / eval_scale(sr, (w.grp << rl.ril) + (int)threadIdx.x, w.tile == 0) : 1.0f;
@@ -266,7 +266,7 @@ __global__ void __launch_bounds__(256) cg_update_p_kernel(const Geom g, const Cg
     }
     if (a.op.kind != 0) {
         apply_ls<T>(pv, a.op, g.Ls, smem_raw);
-        const T oinv_q = work_out_scale<S>(a.sr_q, w, a.rl);
+        const T oinv_q = work_out_scale<S, 1>(a.sr_q, w, a.rl);
         if (live) store_spinor<S>(a.q, rhs, idx, g.N5h, pv, oinv_q);
     }
 }
