@@ -174,6 +174,8 @@ def test_c5_solve_all_four_rhs(c5):
     scratch = torch.empty((1, cfg.Ls, Vh, 4, 3), dtype=torch.complex128, device=dev)
     seed = synth.seed_for(5, 2)
     bench.fill_packed_rhs(psi, cfg, nrhs, seed, dev, scratch)
+    ctx.mdwf_autotune(16, 12, nrhs)             # as bench.py does: the launch parameters bench.py times
+    ctx.mdwf_autotune(64, 18, 1)
     ws = torch.empty(ctx.mdwf_workspace_bytes(nrhs, 16, packed=True), dtype=torch.uint8, device=dev)   # as bench.py does
     ctx.mdwf_set_workspace(ws)
     res = ctx.mdwf_solve_packed(psi[0], psi[1], tol=cfg.tol, inner_prec=16, recon=12, symmetric=True)
