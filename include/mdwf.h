@@ -137,8 +137,12 @@ typedef struct {
  * 5D.  Returns MDWF_OK, or MDWF_NOT_CONVERGED / MDWF_BREAKDOWN if any rhs ended that way. */
 int mdwf_solve(mdwf_ctx* ctx, void* x, const void* b, int nrhs, const mdwf_solve_opts* opts,
                mdwf_solve_info* info, void* stream);
-/* Same with HOST buffers (pageable or pinned): the call stages each batch host->device, solves,
- * and copies the result back; all copies are inside the call. */
+/* Same with HOST buffers (pageable or pinned; pinned lets the copies overlap the packing): all copies are inside the
+ * call.  5D right-hand sides and solutions are never held in canonical form on the device: they stream through two
+ * staging chunks of whole s-slices (<= 1.5 GB each, cudaMalloc'ed for the duration of the call) on a copy stream and are
+ * packed / unpacked as they pass, so as many right-hand sides are in flight as in mdwf_solve_packed (4 at 48^3x64x10).
+ * 4D sources / solutions (src_kind / out_kind = 1) are staged whole per batch.  x_host may alias b_host only if both are
+ * 5D.  MDWF_ENOMEM if workspace plus staging buffers do not fit. */
 int mdwf_solve_host(mdwf_ctx* ctx, void* x_host, const void* b_host, int nrhs, const mdwf_solve_opts* opts,
                     mdwf_solve_info* info, void* stream);
 
